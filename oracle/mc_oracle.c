@@ -1,0 +1,579 @@
+/*
+ * mc_oracle.c -- plain, slow, fp64, single-threaded ORACLE for the red-black checkerboard Metropolis
+ * sweep over unit classical Heisenberg spins (Lepadatu et al., arXiv 2103.03517).
+ *
+ * TEST INFRASTRUCTURE ONLY (see mc_oracle.h).  Shares no code with the CUDA path.
+ * It follows the paper's Tables A1 / A2 step by step, in the paper's order and notation; there is no
+ * blocking, fusion or reordering.  "P:NN" = line NN of /root/reference/PAPER.md.  "C-n" = reading n
+ * in DESIGN.md section 4 (points where the paper is silent, ambiguous or garbled).
+ *
+ * Parity status: "parity unpinned" at the bit level (the paper prints no worked numeric example);
+ * every function below is pinned by closed forms / invariants / brute force in tests/test_oracle_*.py.
+ */
+#include "mc_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define TAG_MOVE     0u   /* unconstrained trial move, keyed on the site                 */
+#define TAG_PAIR     1u   /* constrained pair move, keyed on the leader's site           */
+#define TAG_PAIRING  2u   /* pairing parameters of one (sweep, colour); site word = 0    */
+#define TAG_ORACLE  16u   /* oracle-only cross-check modes (random order, Fisher-Yates)  */
+
+static const double PI = 3.14159265358979323846;
+
+struct orc_ctx {
+    int nx, ny, nz, periodic[3];
+    int64_t N;
+    double J, Ku, eu[3], Kc, B[3];
+    uint8_t* mask;          /* NULL = all bonds allowed by the boundary conditions */
+    uint16_t* region;       /* NULL = uniform easy axis eu                         */
+    double* region_axis; int n_regions;
+    double cone; int adaptive;
+    uint64_t seed, sweep;
+    double* S;              /* [N][3] lexicographic: site = x + nx*(y + ny*z)       */
+    double last_acceptance;
+    /* accumulators (Eq. 6) */
+    uint64_t n_samples;
+    double sum_m[4], sum_m2[4], sum_E, sum_E2, sum_torque[3];
+    /* per-sweep trace */
+    double* trace; int64_t trace_len, trace_cap;
+    /* constrained state */
+    int aligned; double eC[3];
+    int sampling;           /* 1 = measure + trace + accumulate after every sweep (default) */
+};
+
+/* ------------------------------------------------------------------ Philox4x32-10 (pin P-1) */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)M0 * c0, p1 = (uint64_t)M1 * c2;
+        uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+        uint32_t n0 = hi1 ^ c1 ^ k0, n1 = lo1, n2 = hi0 ^ c3 ^ k1, n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += W0; k1 += W1;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* u = ((r>>9) + 0.5) * 2^-23: 24 significant bits, so identical in fp32 and fp64 (pin P-2, reading C-8). */
+double orc_uniform(uint32_t r) { return ((double)(r >> 9) + 0.5) * (1.0 / 8388608.0); }
+
+static void draw(const orc_ctx* c, uint32_t site, uint32_t tag, int colour, uint64_t sweep, uint32_t r[4])
+{
+    uint32_t ctr[4] = { site, tag | ((uint32_t)colour << 8), (uint32_t)sweep, (uint32_t)(sweep >> 32) };
+    uint32_t key[2] = { (uint32_t)c->seed, (uint32_t)(c->seed >> 32) };
+    orc_philox4x32_10(ctr, key, r);
+}
+
+/* ------------------------------------------------------------------ cone trial move (C-6, C-7) */
+void orc_cone_move(const double S[3], double theta, double u0, double u1, double Sn[3])
+{
+    /* polar angle alpha from S uniform in solid angle over the cap of half-angle theta: cos(alpha) = 1 - w */
+    double w = u0 * (1.0 - cos(theta));
+    double sa = sqrt(w * (2.0 - w));
+    double phi = 2.0 * PI * u1;
+    /* orthonormal frame (t1,t2) perpendicular to S (Duff et al. 2017 construction) */
+    double sg = (S[2] >= 0.0) ? 1.0 : -1.0;
+    double a = -1.0 / (sg + S[2]);
+    double b = S[0] * S[1] * a;
+    double t1[3] = { 1.0 + sg * S[0] * S[0] * a, sg * b, -sg * S[0] };
+    double t2[3] = { b, sg + S[1] * S[1] * a, -S[1] };
+    double cp = cos(phi), sp = sin(phi), v[3], n2 = 0.0;
+    for (int k = 0; k < 3; ++k) {
+        double d = -w * S[k] + sa * (cp * t1[k] + sp * t2[k]);
+        v[k] = S[k] + d;
+        n2 += v[k] * v[k];
+    }
+    double inv = 1.0 / sqrt(n2);
+    for (int k = 0; k < 3; ++k) Sn[k] = v[k] * inv;
+}
+
+/* ------------------------------------------------------------------ lattice helpers */
+static inline int64_t site_index(const orc_ctx* c, int x, int y, int z) { return x + (int64_t)c->nx * (y + (int64_t)c->ny * z); }
+
+/* neighbour of (x,y,z) in direction k = (+x,-x,+y,-y,+z,-z); -1 if there is no bond (open face or masked). */
+static int64_t neighbour(const orc_ctx* c, int x, int y, int z, int k)
+{
+    int p[3] = { x, y, z }, dim[3] = { c->nx, c->ny, c->nz };
+    int axis = k >> 1, step = (k & 1) ? -1 : +1;
+    int64_t self = site_index(c, x, y, z);
+    if (c->mask && !((c->mask[self] >> k) & 1)) return -1;
+    p[axis] += step;
+    if (p[axis] < 0 || p[axis] >= dim[axis]) {
+        if (!c->periodic[axis]) return -1;
+        p[axis] = (p[axis] + dim[axis]) % dim[axis];
+    }
+    return site_index(c, p[0], p[1], p[2]);
+}
+
+/* exchange field h_i = sum_{j in N_i} J S_j  (first term of Eq. 2; full J per bond, C-1) */
+static void exchange_field(const orc_ctx* c, int x, int y, int z, double h[3])
+{
+    h[0] = h[1] = h[2] = 0.0;
+    for (int k = 0; k < 6; ++k) {
+        int64_t j = neighbour(c, x, y, z, k);
+        if (j < 0) continue;
+        for (int a = 0; a < 3; ++a) h[a] += c->J * c->S[3 * j + a];
+    }
+}
+
+static const double* easy_axis(const orc_ctx* c, int64_t site)
+{
+    return c->region ? &c->region_axis[3 * (int64_t)c->region[site]] : c->eu;
+}
+
+/* E_i(S) of Eq. (2), given the exchange field h of site i */
+static double site_energy_h(const orc_ctx* c, int64_t site, const double h[3], const double S[3])
+{
+    const double* e = easy_axis(c, site);
+    double se = S[0] * e[0] + S[1] * e[1] + S[2] * e[2];
+    double x2 = S[0] * S[0], y2 = S[1] * S[1], z2 = S[2] * S[2];
+    return -(S[0] * h[0] + S[1] * h[1] + S[2] * h[2])
+           - c->Ku * se * se
+           + c->Kc * (x2 * y2 + x2 * z2 + y2 * z2)
+           - (S[0] * c->B[0] + S[1] * c->B[1] + S[2] * c->B[2]);
+}
+
+double orc_site_energy(const orc_ctx* c, int64_t site, const double S[3])
+{
+    int x = (int)(site % c->nx), y = (int)((site / c->nx) % c->ny), z = (int)(site / ((int64_t)c->nx * c->ny));
+    double h[3];
+    exchange_field(c, x, y, z, h);
+    return site_energy_h(c, site, h, S);
+}
+
+/* extensive H = -J sum_<ij> S_i.S_j + on-site terms, every bond visited ONCE via its + direction (C-1).
+ * Independent of exchange_field's 1/2-sum so that it can pin it (pin P-5). */
+double orc_total_energy(const orc_ctx* c)
+{
+    double E = 0.0;
+    for (int z = 0; z < c->nz; ++z) for (int y = 0; y < c->ny; ++y) for (int x = 0; x < c->nx; ++x) {
+        int64_t i = site_index(c, x, y, z);
+        const double* S = &c->S[3 * i];
+        for (int k = 0; k < 6; k += 2) {          /* +x, +y, +z only */
+            int64_t j = neighbour(c, x, y, z, k);
+            if (j < 0) continue;
+            const double* Sj = &c->S[3 * j];
+            E -= c->J * (S[0] * Sj[0] + S[1] * Sj[1] + S[2] * Sj[2]);
+        }
+        const double* e = easy_axis(c, i);
+        double se = S[0] * e[0] + S[1] * e[1] + S[2] * e[2];
+        double x2 = S[0] * S[0], y2 = S[1] * S[1], z2 = S[2] * S[2];
+        E += -c->Ku * se * se + c->Kc * (x2 * y2 + x2 * z2 + y2 * z2)
+             - (S[0] * c->B[0] + S[1] * c->B[1] + S[2] * c->B[2]);
+    }
+    return E;
+}
+
+/* ------------------------------------------------------------------ create / state */
+orc_ctx* orc_create(int nx, int ny, int nz, const int periodic[3],
+                    double J, double Ku, const double eu[3], double Kc, const double B[3],
+                    const uint8_t* bond_mask, const uint16_t* region,
+                    const double* region_axis, int n_regions,
+                    double cone0_rad, int adaptive, uint64_t seed)
+{
+    if (nx < 1 || ny < 1 || nz < 1) return NULL;
+    int dim[3] = { nx, ny, nz };
+    for (int a = 0; a < 3; ++a) if (periodic[a] && (dim[a] & 1)) return NULL;   /* two-colouring needs even periodic dims */
+    orc_ctx* c = (orc_ctx*)calloc(1, sizeof(orc_ctx));
+    c->nx = nx; c->ny = ny; c->nz = nz;
+    for (int a = 0; a < 3; ++a) c->periodic[a] = periodic[a];
+    c->N = (int64_t)nx * ny * nz;
+    c->J = J; c->Ku = Ku; c->Kc = Kc;
+    double n = sqrt(eu[0] * eu[0] + eu[1] * eu[1] + eu[2] * eu[2]);
+    for (int a = 0; a < 3; ++a) { c->eu[a] = (n > 0) ? eu[a] / n : (a == 2); c->B[a] = B[a]; }
+    if (bond_mask) { c->mask = (uint8_t*)malloc(c->N); memcpy(c->mask, bond_mask, c->N); }
+    if (region) {
+        c->region = (uint16_t*)malloc(2 * c->N); memcpy(c->region, region, 2 * c->N);
+        c->n_regions = n_regions;
+        c->region_axis = (double*)malloc(sizeof(double) * 3 * n_regions);
+        for (int r = 0; r < n_regions; ++r) {
+            const double* v = &region_axis[3 * r];
+            double m = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+            for (int a = 0; a < 3; ++a) c->region_axis[3 * r + a] = v[a] / m;
+        }
+    }
+    c->cone = cone0_rad; c->adaptive = adaptive; c->seed = seed; c->sweep = 0; c->sampling = 1;
+    c->S = (double*)malloc(sizeof(double) * 3 * c->N);
+    for (int64_t i = 0; i < c->N; ++i) { c->S[3 * i] = 0; c->S[3 * i + 1] = 0; c->S[3 * i + 2] = 1; }
+    return c;
+}
+
+void orc_destroy(orc_ctx* c)
+{
+    if (!c) return;
+    free(c->mask); free(c->region); free(c->region_axis); free(c->S); free(c->trace); free(c);
+}
+
+void orc_set_spins(orc_ctx* c, const double* xyz) { memcpy(c->S, xyz, sizeof(double) * 3 * c->N); c->aligned = 0; }
+void orc_set_spins_f32(orc_ctx* c, const float* xyz) { for (int64_t i = 0; i < 3 * c->N; ++i) c->S[i] = (double)xyz[i]; c->aligned = 0; }
+void orc_get_spins(const orc_ctx* c, double* xyz) { memcpy(xyz, c->S, sizeof(double) * 3 * c->N); }
+void orc_init_uniform(orc_ctx* c, const double dir[3])
+{
+    double n = sqrt(dir[0] * dir[0] + dir[1] * dir[1] + dir[2] * dir[2]);
+    for (int64_t i = 0; i < c->N; ++i) for (int a = 0; a < 3; ++a) c->S[3 * i + a] = dir[a] / n;
+    c->aligned = 0;
+}
+void orc_set_cone(orc_ctx* c, double cone) { c->cone = cone; }
+void orc_set_sweep(orc_ctx* c, uint64_t s) { c->sweep = s; }
+void orc_set_adaptive(orc_ctx* c, int a) { c->adaptive = a; }
+void orc_set_sampling(orc_ctx* c, int on) { c->sampling = on; }
+
+/* ------------------------------------------------------------------ Table A1: one colour pass */
+static int metropolis_update(orc_ctx* c, int x, int y, int z, int colour, double T, double* xdec)
+{
+    int64_t i = site_index(c, x, y, z);                       /* P:155  i = Get_Red(Black)SpinIndex(index) */
+    uint32_t r[4];
+    draw(c, (uint32_t)i, TAG_MOVE, colour, c->sweep, r);
+    double u0 = orc_uniform(r[0]), u1 = orc_uniform(r[1]), u2 = orc_uniform(r[2]);
+    double* S = &c->S[3 * i], Sn[3], h[3];
+    orc_cone_move(S, c->cone, u0, u1, Sn);                    /* P:156  S_new = UniformRandom_RotateSpin(S_i, theta) */
+    exchange_field(c, x, y, z, h);
+    double dE = site_energy_h(c, i, h, Sn) - site_energy_h(c, i, h, S);   /* P:158  E(S_new) - E(S_i) */
+    double xd = dE / T + log(u2);                             /* P:157-158  P < exp(-dE/kT)  <=>  dE/T + ln P < 0  (C-8) */
+    if (xdec) xdec[i] = xd;
+    if (xd < 0.0) { S[0] = Sn[0]; S[1] = Sn[1]; S[2] = Sn[2]; return 1; }
+    return 0;
+}
+
+int64_t orc_half_sweep(orc_ctx* c, double T, int colour, double* xdec, uint8_t* acc)
+{
+    int64_t count = 0;
+    for (int z = 0; z < c->nz; ++z) for (int y = 0; y < c->ny; ++y) for (int x = 0; x < c->nx; ++x) {
+        if (((x + y + z) & 1) != colour) continue;            /* red = even (C-10) */
+        int a = metropolis_update(c, x, y, z, colour, T, xdec);
+        if (acc) acc[site_index(c, x, y, z)] = (uint8_t)a;
+        count += a;
+    }
+    return count;
+}
+
+/* ------------------------------------------------------------------ observables (Eq. 6) */
+static void measure(const orc_ctx* c, orc_obs* o)
+{
+    double M[3] = { 0, 0, 0 }, Eex = 0, Ean = 0, Ez = 0, tq[3] = { 0, 0, 0 };
+    for (int z = 0; z < c->nz; ++z) for (int y = 0; y < c->ny; ++y) for (int x = 0; x < c->nx; ++x) {
+        int64_t i = site_index(c, x, y, z);
+        const double* S = &c->S[3 * i];
+        double h[3];
+        exchange_field(c, x, y, z, h);
+        for (int a = 0; a < 3; ++a) M[a] += S[a];
+        Eex += -0.5 * (S[0] * h[0] + S[1] * h[1] + S[2] * h[2]);          /* every bond once (C-1) */
+        const double* e = easy_axis(c, i);
+        double se = S[0] * e[0] + S[1] * e[1] + S[2] * e[2];
+        double x2 = S[0] * S[0], y2 = S[1] * S[1], z2 = S[2] * S[2];
+        Ean += -c->Ku * se * se + c->Kc * (x2 * y2 + x2 * z2 + y2 * z2);
+        Ez  += -(S[0] * c->B[0] + S[1] * c->B[1] + S[2] * c->B[2]);
+        /* on-site field H = -dE_i/dS_i (anisotropy + Zeeman); torque = S x H */
+        double H[3] = {
+            2.0 * c->Ku * se * e[0] - 2.0 * c->Kc * S[0] * (y2 + z2) + c->B[0],
+            2.0 * c->Ku * se * e[1] - 2.0 * c->Kc * S[1] * (x2 + z2) + c->B[1],
+            2.0 * c->Ku * se * e[2] - 2.0 * c->Kc * S[2] * (x2 + y2) + c->B[2] };
+        tq[0] += S[1] * H[2] - S[2] * H[1];
+        tq[1] += S[2] * H[0] - S[0] * H[2];
+        tq[2] += S[0] * H[1] - S[1] * H[0];
+    }
+    double invN = 1.0 / (double)c->N;
+    for (int a = 0; a < 3; ++a) { o->M[a] = M[a] * invN; o->torque[a] = tq[a] * invN; }
+    o->m = sqrt(o->M[0] * o->M[0] + o->M[1] * o->M[1] + o->M[2] * o->M[2]);
+    o->E_exch = Eex * invN; o->E_aniso = Ean * invN; o->E_zeeman = Ez * invN;
+    o->E_total = o->E_exch + o->E_aniso + o->E_zeeman;
+}
+
+void orc_end_sweep(orc_ctx* c, int64_t count)
+{
+    c->last_acceptance = (double)count / (double)c->N;
+    double cone_used = c->cone;
+    if (c->adaptive) {                                        /* P:168-171 read with P:205-209 (C-2, C-3, C-9) */
+        const double deg = PI / 180.0;
+        if (2 * count > c->N) { c->cone += deg; if (c->cone > PI) c->cone = PI; }
+        else                  { c->cone -= deg; if (c->cone < deg) c->cone = deg; }
+    }
+    c->sweep += 1;
+    if (!c->sampling) return;
+    orc_obs o; memset(&o, 0, sizeof o);
+    measure(c, &o);
+    double mv[4] = { o.m, o.M[0], o.M[1], o.M[2] };
+    for (int a = 0; a < 4; ++a) { c->sum_m[a] += mv[a]; c->sum_m2[a] += mv[a] * mv[a]; }
+    c->sum_E += o.E_total; c->sum_E2 += o.E_total * o.E_total;
+    for (int a = 0; a < 3; ++a) c->sum_torque[a] += o.torque[a];
+    c->n_samples += 1;
+    if (c->trace_len == c->trace_cap) {
+        c->trace_cap = c->trace_cap ? 2 * c->trace_cap : 1024;
+        c->trace = (double*)realloc(c->trace, sizeof(double) * 6 * c->trace_cap);
+    }
+    double* row = &c->trace[6 * c->trace_len++];
+    row[0] = c->last_acceptance; row[1] = cone_used; row[2] = o.M[0]; row[3] = o.M[1]; row[4] = o.M[2]; row[5] = o.E_total;
+}
+
+void orc_sweep(orc_ctx* c, double T, int64_t n)
+{
+    for (int64_t it = 0; it < n; ++it) {
+        int64_t count = orc_half_sweep(c, T, 0, NULL, NULL);
+        count += orc_half_sweep(c, T, 1, NULL, NULL);
+        orc_end_sweep(c, count);
+    }
+}
+
+/* serial Metropolis with a random visiting order -- only for the "serial == parallel" pin */
+void orc_sweep_random_order(orc_ctx* c, double T, int64_t n)
+{
+    int64_t* order = (int64_t*)malloc(sizeof(int64_t) * c->N);
+    for (int64_t it = 0; it < n; ++it) {
+        for (int64_t i = 0; i < c->N; ++i) order[i] = i;
+        for (int64_t i = c->N - 1; i > 0; --i) {
+            uint32_t r[4]; draw(c, (uint32_t)i, TAG_ORACLE, 0, c->sweep, r);
+            int64_t j = (int64_t)(((uint64_t)r[0] * (uint64_t)(i + 1)) >> 32);
+            int64_t t = order[i]; order[i] = order[j]; order[j] = t;
+        }
+        int64_t count = 0;
+        for (int64_t k = 0; k < c->N; ++k) {
+            int64_t s = order[k];
+            int x = (int)(s % c->nx), y = (int)((s / c->nx) % c->ny), z = (int)(s / ((int64_t)c->nx * c->ny));
+            count += metropolis_update(c, x, y, z, (x + y + z) & 1, T, NULL);
+        }
+        orc_end_sweep(c, count);
+    }
+    free(order);
+}
+
+/* ------------------------------------------------------------------ constrained MC (Table A2) */
+
+/* colour-linear index: a = (x>>1) + (nx/2)*(y + ny*z) enumerates the sites of one colour (nx even). */
+int64_t orc_site_of(const orc_ctx* c, int colour, int64_t a)
+{
+    int hx = c->nx / 2;
+    int xh = (int)(a % hx); int64_t row = a / hx;
+    int y = (int)(row % c->ny), z = (int)(row / c->ny);
+    int x = 2 * xh + ((colour + y + z) & 1);
+    return site_index(c, x, y, z);
+}
+
+/* Pairing of one (sweep, colour): reading C-11.
+ *   B = largest power of two <= 32 with 2B | Nc;  H = Nc/B chunks of B consecutive colour-linear indices;
+ *   Bl = min(B,4), Bh = B/Bl;
+ *   (r0,r1,r2,.) = Philox(ctr = (0, TAG_PAIRING | colour<<8, sweep_lo, sweep_hi));
+ *   m = 2*floor(r0*(H/2)/2^32) + 1 (odd);  sigma = r1 & 1;  r = r2 mod Bl;  q = (r2 >> 2) mod Bh;
+ *   index a = chunk*B + hi*Bl + lo is a LEADER iff chunk mod 2 == sigma; its follower is
+ *   ((chunk+m) mod H)*B + ((hi+q) mod Bh)*Bl + (lo+r) mod Bl.
+ * Replaces the paper's shuffled index array; requirements R1-R4 in DESIGN.md. */
+int orc_pairing(const orc_ctx* c, uint64_t sweep, int colour, int64_t* partner, uint8_t* is_leader)
+{
+    if (c->nx & 1) return -1;
+    int64_t Nc = c->N / 2;
+    if (Nc & 1) return -1;                                   /* C-15 */
+    int64_t B = 32; while (Nc % (2 * B)) B >>= 1;
+    int64_t H = Nc / B;
+    uint32_t r[4]; draw(c, 0u, TAG_PAIRING, colour, sweep, r);
+    int64_t m = 2 * (int64_t)(((uint64_t)r[0] * (uint64_t)(H / 2)) >> 32) + 1;
+    int64_t sigma = r[1] & 1u;
+    int64_t Bl = B < 4 ? B : 4, Bh = B / Bl;
+    int64_t rot = (int64_t)(r[2] % (uint32_t)Bl), q = (int64_t)((r[2] >> 2) % (uint32_t)Bh);
+    for (int64_t a = 0; a < Nc; ++a) {
+        int64_t chunk = a / B, e = a % B, hi = e / Bl, lo = e % Bl;
+        if ((chunk & 1) == sigma) {
+            int64_t f = ((chunk + m) % H) * B + ((hi + q) % Bh) * Bl + (lo + rot) % Bl;
+            is_leader[a] = 1; partner[a] = f;
+            is_leader[f] = 0; partner[f] = a;
+        }
+    }
+    return 0;
+}
+
+int orc_align_to(orc_ctx* c, const double eC[3])
+{
+    double M[3] = { 0, 0, 0 };
+    for (int64_t i = 0; i < c->N; ++i) for (int a = 0; a < 3; ++a) M[a] += c->S[3 * i + a];
+    double m = sqrt(M[0] * M[0] + M[1] * M[1] + M[2] * M[2]);
+    if (m / (double)c->N < 1e-6) return -1;
+    double u[3] = { M[0] / m, M[1] / m, M[2] / m };
+    /* Rodrigues rotation about k = u x eC by the angle between u and eC */
+    double k[3] = { u[1] * eC[2] - u[2] * eC[1], u[2] * eC[0] - u[0] * eC[2], u[0] * eC[1] - u[1] * eC[0] };
+    double s = sqrt(k[0] * k[0] + k[1] * k[1] + k[2] * k[2]);
+    double co = u[0] * eC[0] + u[1] * eC[1] + u[2] * eC[2];
+    if (s < 1e-300) {
+        if (co > 0) { c->aligned = 1; memcpy(c->eC, eC, sizeof c->eC); return 0; }   /* already aligned */
+        /* antiparallel: rotate by pi about any axis perpendicular to u */
+        double t[3] = { 1, 0, 0 }; if (fabs(u[0]) > 0.9) { t[0] = 0; t[1] = 1; }
+        k[0] = u[1] * t[2] - u[2] * t[1]; k[1] = u[2] * t[0] - u[0] * t[2]; k[2] = u[0] * t[1] - u[1] * t[0];
+        s = sqrt(k[0] * k[0] + k[1] * k[1] + k[2] * k[2]);
+        for (int a = 0; a < 3; ++a) k[a] /= s;
+        s = 0.0;
+    } else {
+        for (int a = 0; a < 3; ++a) k[a] /= s;
+    }
+    for (int64_t i = 0; i < c->N; ++i) {
+        double* S = &c->S[3 * i];
+        double kxS[3] = { k[1] * S[2] - k[2] * S[1], k[2] * S[0] - k[0] * S[2], k[0] * S[1] - k[1] * S[0] };
+        double kS = k[0] * S[0] + k[1] * S[1] + k[2] * S[2];
+        double v[3], n2 = 0;
+        for (int a = 0; a < 3; ++a) { v[a] = S[a] * co + kxS[a] * s + k[a] * kS * (1.0 - co); n2 += v[a] * v[a]; }
+        double inv = 1.0 / sqrt(n2);
+        for (int a = 0; a < 3; ++a) S[a] = v[a] * inv;
+    }
+    c->aligned = 1; memcpy(c->eC, eC, sizeof c->eC);
+    return 0;
+}
+
+/* one pair move, written frame-free: X_par = X.eC, X_perp = X - X_par eC (C-22). */
+static int pair_update(orc_ctx* c, double T, const double e[3], int colour, int64_t si, int64_t sj,
+                       double* ML, int ml_mode, double* xdec, int may_be_neighbours)
+{
+    uint32_t r[4];
+    draw(c, (uint32_t)si, TAG_PAIR, colour, c->sweep, r);
+    double u0 = orc_uniform(r[0]), u1 = orc_uniform(r[1]), u2 = orc_uniform(r[2]);
+    double *Si = &c->S[3 * si], *Sj = &c->S[3 * sj], Sni[3], Snj[3];
+    orc_cone_move(Si, c->cone, u0, u1, Sni);
+    double Si_par = Si[0] * e[0] + Si[1] * e[1] + Si[2] * e[2];
+    double Sj_par = Sj[0] * e[0] + Sj[1] * e[1] + Sj[2] * e[2];
+    double Sni_par = Sni[0] * e[0] + Sni[1] * e[1] + Sni[2] * e[2];
+    double perp[3], p2 = 0;
+    for (int a = 0; a < 3; ++a) {                                         /* P:187-188 transverse compensation */
+        perp[a] = (Sj[a] - Sj_par * e[a]) + (Si[a] - Si_par * e[a]) - (Sni[a] - Sni_par * e[a]);
+        p2 += perp[a] * perp[a];
+    }
+    double xd = INFINITY;
+    int accept = 0;
+    double rho = 1.0 - p2;                                                /* P:189 radicand (|S_j| = 1) */
+    double MLhat = *ML;
+    if (rho > 0.0) {                                                      /* C-13 */
+        double Snj_par = ((Sj_par >= 0.0) ? 1.0 : -1.0) * sqrt(rho);      /* P:189 sign kept */
+        double n2 = 0;
+        for (int a = 0; a < 3; ++a) { Snj[a] = perp[a] + Snj_par * e[a]; n2 += Snj[a] * Snj[a]; }
+        double inv = 1.0 / sqrt(n2);
+        for (int a = 0; a < 3; ++a) Snj[a] *= inv;
+        MLhat = *ML + Sni_par + Snj_par - Si_par - Sj_par;
+        if (MLhat > 0.0) {                                                /* C-13 */
+            int xi = (int)(si % c->nx), yi = (int)((si / c->nx) % c->ny), zi = (int)(si / ((int64_t)c->nx * c->ny));
+            int xj = (int)(sj % c->nx), yj = (int)((sj / c->nx) % c->ny), zj = (int)(sj / ((int64_t)c->nx * c->ny));
+            double hi[3], hj[3];
+            exchange_field(c, xi, yi, zi, hi);
+            exchange_field(c, xj, yj, zj, hj);
+            double dE = site_energy_h(c, si, hi, Sni) + site_energy_h(c, sj, hj, Snj)
+                      - site_energy_h(c, si, hi, Si) - site_energy_h(c, sj, hj, Sj);   /* P:193 (C-4) */
+            if (may_be_neighbours) {
+                /* serial Ref.[15] cross-check only: i and j may share a bond, so the change of the pair energy
+                 * is evaluated sequentially (move i in the old field, then j in the field that already holds S'_i) */
+                double keep[3] = { Si[0], Si[1], Si[2] };
+                double dEi = site_energy_h(c, si, hi, Sni) - site_energy_h(c, si, hi, Si);
+                Si[0] = Sni[0]; Si[1] = Sni[1]; Si[2] = Sni[2];
+                exchange_field(c, xj, yj, zj, hj);
+                dE = dEi + site_energy_h(c, sj, hj, Snj) - site_energy_h(c, sj, hj, Sj);
+                Si[0] = keep[0]; Si[1] = keep[1]; Si[2] = keep[2];
+            }
+            double ratio = MLhat / *ML;
+            /* P < (MLhat/ML)^2 |S_j,par / S'_j,par| exp(-dE/kT), in log form */
+            xd = dE / T - 2.0 * log(ratio) - log(fabs(Sj_par / Snj_par)) + log(u2);
+            accept = (xd < 0.0);
+        }
+    }
+    if (xdec) xdec[si] = xd;
+    if (accept) {
+        for (int a = 0; a < 3; ++a) { Si[a] = Sni[a]; Sj[a] = Snj[a]; }
+        if (ml_mode == 1) *ML = MLhat;                                    /* serial Ref.[15] variant only */
+    }
+    return accept;
+}
+
+int64_t orc_constrained_half_sweep(orc_ctx* c, double T, const double eC[3], int colour, double* ML,
+                                   int ml_mode, int pairing_mode, double* xdec, uint8_t* acc)
+{
+    int64_t Nc = c->N / 2, count = 0;
+    int64_t* partner = (int64_t*)malloc(sizeof(int64_t) * Nc);
+    uint8_t* leader = (uint8_t*)calloc(Nc, 1);
+    if (pairing_mode == 0) {
+        if (orc_pairing(c, c->sweep, colour, partner, leader)) { free(partner); free(leader); return -1; }
+    } else {
+        /* literal P:38 / P:202: shuffle the indexes of this colour, then pick them sequentially in pairs */
+        int64_t* p = (int64_t*)malloc(sizeof(int64_t) * Nc);
+        for (int64_t a = 0; a < Nc; ++a) p[a] = a;
+        for (int64_t a = Nc - 1; a > 0; --a) {
+            uint32_t r[4]; draw(c, (uint32_t)a, TAG_ORACLE, 2 + colour, c->sweep, r);
+            int64_t j = (int64_t)(((uint64_t)r[0] * (uint64_t)(a + 1)) >> 32);
+            int64_t t = p[a]; p[a] = p[j]; p[j] = t;
+        }
+        for (int64_t a = 0; a + 1 < Nc; a += 2) { leader[p[a]] = 1; partner[p[a]] = p[a + 1]; leader[p[a + 1]] = 0; partner[p[a + 1]] = p[a]; }
+        free(p);
+    }
+    for (int64_t a = 0; a < Nc; ++a) {                                    /* P:184 for i in 1..N step 2 */
+        if (!leader[a]) continue;
+        int64_t si = orc_site_of(c, colour, a), sj = orc_site_of(c, colour, partner[a]);
+        int ok = pair_update(c, T, eC, colour, si, sj, ML, ml_mode, xdec, 0);
+        if (acc) { acc[si] = (uint8_t)ok; acc[sj] = (uint8_t)ok; }
+        count += 2 * ok;                                                  /* P:195 (C-23) */
+    }
+    free(partner); free(leader);
+    return count;
+}
+
+/* Serial constrained MC of Ref.[15] ("the serial version as introduced in Ref. [15]"): pairs drawn from ALL
+ * sites regardless of colour (Fisher-Yates over the whole lattice), exact M_L.  Cross-check mode only: it has
+ * neither of the parallel algorithm's approximations (stale M_L, same-colour pairs), so on tiny lattices it must
+ * reproduce the unconstrained ensemble's rotation-invariant observables exactly (pin P-17a). */
+static int64_t serial_any_pair_sweep(orc_ctx* c, double T, const double e[3], double* ML)
+{
+    int64_t N = c->N, count = 0;
+    int64_t* p = (int64_t*)malloc(sizeof(int64_t) * N);
+    for (int64_t a = 0; a < N; ++a) p[a] = a;
+    for (int64_t a = N - 1; a > 0; --a) {
+        uint32_t r[4]; draw(c, (uint32_t)a, TAG_ORACLE, 4, c->sweep, r);
+        int64_t j = (int64_t)(((uint64_t)r[0] * (uint64_t)(a + 1)) >> 32);
+        int64_t t = p[a]; p[a] = p[j]; p[j] = t;
+    }
+    for (int64_t a = 0; a + 1 < N; a += 2) {
+        int64_t si = p[a], sj = p[a + 1];
+        int x = (int)(si % c->nx), y = (int)((si / c->nx) % c->ny), z = (int)(si / ((int64_t)c->nx * c->ny));
+        count += 2 * pair_update(c, T, e, (x + y + z) & 1, si, sj, ML, 1, NULL, 1);
+    }
+    free(p);
+    return count;
+}
+
+int orc_constrained_sweep(orc_ctx* c, double T, double theta, double phi, int64_t n, int ml_mode, int pairing_mode)
+{
+    double e[3] = { sin(theta) * cos(phi), sin(theta) * sin(phi), cos(theta) };
+    if (!c->aligned || e[0] != c->eC[0] || e[1] != c->eC[1] || e[2] != c->eC[2])
+        if (orc_align_to(c, e)) return -1;                                /* C-12 */
+    for (int64_t it = 0; it < n; ++it) {
+        double ML = 0.0;
+        for (int64_t i = 0; i < c->N; ++i) ML += c->S[3 * i] * e[0] + c->S[3 * i + 1] * e[1] + c->S[3 * i + 2] * e[2];
+        if (!(ML > 0.0)) return -1;
+        if (pairing_mode == 2) { orc_end_sweep(c, serial_any_pair_sweep(c, T, e, &ML)); continue; }
+        int64_t count = orc_constrained_half_sweep(c, T, e, 0, &ML, ml_mode, pairing_mode, NULL, NULL);
+        int64_t cb    = orc_constrained_half_sweep(c, T, e, 1, &ML, ml_mode, pairing_mode, NULL, NULL);   /* P:204 (C-5) */
+        if (count < 0 || cb < 0) return -1;
+        orc_end_sweep(c, count + cb);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------ read-out */
+void orc_observables(orc_ctx* c, orc_obs* o)
+{
+    memset(o, 0, sizeof *o);
+    measure(c, o);
+    o->n_sites = (uint64_t)c->N; o->sweep = c->sweep; o->cone_rad = c->cone; o->last_acceptance = c->last_acceptance;
+    o->n_samples = c->n_samples;
+    for (int a = 0; a < 4; ++a) { o->sum_m[a] = c->sum_m[a]; o->sum_m2[a] = c->sum_m2[a]; }
+    o->sum_E = c->sum_E; o->sum_E2 = c->sum_E2;
+    for (int a = 0; a < 3; ++a) o->sum_torque[a] = c->sum_torque[a];
+}
+
+void orc_reset_accumulators(orc_ctx* c)
+{
+    c->n_samples = 0;
+    memset(c->sum_m, 0, sizeof c->sum_m); memset(c->sum_m2, 0, sizeof c->sum_m2);
+    c->sum_E = c->sum_E2 = 0; memset(c->sum_torque, 0, sizeof c->sum_torque);
+}
+
+int64_t orc_trace(const orc_ctx* c, int64_t max, double* rows)
+{
+    int64_t k = c->trace_len < max ? c->trace_len : max;
+    memcpy(rows, &c->trace[6 * (c->trace_len - k)], sizeof(double) * 6 * k);
+    return k;
+}

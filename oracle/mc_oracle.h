@@ -1,0 +1,105 @@
+/*
+ * mc_oracle.h -- C interface of the fp64 serial ORACLE for the checkerboard Metropolis path.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Nothing outside tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may import, call, link or execute anything under oracle/.
+ * It shares no code with the CUDA path (paper_2103_03517_b200/csrc/): no headers, helpers,
+ * tables or constants.  Both sides restate the same written contract.
+ *
+ * Citations "P:NN" are line numbers of /root/reference/PAPER.md (Lepadatu et al., arXiv 2103.03517).
+ *
+ * Parity status: the paper prints no numeric worked example of a single update or sweep, so the
+ * bit-level update sequence is "parity unpinned"; every arithmetic piece is pinned by closed forms,
+ * invariants and brute force in tests/test_oracle_*.py.
+ */
+#ifndef MC_ORACLE_H
+#define MC_ORACLE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct orc_ctx orc_ctx;
+
+/* Per-sweep observables, all fp64, intensive quantities are per site. */
+typedef struct {
+    uint64_t n_sites, sweep;
+    double cone_rad, last_acceptance;
+    double M[3];            /* sum_i S_i / N                                     */
+    double m;               /* |M|                                               */
+    double E_total, E_exch, E_aniso, E_zeeman;   /* per site, bonds counted once */
+    double torque[3];       /* sum_i S_i x (on-site field) / N                   */
+    uint64_t n_samples;
+    double sum_m[4], sum_m2[4];   /* alpha = l,x,y,z  (Eq. 6)              */
+    double sum_E, sum_E2;
+    double sum_torque[3];
+} orc_obs;
+
+/* Philox4x32-10 (Salmon et al., SC'11), exposed for the known-answer pin. */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+/* Uniform in (0,1): ((r >> 9) + 0.5) * 2^-23. */
+double orc_uniform(uint32_t r);
+/* Cone trial move: S unit, theta = cone half-angle, u0,u1 in (0,1). */
+void orc_cone_move(const double S[3], double theta, double u0, double u1, double Snew[3]);
+
+/* mask: optional [N] bits (+x,-x,+y,-y,+z,-z); region: optional [N]; region_axis: [n_regions][3]. */
+orc_ctx* orc_create(int nx, int ny, int nz, const int periodic[3],
+                    double J, double Ku, const double eu[3], double Kc, const double B[3],
+                    const uint8_t* bond_mask, const uint16_t* region,
+                    const double* region_axis, int n_regions,
+                    double cone0_rad, int adaptive, uint64_t seed);
+void orc_destroy(orc_ctx*);
+
+void orc_set_spins(orc_ctx*, const double* xyz /* [N][3] lexicographic */);
+void orc_set_spins_f32(orc_ctx*, const float* xyz);
+void orc_get_spins(const orc_ctx*, double* xyz);
+void orc_init_uniform(orc_ctx*, const double dir[3]);
+void orc_set_cone(orc_ctx*, double cone_rad);
+void orc_set_sweep(orc_ctx*, uint64_t sweep);
+void orc_set_adaptive(orc_ctx*, int adaptive);
+/* 0 = skip the per-sweep measurement / trace / accumulators (long equilibrations in the pins). */
+void orc_set_sampling(orc_ctx*, int on);
+
+/* One colour pass of Table A1.  Does not advance the sweep counter.
+ * xdec[N] (optional): decision variable x = dE/T + ln u2 at the sites of this colour.
+ * acc[N]  (optional): 1 where the move was accepted.  Returns the accepted count. */
+int64_t orc_half_sweep(orc_ctx*, double T, int colour, double* xdec, uint8_t* acc);
+/* Controller + sweep counter + trace + accumulators, count = accepted in both passes. */
+void orc_end_sweep(orc_ctx*, int64_t count);
+/* n repetitions of: red pass, black pass, end_sweep. */
+void orc_sweep(orc_ctx*, double T, int64_t n);
+/* Serial Metropolis, random visiting order -- cross-check mode only. */
+void orc_sweep_random_order(orc_ctx*, double T, int64_t n);
+
+/* Pairing function of the constrained pass (reading C-11).
+ * Writes for every colour-linear index a in [0,Nc): partner[a] (colour-linear) and is_leader[a]. */
+int orc_pairing(const orc_ctx*, uint64_t sweep, int colour, int64_t* partner, uint8_t* is_leader);
+/* Colour-linear index a <-> lexicographic site. */
+int64_t orc_site_of(const orc_ctx*, int colour, int64_t a);
+
+/* Rigid rotation of all spins taking M/|M| onto e_C (reading C-12).  Returns 0, or -1 if |M|/N < 1e-6. */
+int orc_align_to(orc_ctx*, const double eC[3]);
+/* One colour pass of Table A2 with fixed M_L.
+ * mode 0 = stale M_L (the paper's parallel algorithm);  1 = exact M_L updated after every accepted pair (serial, Ref.[15]).
+ * pairing_mode 0 = analytic pairing; 1 = Fisher-Yates shuffle of the colour (literal P:38);
+ * (orc_constrained_sweep only) 2 = serial Ref.[15]: pairs from all sites regardless of colour, exact M_L. */
+int64_t orc_constrained_half_sweep(orc_ctx*, double T, const double eC[3], int colour, double* ML,
+                                   int ml_mode, int pairing_mode, double* xdec, uint8_t* acc);
+/* n repetitions of P:201-209 with e_C = (sin t cos p, sin t sin p, cos t); aligns on first use / direction change. */
+int orc_constrained_sweep(orc_ctx*, double T, double theta, double phi, int64_t n, int ml_mode, int pairing_mode);
+
+void orc_observables(orc_ctx*, orc_obs* out);
+void orc_reset_accumulators(orc_ctx*);
+/* rows [k][6]: acceptance, cone, mx, my, mz, E_total.  Returns number of rows written (most recent <= max). */
+int64_t orc_trace(const orc_ctx*, int64_t max, double* rows);
+
+/* Independent checks used by the pins. */
+double orc_site_energy(const orc_ctx*, int64_t site, const double S[3]);   /* E_i of Eq.(2) */
+double orc_total_energy(const orc_ctx*);   /* extensive H: every bond once + on-site terms */
+
+#ifdef __cplusplus
+}
+#endif
+#endif
