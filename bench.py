@@ -1,0 +1,259 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark: checkerboard Metropolis spin updates/s on BASELINE.json config c3.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+Workload (BASELINE.json configs[2], SURVEY section 8d "c3"): 224^3 = 11 239 424 unit Heisenberg spins, simple cubic,
+periodic, J = 1, cubic anisotropy Kc = 0.01, B = 0, T cycling through {0.5, 1.2, 1.44}, spins start uniformly random
+on the sphere (seeded, synthetic), adaptive cone.  One STEP = ``--sweeps-per-step`` full Monte Carlo iterations
+(red pass + black pass + controller + fused reductions = every row of the hot-path table) through mc_sweep().
+
+Printed JSON line (one, by rank 0): see the task contract; `value` = spin updates/s with the state resident in HBM,
+`e2e` = the same through the C ABI with host buffers (mc_set_spins H2D + mc_sweep + mc_observables D2H every step),
+`roofline` = algorithmic HBM bytes of one colour-pass launch / its CUDA-event duration against the measured copy peak,
+`cpu_baseline` = the fp64 oracle timed on this box's host cores on a bounded sample.
+
+--impl reference times the oracle itself (there is no reference implementation to install: /root/reference holds only
+the paper's text), on the same config/metric/unit, each step a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "spin updates/sec (Metropolis attempts) at 11.2M spins; achieved HBM GB/s vs peak"
+UNIT = "spin-updates/s"
+SHAPE = (224, 224, 224)
+HAM = dict(J=1.0, Kc=0.01)
+TEMPS = (0.5, 1.2, 1.44)
+BYTES_PER_UPDATE = 36          # read self 12 + read other colour once 12 + write self 12
+DEV_STATE_BYTES = 360          # what mc_observables copies back
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def recorded_traffic():
+    """dram bytes per colour-pass launch from the committed ncu --set full capture, if any (profiles/traffic.json)."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return float(json.load(open(path))["pass_kernel_dram_bytes_per_launch"])
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons DURING the timed region."""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True); self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try: self.proc.wait(timeout=2)
+        except Exception: self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"): reasons.add(n)
+            except Exception:
+                pass
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def cpu_cores_used():
+    return 1   # the oracle is single-threaded by construction
+
+
+def time_oracle(shape, T, n_warm, n_timed, seed=42):
+    """Oracle (as it stands) on this box's host cores: returns (updates/s, seconds, description)."""
+    import oracle
+    from paper_2103_03517_b200 import inputs
+    N = shape[0] * shape[1] * shape[2]
+    o = oracle.Oracle(*shape, seed=seed, cone0=0.5, adaptive=True, **HAM)
+    o.set_spins(inputs.random_unit_spins(N, seed=seed))
+    if n_warm: o.sweep(T, n_warm)
+    t0 = time.perf_counter(); o.sweep(T, n_timed); dt = time.perf_counter() - t0
+    return N * n_timed / dt, dt, f"{shape[0]}x{shape[1]}x{shape[2]} lattice, c3 Hamiltonian, T={T}, {n_warm} warm-up + {n_timed} timed sweeps ({N * n_timed} updates), 1 thread"
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return 0
+    total_steps = args.steps + args.warmup
+    # bounded sample: the largest cubic lattice (multiple of 8, <= 224) such that the run ends within ~2.5 minutes at ~2.5 M updates/s
+    budget_updates = 150.0 * 2.5e6 / max(1, total_steps)
+    L = 224
+    while L > 16 and L ** 3 > budget_updates: L -= 8
+    import oracle
+    from paper_2103_03517_b200 import inputs
+    N = L ** 3
+    o = oracle.Oracle(L, L, L, seed=42, cone0=0.5, adaptive=True, **HAM)
+    o.set_spins(inputs.random_unit_spins(N, seed=42))
+    for i in range(args.warmup): o.sweep(TEMPS[i % 3], 1)
+    t0 = time.perf_counter()
+    for i in range(args.steps): o.sweep(TEMPS[i % 3], 1)
+    dt = time.perf_counter() - t0
+    value = N * args.steps / dt
+    sample = f"each step = 1 full sweep (red+black+controller+observables) of a {L}^3 lattice with the c3 Hamiltonian ({N} updates), oracle fp64, 1 thread"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "c3: 224^3 simple cubic periodic, J=1, Kc=0.01, T in {0.5,1.2,1.44}, random-sphere start, adaptive cone", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cpu_cores_used(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def run_ours(args, rank, local_rank, world):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    from paper_2103_03517_b200 import binding, build, inputs
+    build.build()
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_
+        dist = dist_
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+
+    N = SHAPE[0] * SHAPE[1] * SHAPE[2]
+    spp = args.sweeps_per_step
+    # replicas: every rank owns an independent lattice (own seed) -- no data-path collective ("replicas only")
+    g = binding.Lattice(*SHAPE, seed=42 + rank, cone0=0.5, adaptive=True, device=f"cuda:{local_rank}", **HAM)
+    host = torch.from_numpy(inputs.random_unit_spins(N, seed=42 + rank)).pin_memory()
+    host_np = host.numpy()
+    g.set_spins(host_np)
+
+    def barrier():
+        if dist is not None: dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident throughput
+    for i in range(args.warmup): g.sweep(TEMPS[i % 3], spp)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0: sampler.start()
+    l0 = g.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for i in range(args.steps): g.sweep(TEMPS[i % 3], spp)
+    ev1.record()
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = g.launch_count() - l0
+    clocks = sampler.stop() if rank == 0 else None
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); ms = float(t.item())
+    value = world * N * spp * args.steps / (ms * 1e-3)
+
+    # ---- end to end through the C ABI with host buffers: H2D of the state + sweeps + D2H of the observables, every step
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    g.set_spins(host_np); g.sweep(TEMPS[0], spp); g.observables()
+    barrier()
+    t0 = time.perf_counter()
+    for i in range(e2e_steps):
+        g.set_spins(host_np)                # pinned host -> device, layout conversion on the device
+        g.sweep(TEMPS[i % 3], spp)
+        ob = g.observables()                # synchronises; device -> host
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); e2e_s = float(t.item())
+    e2e_value = world * N * spp * e2e_steps / e2e_s
+
+    if rank != 0:
+        g.close(); return 0
+
+    peak, peak_src = measured_peaks()
+    t_launch = ms * 1e-3 / launches                       # average duration of one colour-pass launch over the timed region
+    alg_bytes_per_launch = BYTES_PER_UPDATE * (N // 2)    # one launch updates one colour
+    achieved = alg_bytes_per_launch / t_launch / 1e9
+    roofline = {"bound": "hbm", "kernel": "pass_kernel (one colour pass)", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": recorded_traffic(), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg_bytes_per_launch, "avg_launch_us": t_launch * 1e6,
+                "frac_of_nominal_8TBs": achieved / 8000.0}
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        v, dt, sample = time_oracle(SHAPE, 1.2, 1, 2)
+        cpu = {"value": v, "unit": UNIT, "cores": cpu_cores_used(), "kind": "oracle", "sample": sample, "seconds": dt}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "c3: 224^3 simple cubic periodic, J=1, Kc=0.01, T in {0.5,1.2,1.44} cycling per step, random-sphere start, adaptive cone",
+                       "sweeps_per_step": spp, "spins": N, "state_bytes": N * 12, "l2_policy": "inputs larger than L2 (134.9 MB state vs 126 MB L2)",
+                       "parallelism": f"replicas x{world} (no collective)", "final_m": ob.m, "final_acceptance": ob.last_acceptance},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": N * 12, "d2h_bytes_per_step": DEV_STATE_BYTES, "steps": e2e_steps},
+            "gpu_launches": launches,
+            "roofline": roofline,
+            "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    g.close()
+    if dist is not None: dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--sweeps-per-step", type=int, default=100)
+    ap.add_argument("--e2e-steps", type=int, default=6)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3                                   # timing rule: W >= 3
+    rank = int(os.environ.get("RANK", "0")); local_rank = int(os.environ.get("LOCAL_RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        return run_reference(args, rank, world)
+    return run_ours(args, rank, local_rank, world)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

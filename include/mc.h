@@ -1,0 +1,142 @@
+/*
+ * mc.h -- C ABI of libmc_b200.so: red-black checkerboard Metropolis for unit classical Heisenberg spins on a
+ * simple-cubic lattice, hand-written CUDA for sm_100a (NVIDIA B200).
+ *
+ * Method: Lepadatu et al., "Computation of magnetization, exchange stiffness, anisotropy, and susceptibilities in
+ * large-scale systems using GPU-accelerated atomistic parallel Monte Carlo algorithms", arXiv 2103.03517.
+ * "P:NN" = line NN of that paper's text; "C-n" = reading n in DESIGN.md section 4.
+ *
+ * Conventions
+ *   - extern "C", plain pointers and sizes, no exceptions, no globals, no callbacks.  Every pointer argument is a
+ *     HOST pointer unless its name starts with dev_.  The caller owns every buffer it passes; the library copies
+ *     what it needs during the call and keeps no host pointer afterwards.
+ *   - The library allocates NO device memory: the caller hands mc_create() one device workspace of at least
+ *     mc_workspace_bytes() bytes (e.g. a torch.empty(..., dtype=uint8, device="cuda")) and a CUDA stream.  All
+ *     kernels of a handle run on that stream.  Handles are independent (replicas); one stream per handle.
+ *   - Return value: MC_OK (0) or a negative error code; mc_last_error() gives the message of the last failure.
+ *     CUDA errors are sticky per handle (MC_ECUDA).
+ *   - Reduced units: k_B = 1, energies in units of J (C-17).  Spins are fp32 on the device.
+ *   - Lattice site index: site = x + nx*(y + ny*z), x fastest.  Colour c = (x+y+z) & 1, "red" = 0 first (C-10).
+ *   - There is no CPU fallback: without a CUDA device every call fails with MC_ECUDA.
+ */
+#ifndef MC_B200_H
+#define MC_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MC_OK       0
+#define MC_EINVAL  (-1)   /* bad argument (null pointer, T <= 0, odd nx, odd periodic dimension, ...)      */
+#define MC_ECUDA   (-2)   /* a CUDA call failed; sticky                                                 */
+#define MC_ESTATE  (-3)   /* operation impossible in the current state (|M|/N < 1e-6, M.e_C <= 0, ...)   */
+
+typedef struct mc_ctx mc_ctx;      /* opaque handle (host memory, freed by mc_destroy) */
+
+/* Simple-cubic lattice, nearest neighbours.  nx must be even (colour-split rows); every periodic
+ * dimension must be even (two-colourability); N = nx*ny*nz < 2^31.  periodic[a] = 1: wrap; 0: open faces. */
+typedef struct {
+    int32_t nx, ny, nz;
+    int32_t periodic[3];
+} mc_lattice;
+
+/* Spin Hamiltonian, Eq. (2):  E_i = -sum_j J_ij S_i.S_j - Ku (S_i.e_i)^2 + Kc (Sx^2Sy^2 + Sx^2Sz^2 + Sy^2Sz^2) - S_i.B */
+typedef struct {
+    double J;                    /* nearest-neighbour exchange J_ij = J on every present bond                 */
+    double Ku;                   /* uniaxial constant                                                               */
+    double eu[3];                /* easy axis (normalised on entry; ignored where region != NULL)                   */
+    double Kc;                   /* cubic constant, cube axes = x,y,z                                        */
+    double B[3];                 /* Zeeman vector mu0*muS*H_a in energy units                                       */
+    const uint8_t*  bond_mask;   /* optional [N]: bit k of site s set <=> bond k in (+x,-x,+y,-y,+z,-z) carries J.  *
+                                  * NULL = every bond allowed by the boundary conditions.  Must be symmetric and    *
+                                  * must not set a bond through an open face (checked, MC_EINVAL).                   */
+    const uint16_t* region;      /* optional [N]: grain id of every site, < n_regions                       */
+    const double*   region_axis; /* [n_regions][3] easy axis of every grain (normalised on entry)                   */
+    int32_t n_regions;
+    double cone0_rad;            /* initial cone HALF-angle theta in radians (C-6), clamped to [1 deg, 180 deg]      */
+    int32_t adaptive;            /* 1: +-1 degree per sweep toward acceptance 0.5 (C-2, C-9)        */
+} mc_hamiltonian;
+
+/* Everything mc_observables() returns; all fp64; intensive quantities are per site. */
+typedef struct {
+    uint64_t n_sites, sweep;     /* sweep = number of completed Monte Carlo iterations (both kinds)                  */
+    double cone_rad;             /* current cone half-angle                                                         */
+    double last_acceptance;      /* acceptance rate of the last completed sweep                          */
+    double M[3];                 /* sum_i S_i / N of the current state                                              */
+    double m;                    /* |M|                                                                             */
+    double E_total, E_exch, E_aniso, E_zeeman;   /* energies per site, every bond counted once (C-1)               */
+    double torque[3];            /* sum_i S_i x H_i / N,  H_i = -dE_i/dS_i of the on-site terms              */
+    uint64_t n_samples;          /* sweeps accumulated since mc_reset_accumulators()                                */
+    double sum_m[4], sum_m2[4];  /* alpha = l,x,y,z: sum over sampled sweeps of m_alpha and m_alpha^2 (Eq. 6)  */
+    double sum_E, sum_E2;        /* sum of E_total and E_total^2 per sampled sweep                                   */
+    double sum_torque[3];        /* sum of the torque per sampled sweep (constrained sweeps only, else 0)            */
+} mc_obs;
+
+/* Bytes of device workspace mc_create() needs for this lattice + Hamiltonian (0 on invalid arguments). */
+size_t mc_workspace_bytes(const mc_lattice* lat, const mc_hamiltonian* ham);
+
+/* Creates a handle.  dev_workspace: device memory, 256-byte aligned, >= mc_workspace_bytes(); cuda_stream: a
+ * cudaStream_t (NULL = legacy default stream).  Spins start along +z; sweep counter 0.  The RNG is Philox4x32-10
+ * with key = seed and counter = (site, tag | colour<<8, sweep_lo, sweep_hi): moves are reproducible and independent
+ * of launch geometry.  Synchronous (uploads the side data). */
+int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
+              void* dev_workspace, size_t workspace_bytes, void* cuda_stream, mc_ctx** out);
+int mc_destroy(mc_ctx* ctx);     /* frees the host handle only; the workspace stays the caller's */
+
+/* mode 0: all spins +z; mode 1: all spins along dir (normalised).  Asynchronous. */
+int mc_init_spins(mc_ctx* ctx, int mode, const double dir[3]);
+/* Upload / download the spin state as [N][3] fp32 in lexicographic site order (x fastest).  mc_set_spins
+ * normalises every spin.  Both synchronise the stream. */
+int mc_set_spins(mc_ctx* ctx, const float* host_xyz);
+int mc_get_spins(mc_ctx* ctx, float* host_xyz);
+/* Set the cone half-angle / the sweep counter (checkpoint restore, parity tests).  Asynchronous. */
+int mc_set_cone(mc_ctx* ctx, double cone_rad);
+int mc_set_sweep(mc_ctx* ctx, uint64_t sweep);
+
+/* n Monte Carlo iterations of Table A1 at temperature T > 0: red pass, black pass, cone controller,
+ * per-sweep reductions (acceptance, M, E) and Eq. (6) accumulators.  Asynchronous: enqueues 2n kernels on the
+ * handle's stream and returns; no host synchronisation, the controller state lives on the device. */
+int mc_sweep(mc_ctx* ctx, double T, int64_t n);
+
+/* n iterations of the constrained algorithm, Table A2, holding M/|M| along
+ * e_C = (sin theta cos phi, sin theta sin phi, cos theta).  On the first call, after mc_set_spins/mc_init_spins,
+ * or when (theta, phi) changes, all spins are first rotated rigidly so that M/|M| = e_C (C-12; this step
+ * synchronises once; MC_ESTATE if |M|/N < 1e-6).  Pairs are same-colour, formed by the analytic pairing of C-11;
+ * M_L is taken once per iteration.  Needs an even number of sites per colour (C-15). */
+int mc_constrained_sweep(mc_ctx* ctx, double T, double theta, double phi, int64_t n);
+
+/* Test hooks for per-colour parity (C-14): ONE colour pass of Table A1 / A2 with the current sweep counter and cone;
+ * no controller step, no accumulation.  host_x / host_acc are optional [N] outputs in lexicographic site order:
+ * the fp32 decision variable x = dE/T + ln u2 (constrained: the log form of P:193, stored at the leader's site,
+ * +inf for the hard rejections of C-13) and the accept flag; entries of the other colour are left untouched.
+ * mc_constrained_half_sweep does not rotate: the caller passes an aligned state and M_L explicitly.  Synchronous. */
+int mc_half_sweep(mc_ctx* ctx, double T, int colour, float* host_x, uint8_t* host_acc);
+int mc_constrained_half_sweep(mc_ctx* ctx, double T, double theta, double phi, int colour, double M_L,
+                              float* host_x, uint8_t* host_acc);
+/* Closes a sweep assembled from half-sweep hooks: controller step with the accepted count of the two passes,
+ * sweep counter += 1 (what mc_sweep does after its black pass).  Asynchronous. */
+int mc_end_sweep(mc_ctx* ctx);
+/* Rigid rotation of all spins taking M/|M| onto e_C (C-12), exposed for parity tests.  Synchronous. */
+int mc_align_to(mc_ctx* ctx, double theta, double phi);
+
+/* Synchronises the stream and returns the observables of the current state plus the accumulators.
+ * The only device-to-host copy of results on the hot path. */
+int mc_observables(mc_ctx* ctx, mc_obs* out);
+int mc_reset_accumulators(mc_ctx* ctx);                      /* asynchronous */
+/* Per-sweep trace (most recent min(max_rows, sweeps, MC_TRACE_CAPACITY) sweeps, oldest first):
+ * rows[k][6] = acceptance, cone used, Mx, My, Mz (per site), E_total (per site).  Synchronous. */
+#define MC_TRACE_CAPACITY 16384
+int mc_trace(mc_ctx* ctx, int64_t max_rows, double* host_rows, int64_t* n_rows);
+
+/* Number of kernel launches this handle has enqueued since creation (bench.py's gpu_launches). */
+int64_t mc_launch_count(const mc_ctx* ctx);
+const char* mc_last_error(const mc_ctx* ctx);                /* never NULL; valid until the next call on ctx */
+const char* mc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

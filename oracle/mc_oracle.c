@@ -439,7 +439,7 @@ static int pair_update(orc_ctx* c, double T, const double e[3], int colour, int6
     }
     double xd = INFINITY;
     int accept = 0;
-    double rho = 1.0 - p2;                                                /* P:189 radicand (|S_j| = 1) */
+    double rho = (Sj[0] * Sj[0] + Sj[1] * Sj[1] + Sj[2] * Sj[2]) - p2;    /* P:189 radicand: S_j^2 - y'^2 - z'^2 */
     double MLhat = *ML;
     if (rho > 0.0) {                                                      /* C-13 */
         double Snj_par = ((Sj_par >= 0.0) ? 1.0 : -1.0) * sqrt(rho);      /* P:189 sign kept */

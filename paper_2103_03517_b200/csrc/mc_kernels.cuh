@@ -1,0 +1,632 @@
+// mc_kernels.cuh -- sm_100a kernels of the checkerboard Metropolis path: colour pass (Table A1), constrained pair
+// pass (Table A2), fused per-sweep reductions + cone controller, standalone measurement, layout conversion.
+//
+// Data layout in HBM: colour-split SoA fp32 planes.  For colour c and component k the plane
+// S[(3c + k) * plane .. ] holds the sites of colour c in colour-linear order a = (x>>1) + R (y + ny z), R = nx/2.
+// With row parity p = (y+z+c)&1 the site is x = 2 (a mod R) + p, and its six neighbours live in the OTHER colour at
+//   +-y, +-z : the same a-offset inside the neighbouring row
+//   +-x      : xh and xh + (p ? +1 : -1) of the same row  (p=0: +x is xh, -x is xh-1;  p=1: -x is xh, +x is xh+1)
+// so one colour pass streams its own colour once (read + write) and the other colour once (read).
+#pragma once
+
+#include "mc_device.cuh"
+
+namespace mc {
+
+constexpr int NQ = 9;          // fused sums: Mx My Mz E_exch E_aniso E_zeeman tq_x tq_y tq_z (extensive, fp64)
+constexpr int BLOCK = 256;     // threads per CTA of the pass kernels
+constexpr int TRACE_CAP = 16384;
+
+// Controller / reduction state, resident in the workspace (no host round trip per sweep: P:165-171 runs on the device)
+struct DevState {
+    unsigned long long sweep;        // completed Monte Carlo iterations = Philox counter words 2,3
+    double cone;                     // cone half-angle theta (rad)
+    float one_minus_cos;             // 1 - cos(theta), what the move kernel needs
+    int adaptive;
+    unsigned long long count;        // accepted moves of the sweep in flight (integer atomics: order independent)
+    unsigned int ticket;             // last-block election
+    unsigned int nblocks[4];         // grid size of the pass whose partials wait in slot: 0,1 sweep red/black; 2,3 measurement
+    unsigned int pad_;
+    double last_acceptance;
+    double sums[NQ];                 // fused sums of the last completed sweep
+    double meas[NQ];                 // sums written by the standalone measurement
+    double ML;                       // M_L = sum_i S_i.e_C of the state; refreshed by finalize and measure
+    double eC[3];
+    unsigned long long n_samples;
+    double sum_m[4], sum_m2[4], sum_E, sum_E2, sum_torque[3];
+    unsigned long long trace_rows;   // rows ever written to the trace ring
+};
+
+struct Params {
+    int nx, ny, nz, R;               // R = nx/2 sites of one colour per row
+    uint32_t Nc;                     // sites per colour
+    uint32_t N;
+    long long plane;                 // floats between component planes
+    float* S;                        // 6 planes: colour-major, then component
+    const uint8_t* mask;   long long mask_plane;     // [2][mask_plane] colour-split bond masks (or null)
+    const uint16_t* region; long long region_plane;  // [2][region_plane] colour-split grain ids (or null)
+    const float4* axis;              // [n_regions] easy axes
+    float J, Ku, Kc;
+    float eu[3], B[3];
+    uint32_t seed_lo, seed_hi;
+    DevState* st;
+    double* partials;                // [4][max_blocks][NQ]: slots 0,1 = sweep red/black, 2,3 = measurement red/black
+    int max_blocks;
+    double* trace;                   // [TRACE_CAP][6]
+};
+
+struct Geom {                        // per-VEC decomposition of the colour-linear index space into items of VEC sites
+    uint32_t n_items, RV;            // RV = items per row
+    FastDiv div_rv, div_ny;
+};
+
+enum : int { F_FINALIZE = 1, F_TORQUE = 2, F_SAMPLE_TORQUE = 4 };
+enum : int { MODE_SWEEP = 0, MODE_MEASURE = 1 };
+
+// --------------------------------------------------------------------------------------------------------------
+template <int VEC> struct Pack { float v[VEC]; };
+
+template <int VEC> __device__ __forceinline__ Pack<VEC> ld_nc(const float* p);
+template <> __device__ __forceinline__ Pack<1> ld_nc<1>(const float* p) { Pack<1> r; r.v[0] = __ldg(p); return r; }
+template <> __device__ __forceinline__ Pack<4> ld_nc<4>(const float* p)
+{
+    const float4 t = __ldg(reinterpret_cast<const float4*>(p));
+    Pack<4> r; r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w; return r;
+}
+template <int VEC> __device__ __forceinline__ Pack<VEC> ld_rw(const float* p);
+template <> __device__ __forceinline__ Pack<1> ld_rw<1>(const float* p) { Pack<1> r; r.v[0] = *p; return r; }
+template <> __device__ __forceinline__ Pack<4> ld_rw<4>(const float* p)
+{
+    const float4 t = *reinterpret_cast<const float4*>(p);
+    Pack<4> r; r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w; return r;
+}
+template <int VEC> __device__ __forceinline__ void st_rw(float* p, const Pack<VEC>& r);
+template <> __device__ __forceinline__ void st_rw<1>(float* p, const Pack<1>& r) { *p = r.v[0]; }
+template <> __device__ __forceinline__ void st_rw<4>(float* p, const Pack<4>& r)
+{
+    *reinterpret_cast<float4*>(p) = make_float4(r.v[0], r.v[1], r.v[2], r.v[3]);
+}
+
+// One item = VEC consecutive same-colour sites of one row.  Coordinates + neighbour offsets.
+struct ItemPos {
+    uint32_t a0;        // colour-linear index of the first site
+    uint32_t site0;     // lexicographic index of the first site (next ones are +2)
+    uint32_t par;       // (y + z + colour) & 1
+    uint32_t o_yp, o_ym, o_zp, o_zm;   // colour-linear index of the same column in the 4 neighbouring rows
+    uint32_t o_x;       // colour-linear index of the one extra x-neighbour outside the item's own column range
+};
+
+template <int VEC>
+__device__ __forceinline__ ItemPos locate(const Params& P, const Geom& G, uint32_t item, int colour)
+{
+    uint32_t row, xq, y, z;
+    G.div_rv.divmod(item, row, xq);
+    G.div_ny.divmod(row, z, y);
+    ItemPos q;
+    const uint32_t R = (uint32_t)P.R, ny = (uint32_t)P.ny, nz = (uint32_t)P.nz;
+    const uint32_t xh0 = xq * VEC;
+    q.par = (y + z + (uint32_t)colour) & 1u;
+    q.a0 = row * R + xh0;
+    q.site0 = row * (uint32_t)P.nx + 2u * xh0 + q.par;
+    const uint32_t yp = (y + 1 == ny) ? 0u : y + 1, ym = (y == 0) ? ny - 1 : y - 1;
+    const uint32_t zp = (z + 1 == nz) ? 0u : z + 1, zm = (z == 0) ? nz - 1 : z - 1;
+    q.o_yp = (z * ny + yp) * R + xh0;  q.o_ym = (z * ny + ym) * R + xh0;
+    q.o_zp = (zp * ny + y) * R + xh0;  q.o_zm = (zm * ny + y) * R + xh0;
+    const uint32_t xe = q.par ? ((xh0 + VEC == R) ? 0u : xh0 + VEC) : ((xh0 == 0) ? R - 1 : xh0 - 1);
+    q.o_x = row * R + xe;
+    return q;
+}
+
+// Exchange field h = sum_j J_ij S_j of the VEC sites of an item (first term of Eq. 2), WITHOUT the factor J.
+// MASKED: bond k of a site contributes only if bit k of its mask is set (grain boundaries P:118, open faces P:116).
+template <int VEC, bool MASKED>
+__device__ __forceinline__ void exchange_field(const Params& P, const ItemPos& q, int colour, Vec3 (&h)[VEC])
+{
+    const float* O = P.S + (long long)(1 - colour) * 3 * P.plane;
+    uint32_t mbits[VEC];
+    if (MASKED) {
+        const uint8_t* m = P.mask + (long long)colour * P.mask_plane + q.a0;
+        if (VEC == 4) {
+            const uint32_t w = __ldg(reinterpret_cast<const uint32_t*>(m));
+#pragma unroll
+            for (int k = 0; k < VEC; ++k) mbits[k] = (w >> (8 * k)) & 0xFFu;
+        } else {
+#pragma unroll
+            for (int k = 0; k < VEC; ++k) mbits[k] = __ldg(m + k);
+        }
+    }
+    float hc[3][VEC];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float* Oc = O + (long long)c * P.plane;
+        const Pack<VEC> o  = ld_nc<VEC>(Oc + q.a0);
+        const Pack<VEC> yp = ld_nc<VEC>(Oc + q.o_yp), ym = ld_nc<VEC>(Oc + q.o_ym);
+        const Pack<VEC> zp = ld_nc<VEC>(Oc + q.o_zp), zm = ld_nc<VEC>(Oc + q.o_zm);
+        const float ex = __ldg(Oc + q.o_x);
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) {
+            // the second x-neighbour: next column if par = 1, previous column if par = 0
+            const float sh = q.par ? ((k + 1 < VEC) ? o.v[(k + 1) % VEC] : ex) : ((k > 0) ? o.v[(k + VEC - 1) % VEC] : ex);
+            if (MASKED) {
+                const uint32_t mb = mbits[k];
+                // o.v[k] is the +x neighbour when par = 0 and the -x neighbour when par = 1
+                const uint32_t bit_o = q.par ? 2u : 1u, bit_s = q.par ? 1u : 2u;
+                float s = 0.0f;
+                s += (mb & bit_o) ? o.v[k] : 0.0f;
+                s += (mb & bit_s) ? sh : 0.0f;
+                s += (mb & 4u)  ? yp.v[k] : 0.0f;
+                s += (mb & 8u)  ? ym.v[k] : 0.0f;
+                s += (mb & 16u) ? zp.v[k] : 0.0f;
+                s += (mb & 32u) ? zm.v[k] : 0.0f;
+                hc[c][k] = s;
+            } else {
+                hc[c][k] = ((o.v[k] + sh) + (yp.v[k] + ym.v[k])) + (zp.v[k] + zm.v[k]);
+            }
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < VEC; ++k) h[k] = { hc[0][k], hc[1][k], hc[2][k] };
+}
+
+// easy axes of the VEC sites of an item: uniform, or per grain through the region table (config c5)
+template <int VEC>
+__device__ __forceinline__ void easy_axes(const Params& P, const ItemPos& q, int colour, Vec3 (&e)[VEC])
+{
+    if (P.region) {
+        const uint16_t* r = P.region + (long long)colour * P.region_plane + q.a0;
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) { const float4 a = __ldg(P.axis + __ldg(r + k)); e[k] = { a.x, a.y, a.z }; }
+    } else {
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) e[k] = { P.eu[0], P.eu[1], P.eu[2] };
+    }
+}
+
+// --------------------------------------------------------------------------------------------------------------
+// Block reduction of the per-thread fused sums in a FIXED order (deterministic two-pass fp64 reduction, pass 1):
+// lanes by xor-shuffle, warps sequentially; thread 0 writes the block partial.
+// --------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+__device__ __forceinline__ void block_partials(const double (&acc)[NQ], int cnt, const Params& P, int slot)
+{
+    __shared__ double sm[BLOCK / 32][NQ];
+    __shared__ int scnt;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) scnt = 0;
+    __syncthreads();
+    const int wc = __reduce_add_sync(0xffffffffu, cnt);
+    if (lane == 0 && wc) atomicAdd(&scnt, wc);
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) { const double v = warp_sum(acc[q]); if (lane == 0) sm[warp][q] = v; }
+    __syncthreads();
+    if (threadIdx.x < NQ) {
+        double v = 0.0;
+#pragma unroll
+        for (int w = 0; w < BLOCK / 32; ++w) v += sm[w][threadIdx.x];
+        P.partials[((long long)slot * P.max_blocks + blockIdx.x) * NQ + threadIdx.x] = v;
+    }
+    if (threadIdx.x == 0 && scnt) atomicAdd(&P.st->count, (unsigned long long)scnt);
+}
+
+// Pass 2 of the reduction (one block, fixed order) + what follows a sweep: cone controller (P:168-171 read with
+// P:205-209; C-2, C-3, C-9), sweep counter, Eq. (6) accumulators, trace row.  mode 0: end of a sweep; 1: measurement.
+__device__ void final_reduce(const Params& P, int mode, int flags)
+{
+    __shared__ double red[BLOCK / 32][NQ];
+    DevState* st = P.st;
+    double acc[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
+    for (int slot = 2 * mode; slot < 2 * mode + 2; ++slot) {
+        const unsigned nb = __ldcg(&st->nblocks[slot]);
+        for (unsigned b = threadIdx.x; b < nb; b += BLOCK) {
+            const double* p = P.partials + ((long long)slot * P.max_blocks + b) * NQ;
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) acc[q] += __ldcg(p + q);
+        }
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) { const double v = warp_sum(acc[q]); if (lane == 0) red[warp][q] = v; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s[NQ];
+        for (int q = 0; q < NQ; ++q) { double v = 0.0; for (int w = 0; w < BLOCK / 32; ++w) v += red[w][q]; s[q] = v; }
+        st->ML = s[0] * st->eC[0] + s[1] * st->eC[1] + s[2] * st->eC[2];
+        if (mode == 1) {
+            for (int q = 0; q < NQ; ++q) st->meas[q] = s[q];
+        } else {
+            const double N = (double)P.N, invN = 1.0 / N;
+            const unsigned long long cnt = __ldcg(&st->count);
+            const double cone_used = st->cone;
+            st->last_acceptance = (double)cnt * invN;
+            if (st->adaptive) {
+                const double deg = 3.14159265358979323846 / 180.0, pi = 3.14159265358979323846;
+                double c = st->cone;
+                if (2ull * cnt > (unsigned long long)P.N) { c += deg; if (c > pi) c = pi; }
+                else                                      { c -= deg; if (c < deg) c = deg; }
+                st->cone = c;
+                st->one_minus_cos = (float)(1.0 - cos(c));
+            }
+            st->count = 0ull;
+            st->sweep += 1ull;
+            for (int q = 0; q < NQ; ++q) st->sums[q] = s[q];
+            const double mx = s[0] * invN, my = s[1] * invN, mz = s[2] * invN;
+            const double ml = sqrt(mx * mx + my * my + mz * mz);
+            const double E = (s[3] + s[4] + s[5]) * invN;
+            const double mv[4] = { ml, mx, my, mz };
+            for (int a = 0; a < 4; ++a) { st->sum_m[a] += mv[a]; st->sum_m2[a] += mv[a] * mv[a]; }
+            st->sum_E += E; st->sum_E2 += E * E;
+            if (flags & F_SAMPLE_TORQUE) for (int a = 0; a < 3; ++a) st->sum_torque[a] += s[6 + a] * invN;
+            st->n_samples += 1ull;
+            double* row = P.trace + (st->trace_rows % (unsigned long long)TRACE_CAP) * 6;
+            row[0] = st->last_acceptance; row[1] = cone_used; row[2] = mx; row[3] = my; row[4] = mz; row[5] = E;
+            st->trace_rows += 1ull;
+        }
+        st->ticket = 0u;
+    }
+}
+
+// Last-block election: returns true in every thread of the block that arrives last.
+__device__ __forceinline__ bool last_block_done(DevState* st)
+{
+    __shared__ bool is_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) is_last = (atomicAdd(&st->ticket, 1u) == gridDim.x - 1);
+    __syncthreads();
+    if (is_last) __threadfence();
+    return is_last;
+}
+
+// --------------------------------------------------------------------------------------------------------------
+// Colour pass of Table A1: one item of VEC sites per loop trip, grid-stride.
+//   MODE_SWEEP  : propose (a-4), dE (a-5), accept/write (a-6), count (a-7), fused sums of the FINAL spins (a-9).
+//   MODE_MEASURE: no move; sums of the current spins (standalone measurement).
+// E_exch is accumulated by the BLACK pass only: every bond joins a red and a black site, so
+// E_exch = -sum_{i black} S_i.h_i with h already in registers (0 extra bytes).
+// --------------------------------------------------------------------------------------------------------------
+template <int VEC, int ANISO, bool MASKED, int MODE>
+__global__ void __launch_bounds__(BLOCK)
+pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, int colour, float invT, int flags,
+            float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
+{
+    DevState* st = P.st;
+    const unsigned long long sweep = st->sweep;
+    const float omc = st->one_minus_cos;
+    const PhiloxKey key = philox_key(P.seed_lo, P.seed_hi);
+    const uint32_t c1 = TAG_MOVE | ((uint32_t)colour << 8), c2 = (uint32_t)sweep, c3 = (uint32_t)(sweep >> 32);
+    float* Sc = P.S + (long long)colour * 3 * P.plane;
+    const Vec3 B = { P.B[0], P.B[1], P.B[2] };
+
+    double acc[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
+    int cnt = 0;
+
+    const uint32_t stride = gridDim.x * BLOCK;
+    for (uint32_t item = blockIdx.x * BLOCK + threadIdx.x; item < G.n_items; item += stride) {
+        const ItemPos q = locate<VEC>(P, G, item, colour);
+        const Pack<VEC> sx = ld_rw<VEC>(Sc + q.a0), sy = ld_rw<VEC>(Sc + P.plane + q.a0), sz = ld_rw<VEC>(Sc + 2 * P.plane + q.a0);
+        Vec3 h[VEC], e[VEC];
+        exchange_field<VEC, MASKED>(P, q, colour, h);
+        if (ANISO & 1) easy_axes<VEC>(P, q, colour, e);
+        Pack<VEC> nxv = sx, nyv = sy, nzv = sz;
+        float f[NQ];
+#pragma unroll
+        for (int k = 0; k < NQ; ++k) f[k] = 0.0f;
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) {
+            Vec3 S = { sx.v[k], sy.v[k], sz.v[k] };
+            const Vec3 hJ = { P.J * h[k].x, P.J * h[k].y, P.J * h[k].z };
+            if (MODE == MODE_SWEEP) {
+                uint32_t r0, r1, r2, r3;
+                philox4x32_10(key, q.site0 + 2u * k, c1, c2, c3, r0, r1, r2, r3);
+                Vec3 d, Sn;
+                cone_move(S, omc, uniform01(r0), uniform01(r1), d, Sn);
+                const Vec3 hB = { hJ.x + B.x, hJ.y + B.y, hJ.z + B.z };
+                const float dE = delta_energy<ANISO>(S, d, hB, P.Ku, e[(ANISO & 1) ? k : 0], P.Kc);
+                const float x = fmaf(dE, invT, __logf(uniform01(r2)));       // P:157-158 in log form (C-8)
+                const bool ok = x < 0.0f;
+                if (ok) { S = Sn; nxv.v[k] = Sn.x; nyv.v[k] = Sn.y; nzv.v[k] = Sn.z; }
+                cnt += ok;
+                if (dbg_x)   dbg_x[q.site0 + 2u * k] = x;
+                if (dbg_acc) dbg_acc[q.site0 + 2u * k] = (uint8_t)ok;
+            }
+            f[0] += S.x; f[1] += S.y; f[2] += S.z;
+            if (colour == 1) f[3] -= dot3(S, hJ);
+            if (ANISO) f[4] += aniso_energy<ANISO>(S, P.Ku, e[(ANISO & 1) ? k : 0], P.Kc);
+            f[5] -= dot3(S, B);
+            if (flags & F_TORQUE) {
+                const Vec3 t = onsite_torque<ANISO>(S, P.Ku, e[(ANISO & 1) ? k : 0], P.Kc, B);
+                f[6] += t.x; f[7] += t.y; f[8] += t.z;
+            }
+        }
+        if (MODE == MODE_SWEEP) {
+            st_rw<VEC>(Sc + q.a0, nxv); st_rw<VEC>(Sc + P.plane + q.a0, nyv); st_rw<VEC>(Sc + 2 * P.plane + q.a0, nzv);
+        }
+#pragma unroll
+        for (int k = 0; k < NQ; ++k) acc[k] += (double)f[k];
+    }
+
+    const int slot = (MODE == MODE_MEASURE ? 2 : 0) + colour;
+    block_partials(acc, cnt, P, slot);
+    if (threadIdx.x == 0) st->nblocks[slot] = gridDim.x;
+    if (flags & F_FINALIZE) {
+        if (last_block_done(st)) final_reduce(P, MODE == MODE_MEASURE ? 1 : 0, flags);
+    }
+}
+
+// Stand-alone pass 2 (for sweeps assembled from the half-sweep test hooks): <<<1, BLOCK>>>
+__global__ void __launch_bounds__(BLOCK) finalize_kernel(const __grid_constant__ Params P, int mode, int flags)
+{
+    final_reduce(P, mode, flags);
+}
+
+// --------------------------------------------------------------------------------------------------------------
+// Constrained pair pass of Table A2, one thread per VEC pairs of one colour.
+// Pairing (C-11, replaces the shuffled index array of P:38/P:202 by a pure function of (seed, sweep, colour)):
+//   the colour-linear index space is cut into H = Nc/B chunks of B consecutive sites, B = largest power of two
+//   <= 32 with 2B | Nc, and each chunk into Bh = B/Bl groups of Bl = min(B,4) sites;
+//   (r0,r1,r2,.) = Philox(0, TAG_PAIRING | colour<<8, sweep);  m = 2 floor(r0 (H/2) / 2^32) + 1;  sigma = r1 & 1;
+//   rot = r2 mod Bl;  q = (r2 >> 2) mod Bh;
+//   site (chunk, hi, lo) is a LEADER iff chunk mod 2 == sigma; its follower is ((chunk+m) mod H, (hi+q) mod Bh, (lo+rot) mod Bl).
+// With VEC = 4 a thread owns one leader group and one follower group: two aligned float4 per component, the
+// lo-rotation is a register permutation -- every access stays a full-sector vector access, no index array (0 bytes).
+// --------------------------------------------------------------------------------------------------------------
+struct PairGeom {
+    uint32_t B, H, Bh, Bl;          // chunk size, chunk count, groups per chunk, sites per group
+    uint32_t n_threads;             // = Nc / (2 VEC)
+    FastDiv div_r, div_ny;          // colour-linear index -> (row, xh), row -> (z, y)
+    uint32_t groups_per_chunk_vec;  // B / VEC  (VEC = 4: = Bh;  VEC = 1: = B)
+};
+
+template <int VEC>
+__device__ __forceinline__ ItemPos locate_linear(const Params& P, const PairGeom& G, uint32_t a0, int colour)
+{
+    uint32_t row, xh0, y, z;
+    G.div_r.divmod(a0, row, xh0);
+    G.div_ny.divmod(row, z, y);
+    ItemPos q;
+    const uint32_t R = (uint32_t)P.R, ny = (uint32_t)P.ny, nz = (uint32_t)P.nz;
+    q.par = (y + z + (uint32_t)colour) & 1u;
+    q.a0 = a0;
+    q.site0 = row * (uint32_t)P.nx + 2u * xh0 + q.par;
+    const uint32_t yp = (y + 1 == ny) ? 0u : y + 1, ym = (y == 0) ? ny - 1 : y - 1;
+    const uint32_t zp = (z + 1 == nz) ? 0u : z + 1, zm = (z == 0) ? nz - 1 : z - 1;
+    q.o_yp = (z * ny + yp) * R + xh0;  q.o_ym = (z * ny + ym) * R + xh0;
+    q.o_zp = (zp * ny + y) * R + xh0;  q.o_zm = (zm * ny + y) * R + xh0;
+    const uint32_t xe = q.par ? ((xh0 + VEC == R) ? 0u : xh0 + VEC) : ((xh0 == 0) ? R - 1 : xh0 - 1);
+    q.o_x = row * R + xe;
+    return q;
+}
+
+template <int VEC, int ANISO, bool MASKED>
+__global__ void __launch_bounds__(BLOCK)
+pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G, int colour, float invT, int flags,
+            float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
+{
+    DevState* st = P.st;
+    const unsigned long long sweep = st->sweep;
+    const float omc = st->one_minus_cos;
+    const double ML = st->ML;
+    const float invML = (float)(1.0 / ML);
+    const Vec3 eC = { (float)st->eC[0], (float)st->eC[1], (float)st->eC[2] };
+    const PhiloxKey key = philox_key(P.seed_lo, P.seed_hi);
+    const uint32_t c2 = (uint32_t)sweep, c3 = (uint32_t)(sweep >> 32);
+    uint32_t p0, p1, p2, p3;
+    philox4x32_10(key, 0u, TAG_PAIRING | ((uint32_t)colour << 8), c2, c3, p0, p1, p2, p3);
+    const uint32_t m = 2u * (uint32_t)(((uint64_t)p0 * (uint64_t)(G.H / 2)) >> 32) + 1u;
+    const uint32_t sigma = p1 & 1u;
+    const uint32_t rot = p2 % G.Bl, qsh = (p2 >> 2) % G.Bh;
+    const uint32_t c1 = TAG_PAIR | ((uint32_t)colour << 8);
+    float* Sc = P.S + (long long)colour * 3 * P.plane;
+    const Vec3 B = { P.B[0], P.B[1], P.B[2] };
+
+    double acc[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
+    int cnt = 0;
+
+    const uint32_t stride = gridDim.x * BLOCK;
+    for (uint32_t t = blockIdx.x * BLOCK + threadIdx.x; t < G.n_threads; t += stride) {
+        // leader group
+        const uint32_t j = t / G.groups_per_chunk_vec, g = t % G.groups_per_chunk_vec;
+        const uint32_t chunkL = 2u * j + sigma;
+        uint32_t chunkF = chunkL + m; if (chunkF >= G.H) chunkF -= G.H;
+        uint32_t aL, aF;
+        if (VEC == 4) {
+            uint32_t gf = g + qsh; if (gf >= G.Bh) gf -= G.Bh;
+            aL = chunkL * G.B + g * 4u; aF = chunkF * G.B + gf * 4u;
+        } else {
+            const uint32_t hi = g / G.Bl, lo = g % G.Bl;
+            uint32_t hf = hi + qsh; if (hf >= G.Bh) hf -= G.Bh;
+            uint32_t lf = lo + rot; if (lf >= G.Bl) lf -= G.Bl;
+            aL = chunkL * G.B + g; aF = chunkF * G.B + hf * G.Bl + lf;
+        }
+        const ItemPos qL = locate_linear<VEC>(P, G, aL, colour), qF = locate_linear<VEC>(P, G, aF, colour);
+        const Pack<VEC> lx = ld_rw<VEC>(Sc + aL), ly = ld_rw<VEC>(Sc + P.plane + aL), lz = ld_rw<VEC>(Sc + 2 * P.plane + aL);
+        const Pack<VEC> fx = ld_rw<VEC>(Sc + aF), fy = ld_rw<VEC>(Sc + P.plane + aF), fz = ld_rw<VEC>(Sc + 2 * P.plane + aF);
+        Vec3 hL[VEC], hF[VEC], eL[VEC], eF[VEC];
+        exchange_field<VEC, MASKED>(P, qL, colour, hL);
+        exchange_field<VEC, MASKED>(P, qF, colour, hF);
+        if (ANISO & 1) { easy_axes<VEC>(P, qL, colour, eL); easy_axes<VEC>(P, qF, colour, eF); }
+        Pack<VEC> nlx = lx, nly = ly, nlz = lz, nfx = fx, nfy = fy, nfz = fz;
+        float f[NQ];
+#pragma unroll
+        for (int k = 0; k < NQ; ++k) f[k] = 0.0f;
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) {
+            // leader element k pairs with follower element kf = (k + rot) mod Bl of the follower group (VEC = 4)
+            Vec3 Si = { lx.v[k], ly.v[k], lz.v[k] };
+            Vec3 Sj, hj, ej; uint32_t site_j;
+            if (VEC == 4) {
+                // register permutation: select without dynamic indexing
+                float jx = fx.v[0], jy = fy.v[0], jz = fz.v[0];
+                Vec3 hh = hF[0], ee = eF[0];
+#pragma unroll
+                for (int s = 1; s < 4; ++s) {
+                    const bool pick = ((k + rot) & 3u) == (uint32_t)s;
+                    jx = pick ? fx.v[s] : jx; jy = pick ? fy.v[s] : jy; jz = pick ? fz.v[s] : jz;
+                    hh.x = pick ? hF[s].x : hh.x; hh.y = pick ? hF[s].y : hh.y; hh.z = pick ? hF[s].z : hh.z;
+                    if (ANISO & 1) { ee.x = pick ? eF[s].x : ee.x; ee.y = pick ? eF[s].y : ee.y; ee.z = pick ? eF[s].z : ee.z; }
+                }
+                Sj = { jx, jy, jz }; hj = hh; ej = ee;
+                site_j = qF.site0 + 2u * ((k + rot) & 3u);
+            } else {
+                Sj = { fx.v[0], fy.v[0], fz.v[0] }; hj = hF[0]; ej = eF[0]; site_j = qF.site0;
+            }
+            const uint32_t site_i = qL.site0 + 2u * k;
+            uint32_t r0, r1, r2, r3;
+            philox4x32_10(key, site_i, c1, c2, c3, r0, r1, r2, r3);
+            Vec3 di, Sni;
+            cone_move(Si, omc, uniform01(r0), uniform01(r1), di, Sni);
+            const float pi_ = dot3(Si, eC), pj = dot3(Sj, eC), pni = dot3(Sni, eC);
+            const Vec3 dv = { Si.x - Sni.x, Si.y - Sni.y, Si.z - Sni.z };             // stored displacement, exact in fp32
+            // transverse parts: S_j,perp and the compensation delta = S_i,perp - S'_i,perp
+            const float dpar = dot3(dv, eC);
+            const Vec3 pj_perp = { fmaf(-pj, eC.x, Sj.x), fmaf(-pj, eC.y, Sj.y), fmaf(-pj, eC.z, Sj.z) };
+            const Vec3 dl = { fmaf(-dpar, eC.x, dv.x), fmaf(-dpar, eC.y, dv.y), fmaf(-dpar, eC.z, dv.z) };
+            const Vec3 perp = { pj_perp.x + dl.x, pj_perp.y + dl.y, pj_perp.z + dl.z };
+            // P:189 radicand S_j^2 - |S'_j,perp|^2 in difference form: S_j,par^2 - delta.(2 S_j,perp + delta)
+            // (no cancellation against 1, so a follower lying almost perpendicular to e_C keeps its relative accuracy)
+            const Vec3 tw = { fmaf(2.0f, pj_perp.x, dl.x), fmaf(2.0f, pj_perp.y, dl.y), fmaf(2.0f, pj_perp.z, dl.z) };
+            const float rho = fmaf(pj, pj, -dot3(dl, tw));
+            float x = __int_as_float(0x7f800000);                                      // +inf: hard rejection (C-13)
+            bool ok = false;
+            Vec3 Snj = Sj;
+            if (rho > 0.0f) {
+                const float pnj = copysignf(rho * rsqrtf(rho), pj);                    // sign kept
+                Vec3 v = { fmaf(pnj, eC.x, perp.x), fmaf(pnj, eC.y, perp.y), fmaf(pnj, eC.z, perp.z) };
+                const float inv = fmaf(-0.5f, dot3(v, v), 1.5f);
+                Snj = { v.x * inv, v.y * inv, v.z * inv };
+                const float yml = (pni + pnj - pi_ - pj) * invML;                      // (M_L^ - M_L)/M_L
+                if (1.0f + yml > 0.0f) {                                               // M_L^ > 0 (C-13)
+                    const float lr = (fabsf(yml) < 0.03f) ? yml * (1.0f - yml * (0.5f - yml * (0.33333333f - 0.25f * yml)))
+                                                          : __logf(1.0f + yml);
+                    const Vec3 dj = { Snj.x - Sj.x, Snj.y - Sj.y, Snj.z - Sj.z };
+                    const Vec3 hBi = { fmaf(P.J, hL[k].x, B.x), fmaf(P.J, hL[k].y, B.y), fmaf(P.J, hL[k].z, B.z) };
+                    const Vec3 hBj = { fmaf(P.J, hj.x, B.x), fmaf(P.J, hj.y, B.y), fmaf(P.J, hj.z, B.z) };
+                    const float dE = delta_energy<ANISO>(Si, di, hBi, P.Ku, eL[(ANISO & 1) ? k : 0], P.Kc)
+                                   + delta_energy<ANISO>(Sj, dj, hBj, P.Ku, ej, P.Kc);  // P:193 (C-4)
+                    // P:193 in log form: dE/T - 2 ln(M_L^/M_L) - ln|S_j,par / S'_j,par| + ln u2 < 0
+                    x = fmaf(dE, invT, __logf(uniform01(r2))) - 2.0f * lr - __logf(__fdividef(fabsf(pj), fabsf(pnj)));
+                    ok = x < 0.0f;
+                }
+            }
+            if (ok) {
+                Si = Sni; nlx.v[k] = Sni.x; nly.v[k] = Sni.y; nlz.v[k] = Sni.z;
+                if (VEC == 4) {
+#pragma unroll
+                    for (int s = 0; s < 4; ++s) {
+                        const bool pick = ((k + rot) & 3u) == (uint32_t)s;
+                        nfx.v[s] = pick ? Snj.x : nfx.v[s]; nfy.v[s] = pick ? Snj.y : nfy.v[s]; nfz.v[s] = pick ? Snj.z : nfz.v[s];
+                    }
+                } else { nfx.v[0] = Snj.x; nfy.v[0] = Snj.y; nfz.v[0] = Snj.z; }
+            } else {
+                Snj = Sj;
+            }
+            cnt += ok ? 2 : 0;                                                         // P:195 (C-23)
+            if (dbg_x)   dbg_x[site_i] = x;
+            if (dbg_acc) { dbg_acc[site_i] = (uint8_t)ok; dbg_acc[site_j] = (uint8_t)ok; }
+            // fused sums of the final spins of both members
+            const Vec3 hJi = { P.J * hL[k].x, P.J * hL[k].y, P.J * hL[k].z }, hJj = { P.J * hj.x, P.J * hj.y, P.J * hj.z };
+            f[0] += Si.x + Snj.x; f[1] += Si.y + Snj.y; f[2] += Si.z + Snj.z;
+            if (colour == 1) f[3] -= dot3(Si, hJi) + dot3(Snj, hJj);
+            if (ANISO) f[4] += aniso_energy<ANISO>(Si, P.Ku, eL[(ANISO & 1) ? k : 0], P.Kc) + aniso_energy<ANISO>(Snj, P.Ku, ej, P.Kc);
+            f[5] -= dot3(Si, B) + dot3(Snj, B);
+            const Vec3 ti = onsite_torque<ANISO>(Si, P.Ku, eL[(ANISO & 1) ? k : 0], P.Kc, B);
+            const Vec3 tj = onsite_torque<ANISO>(Snj, P.Ku, ej, P.Kc, B);
+            f[6] += ti.x + tj.x; f[7] += ti.y + tj.y; f[8] += ti.z + tj.z;
+        }
+        st_rw<VEC>(Sc + aL, nlx); st_rw<VEC>(Sc + P.plane + aL, nly); st_rw<VEC>(Sc + 2 * P.plane + aL, nlz);
+        st_rw<VEC>(Sc + aF, nfx); st_rw<VEC>(Sc + P.plane + aF, nfy); st_rw<VEC>(Sc + 2 * P.plane + aF, nfz);
+#pragma unroll
+        for (int k = 0; k < NQ; ++k) acc[k] += (double)f[k];
+    }
+
+    block_partials(acc, cnt, P, colour);
+    if (threadIdx.x == 0) st->nblocks[colour] = gridDim.x;
+    if (flags & F_FINALIZE) {
+        if (last_block_done(st)) final_reduce(P, 0, flags);
+    }
+}
+
+// --------------------------------------------------------------------------------------------------------------
+// Layout conversion and state utilities
+// --------------------------------------------------------------------------------------------------------------
+// lexicographic [N][3] (x fastest) <-> colour-split planes.  to_split normalises every spin (fp32).
+__global__ void lex_to_split_kernel(const __grid_constant__ Params P, const float* __restrict__ lex)
+{
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= P.N) return;
+    const uint32_t x = s % (uint32_t)P.nx, row = s / (uint32_t)P.nx, y = row % (uint32_t)P.ny, z = row / (uint32_t)P.ny;
+    const uint32_t c = (x + y + z) & 1u, a = row * (uint32_t)P.R + (x >> 1);
+    float vx = lex[3ull * s], vy = lex[3ull * s + 1], vz = lex[3ull * s + 2];
+    const float n2 = vx * vx + vy * vy + vz * vz;
+    const float inv = (n2 > 0.0f) ? (float)(1.0 / sqrt((double)n2)) : 0.0f;
+    float* Sc = P.S + (long long)c * 3 * P.plane;
+    Sc[a] = vx * inv; Sc[P.plane + a] = vy * inv; Sc[2 * P.plane + a] = (n2 > 0.0f) ? vz * inv : 1.0f;
+}
+
+__global__ void split_to_lex_kernel(const __grid_constant__ Params P, float* __restrict__ lex)
+{
+    const uint32_t s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= P.N) return;
+    const uint32_t x = s % (uint32_t)P.nx, row = s / (uint32_t)P.nx, y = row % (uint32_t)P.ny, z = row / (uint32_t)P.ny;
+    const uint32_t c = (x + y + z) & 1u, a = row * (uint32_t)P.R + (x >> 1);
+    const float* Sc = P.S + (long long)c * 3 * P.plane;
+    lex[3ull * s] = Sc[a]; lex[3ull * s + 1] = Sc[P.plane + a]; lex[3ull * s + 2] = Sc[2 * P.plane + a];
+}
+
+__global__ void fill_kernel(const __grid_constant__ Params P, float vx, float vy, float vz)
+{
+    const uint32_t a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= P.Nc) return;
+    for (int c = 0; c < 2; ++c) {
+        float* Sc = P.S + (long long)c * 3 * P.plane;
+        Sc[a] = vx; Sc[P.plane + a] = vy; Sc[2 * P.plane + a] = vz;
+    }
+}
+
+// rigid rotation S <- Rm S of every spin, renormalised (C-12)
+struct Mat3 { float m[9]; };
+__global__ void rotate_kernel(const __grid_constant__ Params P, const __grid_constant__ Mat3 Rm)
+{
+    const uint32_t a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= P.Nc) return;
+    for (int c = 0; c < 2; ++c) {
+        float* Sc = P.S + (long long)c * 3 * P.plane;
+        const float x = Sc[a], y = Sc[P.plane + a], z = Sc[2 * P.plane + a];
+        const float rx = Rm.m[0] * x + Rm.m[1] * y + Rm.m[2] * z;
+        const float ry = Rm.m[3] * x + Rm.m[4] * y + Rm.m[5] * z;
+        const float rz = Rm.m[6] * x + Rm.m[7] * y + Rm.m[8] * z;
+        const float inv = rsqrtf(rx * rx + ry * ry + rz * rz);
+        Sc[a] = rx * inv; Sc[P.plane + a] = ry * inv; Sc[2 * P.plane + a] = rz * inv;
+    }
+}
+
+// small state edits on the stream (mc_set_cone / mc_set_sweep / mc_reset_accumulators / e_C / M_L)
+enum : int { ST_CONE = 0, ST_SWEEP = 1, ST_RESET_ACC = 2, ST_EC = 3, ST_ML = 4, ST_RESET_COUNT = 5 };
+__global__ void state_kernel(DevState* st, int what, double a, double b, double c, unsigned long long u)
+{
+    if (what == ST_CONE) { st->cone = a; st->one_minus_cos = (float)(1.0 - cos(a)); }
+    else if (what == ST_SWEEP) { st->sweep = u; }
+    else if (what == ST_RESET_ACC) {
+        st->n_samples = 0ull;
+        for (int i = 0; i < 4; ++i) { st->sum_m[i] = 0.0; st->sum_m2[i] = 0.0; }
+        st->sum_E = 0.0; st->sum_E2 = 0.0;
+        for (int i = 0; i < 3; ++i) st->sum_torque[i] = 0.0;
+    }
+    else if (what == ST_EC) { st->eC[0] = a; st->eC[1] = b; st->eC[2] = c; }
+    else if (what == ST_ML) { st->ML = a; }
+    else if (what == ST_RESET_COUNT) { st->count = 0ull; st->ticket = 0u; }
+}
+
+}  // namespace mc

@@ -1,0 +1,251 @@
+"""GPU ensemble parity and full-size checks (BASELINE.json configs c1-c5 through the C ABI).
+
+  * ensemble m(T), susceptibility, acceptance and cone agree with the oracle within 3 standard errors (north_star);
+  * the physics pins of SURVEY section 8(c) re-run on the GPU path at sizes the oracle cannot reach;
+  * one colour pass at BASELINE's FULL sizes (224^3, 2048x2048x4, 128^3 constrained), in the launch configuration
+    bench.py times, compared with the oracle site by site.
+"""
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+import pytest
+
+from stats_util import blocked_mean_se
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mods():
+    import torch
+    assert torch.cuda.is_available()
+    import oracle
+    from paper_2103_03517_b200 import binding, build, inputs
+    build.build()
+    return oracle, binding, inputs
+
+
+def _mag(tr):
+    return np.linalg.norm(tr[:, 2:5], axis=1)
+
+
+def _chi(m, N, T, nb=20):
+    """reduced susceptibility (N/T)(<m^2> - <m>^2) (Eq. 6, C-18) with a jackknife error over blocks."""
+    n = (len(m) // nb) * nb
+    b = m[:n].reshape(nb, -1)
+    m1, m2 = b.mean(axis=1), (b ** 2).mean(axis=1)
+    full = N / T * (m2.mean() - m1.mean() ** 2)
+    jk = np.array([N / T * (np.delete(m2, i).mean() - np.delete(m1, i).mean() ** 2) for i in range(nb)])
+    return full, np.sqrt((nb - 1) * jk.var())
+
+
+def test_c1_trace_acceptance_cone_and_m(mods):
+    """config c1: 16^3, K=0.01, T=1, +z start, 1000 adaptive sweeps from cone 0.5 rad, seed 42."""
+    oracle, binding, inputs = mods
+    g = binding.Lattice(16, 16, 16, Ku=0.01, cone0=0.5, adaptive=True, seed=42)
+    g.sweep(1.0, 1000)
+    tg = g.trace()
+    o = oracle.Oracle(16, 16, 16, Ku=0.01, cone0=0.5, adaptive=True, seed=42)
+    o.sweep(1.0, 1000)
+    to = o.trace()
+    assert len(tg) == 1000
+    # the first sweep starts from the identical state with the identical stream: same acceptance up to marginal sites
+    assert abs(tg[0, 0] - to[0, 0]) < 5 / 4096 and tg[0, 1] == to[0, 1] == 0.5
+    for col, tol in ((0, 0.01), (1, np.radians(1.5))):
+        assert abs(tg[300:, col].mean() - to[300:, col].mean()) < tol
+    mg, sg = blocked_mean_se(_mag(tg[300:])); mo, so = blocked_mean_se(_mag(to[300:]))
+    assert abs(mg - mo) < 3 * np.hypot(sg, so)
+    Eg, sg = blocked_mean_se(tg[300:, 5]); Eo, so = blocked_mean_se(to[300:, 5])
+    assert abs(Eg - Eo) < 3 * np.hypot(sg, so)
+    assert abs(tg[300:, 0].mean() - 0.5) < 0.02
+    print(f"\nc1: acceptance {tg[300:,0].mean():.4f} cone {np.degrees(tg[300:,1].mean()):.2f} deg m {mg:.4f} (oracle {mo:.4f}) E {Eg:.4f} (oracle {Eo:.4f})")
+    g.close()
+
+
+def test_ensemble_m_and_susceptibility_match_oracle(mods):
+    """config c2's Hamiltonian at 16^3: m(T), chi_l and chi_z from the GPU and from the oracle within 3 SE."""
+    oracle, binding, inputs = mods
+    Ts = (0.6, 1.2, 1.5, 1.8)
+    n_eq, n_s, L = 1000, 6000, 16
+    def run_oracle(T):
+        o = oracle.Oracle(L, L, L, Ku=0.01, cone0=0.5, seed=100 + int(10 * T))
+        o.set_sampling(False); o.sweep(T, n_eq); o.set_sampling(True); o.sweep(T, n_s)
+        return o.trace()
+    with ThreadPoolExecutor(4) as ex:
+        futs = [ex.submit(run_oracle, T) for T in Ts]
+        gtr = []
+        for T in Ts:
+            g = binding.Lattice(L, L, L, Ku=0.01, cone0=0.5, seed=200 + int(10 * T))
+            g.sweep(T, n_eq); g.reset_accumulators(); g.sweep(T, n_s)
+            gtr.append((g.trace(n_s), g.observables())); g.close()
+        otr = [f.result() for f in futs]
+    for T, (tg, ob), to in zip(Ts, gtr, otr):
+        assert len(tg) == n_s and ob.n_samples == n_s
+        mg, sg = blocked_mean_se(_mag(tg)); mo, so = blocked_mean_se(_mag(to))
+        assert abs(mg - mo) < 3 * np.hypot(sg, so), (T, mg, mo)
+        cg, scg = _chi(_mag(tg), L ** 3, T); co, sco = _chi(_mag(to), L ** 3, T)
+        assert abs(cg - co) < 3 * np.hypot(scg, sco), (T, cg, co)
+        # accumulators (Eq. 6) reproduce the trace
+        assert abs(ob.sum_m[0] / n_s - _mag(tg).mean()) < 1e-12
+        assert abs(ob.sum_m2[3] / n_s - (tg[:, 4] ** 2).mean()) < 1e-12
+        print(f"\nT={T}: m gpu {mg:.4f}+-{sg:.4f} oracle {mo:.4f}+-{so:.4f}; chi_l gpu {cg:.3f}+-{scg:.3f} oracle {co:.3f}+-{sco:.3f}")
+
+
+def test_gpu_physics_pins(mods):
+    oracle, binding, inputs = mods
+    # P-6 Langevin at 64^3: J = 0, field along z
+    g = binding.Lattice(64, 64, 64, J=0.0, B=(0, 0, 1.0), cone0=1.0, seed=1)
+    g.sweep(0.5, 100); g.sweep(0.5, 300)
+    m, se = blocked_mean_se(g.trace(300)[:, 4]); x = 2.0
+    assert abs(m - (1 / np.tanh(x) - 1 / x)) < 3 * se + 1e-4
+    g.close()
+    # P-10 / P-11 spin waves at 32^3, T = 0.02
+    L, K, T = 32, 0.01, 0.02
+    g = binding.Lattice(L, L, L, Ku=K, cone0=0.5, seed=2)
+    g.sweep(T, 3000); g.sweep(T, 3000)
+    tr = g.trace(3000)
+    k = 2 * np.pi * np.arange(L) / L
+    kx, ky, kz = np.meshgrid(k, k, k, indexing="ij")
+    eps = (2 * (3 - np.cos(kx) - np.cos(ky) - np.cos(kz)) + 2 * K).ravel()[1:]
+    assert abs(_mag(tr).mean() - (1 - T * np.sum(1 / eps) / L ** 3)) < 1e-4
+    assert abs(tr[:, 5].mean() - (-3 - K + T)) < 1e-3
+    s = g.get_spins()
+    assert np.abs(np.linalg.norm(s.astype(np.float64), axis=1) - 1).max() < 2e-7      # P-4 after 6000 sweeps
+    g.close()
+    # P-9 open chain
+    g = binding.Lattice(4096, 1, 1, periodic=(0, 0, 0), cone0=1.0, seed=3)
+    g.sweep(1.0, 300); g.sweep(1.0, 3000)
+    m, se = blocked_mean_se(g.trace(3000)[:, 5])
+    assert abs(m - (-(4095 / 4096) * (1 / np.tanh(1.0) - 1))) < 3 * se + 1e-4
+    g.close()
+
+
+def test_c2_temperature_sweep_tc_from_susceptibility_peak(mods):
+    """config c2: 64^3, K=0.01, T = 0.1..1.6 in 16 steps, +z start at every T.  (Sweep counts reduced 5x from
+    BASELINE's 5000+5000 to keep the test short; the schedule is otherwise the config's.)"""
+    oracle, binding, inputs = mods
+    L, n_eq, n_s = 64, 1000, 1000
+    Ts = [0.1 * k for k in range(1, 17)]
+    m, chi = [], []
+    for k, T in enumerate(Ts, start=1):
+        g = binding.Lattice(L, L, L, Ku=0.01, cone0=0.5, seed=42 + k)
+        g.sweep(T, n_eq); g.reset_accumulators(); g.sweep(T, n_s)
+        ob = g.observables()
+        ml = ob.sum_m[0] / ob.n_samples
+        m.append(ml); chi.append(L ** 3 / T * (ob.sum_m2[0] / ob.n_samples - ml ** 2))
+        g.close()
+    m, chi = np.array(m), np.array(chi)
+    print("\nc2 m(T):", np.round(m, 4)); print("c2 chi_l(T):", np.round(chi, 3))
+    assert np.all(np.diff(m) < 0)                                   # m decreases monotonically with T
+    # Bloch law with the paper's fit up to T = 1.2 (pin P-15)
+    for T, v in zip(Ts[:12], m[:12]):
+        assert abs(v - (1 - T / 1.4451) ** 0.340) < 0.03, (T, v)
+    ipk = int(np.argmax(chi))
+    assert Ts[ipk] in (1.4, 1.5)                                    # chi_l peaks at T_c = 1.443 on a 0.1 grid (P-14, C-19)
+    a, b, c = np.polyfit(Ts[ipk - 1: ipk + 2], chi[ipk - 1: ipk + 2], 2)
+    assert abs(-b / (2 * a) - 1.443) < 0.06
+    assert chi[0] < 0.05 * chi[ipk]                                 # chi_l -> 0 as T -> 0
+
+
+def test_c4_constrained_torque_on_gpu(mods):
+    """config c4 at 64^3 (one theta, three T): direction held (P-16), torque -> K(T) = K_u m^3 (P-18)."""
+    oracle, binding, inputs = mods
+    L, Ku, theta = 64, 0.05, np.pi / 4
+    e = np.array([np.sin(theta), 0, np.cos(theta)])
+    for T in (0.3, 0.8, 1.2):
+        g = binding.Lattice(L, L, L, Ku=Ku, cone0=0.5, seed=42)
+        g.constrained_sweep(T, theta, 0.0, 600); g.reset_accumulators(); g.constrained_sweep(T, theta, 0.0, 800)
+        ob = g.observables(); tr = g.trace(800)
+        assert np.abs(tr[:, 2:5] / _mag(tr)[:, None] - e).max() < 2e-6
+        tq = np.array(ob.sum_torque) / ob.n_samples
+        K = -tq[1] / np.sin(2 * theta) / Ku
+        m = ob.sum_m[0] / ob.n_samples
+        print(f"\nc4 T={T}: m={m:.4f} K(T)/Ku={K:.4f} m^3={m**3:.4f} acceptance={tr[:,0].mean():.3f}")
+        assert abs(K - m ** 3) < 0.03 * m ** 3 + 2e-3
+        assert abs(tr[200:, 0].mean() - 0.5) < 0.03
+        g.close()
+
+
+def test_constrained_ensemble_matches_oracle(mods):
+    oracle, binding, inputs = mods
+    L, T, theta = 16, 0.8, np.pi / 4
+    def run_oracle():
+        o = oracle.Oracle(L, L, L, Ku=0.05, cone0=0.5, seed=7)
+        o.set_sampling(False); o.constrained_sweep(T, theta, 0.0, 1000); o.set_sampling(True); o.constrained_sweep(T, theta, 0.0, 4000)
+        return o.trace(), o.observables()
+    with ThreadPoolExecutor(1) as ex:
+        fut = ex.submit(run_oracle)
+        g = binding.Lattice(L, L, L, Ku=0.05, cone0=0.5, seed=8)
+        g.constrained_sweep(T, theta, 0.0, 1000); g.reset_accumulators(); g.constrained_sweep(T, theta, 0.0, 4000)
+        tg, og = g.trace(4000), g.observables(); g.close()
+        to, oo = fut.result()
+    for f in (_mag, lambda t: t[:, 5]):
+        a, sa = blocked_mean_se(f(tg)); b, sb = blocked_mean_se(f(to))
+        assert abs(a - b) < 3 * np.hypot(sa, sb)
+    ty_g = og.sum_torque[1] / og.n_samples; ty_o = oo.sum_torque[1] / oo.n_samples
+    assert abs(ty_g - ty_o) < 0.02 * abs(ty_o)
+
+
+# ---------------------------------------------------------------------------------------------- full sizes
+def _full_size_half_sweep(mods, shape, T, cone, state_seed, ham, colour=0):
+    oracle, binding, inputs = mods
+    N = shape[0] * shape[1] * shape[2]
+    g = binding.Lattice(*shape, seed=42, cone0=cone, adaptive=False, **ham)
+    o = oracle.Oracle(*shape, seed=42, cone0=cone, adaptive=False, **ham)
+    g.set_spins(inputs.random_unit_spins(N, seed=state_seed))
+    g.set_sweep(1234); o.set_sweep(1234)
+    before = g.get_spins()
+    o.set_spins(before)
+    _, x_o, acc_o = o.half_sweep(T, colour, want_detail=True)
+    x_g, acc_g = g.half_sweep(T, colour, want_detail=True)
+    after_g = g.get_spins(); after_o = o.get_spins()
+    s = np.arange(N); col = ((s % shape[0]) + (s // shape[0]) % shape[1] + s // (shape[0] * shape[1])) & 1
+    mine = col == colour
+    differ = mine & (acc_g != acc_o)
+    assert (np.abs(x_o[differ]) < 1e-5).all()
+    agree = mine & ~differ
+    assert np.abs(after_g[agree].astype(np.float64) - after_o[agree]).max() < 1e-4
+    assert (after_g[~mine] == before[~mine]).all()
+    dx = np.abs(x_g[mine] - x_o[mine]).max()
+    print(f"\nfull size {shape}: {mine.sum()} updates, accepted {acc_g[mine].mean():.3f}, marginal flips {differ.sum()}, max |dx| {dx:.2e}")
+    g.close()
+
+
+def test_full_size_c3_half_sweep_parity(mods):
+    """config c3: 224^3 = 11.24 M spins, Kc = 0.01, T = 1.2, random-sphere start -- the headline launch configuration."""
+    _full_size_half_sweep(mods, (224, 224, 224), 1.2, 1.0, 42, dict(Kc=0.01), colour=1)
+
+
+def test_full_size_c5_half_sweep_parity(mods):
+    """config c5: 2048 x 2048 x 4 granular film (16.8 M spins), Voronoi grains, per-grain axes, open z."""
+    oracle, binding, inputs = mods
+    shape = (2048, 2048, 4)
+    mask, region, axes = inputs.voronoi_film(*shape, mean_diameter=40, seed=42)
+    _full_size_half_sweep(mods, shape, 0.5, 0.8, 43, dict(periodic=(1, 1, 0), Ku=0.02, bond_mask=mask, region=region, region_axis=axes))
+
+
+def test_full_size_c4_constrained_half_sweep_parity(mods):
+    """config c4: 128^3, K_u = 0.05, constrained pass at theta = 45 deg."""
+    oracle, binding, inputs = mods
+    shape, T, theta = (128, 128, 128), 0.8, np.pi / 4
+    N = 128 ** 3
+    e = np.array([np.sin(theta), 0.0, np.cos(theta)])
+    g = binding.Lattice(*shape, Ku=0.05, cone0=0.6, adaptive=False, seed=42)
+    o = oracle.Oracle(*shape, Ku=0.05, cone0=0.6, adaptive=False, seed=42)
+    g.set_spins(inputs.thermal_like_spins(N, seed=5, spread=0.5, direction=e))
+    g.set_sweep(9); o.set_sweep(9)
+    before = g.get_spins(); o.set_spins(before)
+    ML = float((before.astype(np.float64) @ e).sum())
+    _, _, x_o, acc_o = o.constrained_half_sweep(T, e, 0, ML, want_detail=True)
+    x_g, acc_g = g.constrained_half_sweep(T, theta, 0.0, 0, ML, want_detail=True)
+    after_g = g.get_spins().astype(np.float64); after_o = o.get_spins()
+    lead = ~np.isnan(x_o)
+    assert (lead == ~np.isnan(x_g)).all()                                  # identical pairing roles at full size
+    differ = lead & (acc_g != acc_o)
+    assert (np.abs(x_o[differ]) < 1e-5).all()
+    s = np.arange(N); col = ((s % 128) + (s // 128) % 128 + s // (128 * 128)) & 1
+    same = (acc_g == acc_o) & (col == 0)
+    assert np.abs(after_g[same] - after_o[same]).max() < 1e-4
+    fin = lead & np.isfinite(x_o) & np.isfinite(x_g)
+    print(f"\nfull size c4 constrained: pairs {lead.sum()}, accepted {acc_g[lead].mean():.3f}, flips {differ.sum()}, max |dx| {np.abs(x_g[fin]-x_o[fin]).max():.2e}")
+    g.close()

@@ -1,0 +1,273 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element, on seeded inputs.
+
+The bar (BASELINE.json north_star; reading C-14): ONE colour pass from an identical fp32 state --
+  * spins agree to 1e-4 max abs wherever the decisions agree;
+  * accept/reject decisions may differ only where the oracle's |x| < 1e-5, x = dE/T + ln u2 (constrained: the
+    log form of P:193);
+and (measured, not required) the GPU's own fp32 x stays within a few 1e-6 of the oracle's.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+X_BAND = 1e-5       # decisions may differ only inside this band of the oracle's decision variable
+SPIN_TOL = 1e-4     # max abs spin difference where decisions agree
+
+
+@pytest.fixture(scope="module")
+def mods():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    import oracle
+    from paper_2103_03517_b200 import binding, build, inputs
+    build.build()
+    return oracle, binding, inputs
+
+
+def _colour(shape):
+    nx, ny, nz = shape
+    s = np.arange(nx * ny * nz)
+    return ((s % nx) + (s // nx) % ny + s // (nx * ny)) & 1
+
+
+def _pair(mods, shape, seed=42, cone=0.5, sweep=0, **ham):
+    oracle, binding, inputs = mods
+    o = oracle.Oracle(*shape, seed=seed, cone0=cone, adaptive=False, **ham)
+    g = binding.Lattice(*shape, seed=seed, cone0=cone, adaptive=False, **ham)
+    o.set_sweep(sweep); g.set_sweep(sweep)
+    return o, g
+
+
+def _check_half_sweep(o, g, T, colour, shape, allow_flips=True):
+    """One colour pass on both sides from the GPU's current fp32 state.  Returns (n_flips, max |x_gpu - x_oracle|)."""
+    before = g.get_spins()
+    o.set_spins(before)                                  # identical state: the oracle takes the fp32 values
+    n_o, x_o, acc_o = o.half_sweep(T, colour, want_detail=True)
+    x_g, acc_g = g.half_sweep(T, colour, want_detail=True)
+    after_g = g.get_spins().astype(np.float64); after_o = o.get_spins()
+    col = _colour(shape)
+    mine = col == colour
+    # the other colour is untouched, bit for bit
+    assert (after_g[~mine] == before[~mine].astype(np.float64)).all()
+    # every site of this colour got a decision variable
+    assert not np.isnan(x_g[mine]).any()
+    differ = mine & (acc_g != acc_o)
+    assert (np.abs(x_o[differ]) < X_BAND).all(), f"decision differs outside the band: {np.abs(x_o[differ]).max()}"
+    if not allow_flips:
+        assert differ.sum() == 0
+    agree = mine & ~differ
+    assert np.abs(after_g[agree] - after_o[agree]).max() < SPIN_TOL
+    # accepted <=> changed, rejected <=> bit-identical
+    changed = (after_g != before.astype(np.float64)).any(axis=1)
+    assert (changed[mine] == (acc_g[mine] == 1)).all()
+    # unit norm (pin P-4, GPU bound)
+    assert np.abs(np.linalg.norm(after_g, axis=1) - 1).max() < 2e-7
+    # accuracy of the GPU's own fp32 decision variable where it matters: near the decision boundary
+    near = mine & (np.abs(x_o) < 2.0)
+    return int(differ.sum()), float(np.abs(x_g[near] - x_o[near]).max()) if near.any() else 0.0
+
+
+CASES = [
+    # (shape, T, cone, ham kwargs)                                         what it covers
+    ((16, 16, 16), 1.0, 0.5, dict(Ku=0.01)),                              # c1: VEC=4, one CTA row tiles
+    ((24, 10, 6), 0.7, 1.2, dict(Kc=0.3, B=(0.1, -0.05, 0.2))),           # VEC=4, ragged rows (R=12), cubic + field
+    ((40, 12, 10), 1.44, 2.0, dict(Kc=0.01)),                              # c3 parameters, several CTAs + tail
+    ((6, 4, 4), 1.0, 0.8, dict(Ku=0.2, eu=(0.3, -0.5, 0.81))),            # VEC=1 path (nx % 8 != 0), tilted axis
+    ((2, 2, 2), 3.0, np.pi, dict(Ku=0.1)),                                 # L = 2: every neighbour counted twice
+    ((8, 6, 5), 0.9, 1.0, dict(periodic=(1, 0, 0), Ku=0.05, Kc=0.1)),      # open faces, odd open dims, both anisotropies
+    ((2, 1, 1), 1.0, 1.5, dict(periodic=(0, 0, 0))),                       # the dimer
+    ((64, 64, 64), 0.1, 0.3, dict(Ku=0.01)),                               # c2 first T-point (low T, random state = worst case)
+]
+
+
+@pytest.mark.parametrize("shape,T,cone,ham", CASES)
+def test_half_sweep_parity_random_state(mods, shape, T, cone, ham):
+    oracle, binding, inputs = mods
+    o, g = _pair(mods, shape, cone=cone, sweep=(3 << 32) | 12345, **ham)
+    g.set_spins(inputs.random_unit_spins(g.N, seed=7))
+    worst = 0.0; flips = 0
+    for colour in (0, 1, 0, 1):
+        f, dx = _check_half_sweep(o, g, T, colour, shape)
+        flips += f; worst = max(worst, dx)
+    print(f"\n{shape} T={T}: decision flips {flips}, max |x_gpu - x_oracle| = {worst:.2e}")
+    assert worst < X_BAND      # |x_gpu - x_oracle| over the sites with |x_oracle| < 2 (where a decision can flip)
+    g.close()
+
+
+def test_half_sweep_parity_masked_and_grain_axes(mods):
+    """config c5 at reduced size: Voronoi film, J = 0 across grain boundaries, per-grain easy axes, open top/bottom."""
+    oracle, binding, inputs = mods
+    shape = (64, 48, 4)
+    mask, region, axes = inputs.voronoi_film(*shape, mean_diameter=12, seed=3)
+    ham = dict(periodic=(1, 1, 0), Ku=0.02, bond_mask=mask, region=region, region_axis=axes)
+    for T, cone, state in ((0.1, 0.25, "ordered"), (1.0, 1.0, "random")):
+        o, g = _pair(mods, shape, cone=cone, sweep=99, **ham)
+        g.set_spins(inputs.thermal_like_spins(g.N, 5, 0.15) if state == "ordered" else inputs.random_unit_spins(g.N, 5))
+        for colour in (0, 1):
+            f, dx = _check_half_sweep(o, g, T, colour, shape)
+            print(f"\nfilm {state} T={T} colour {colour}: flips {f}, max dx {dx:.2e}")
+        g.close()
+    # random symmetric dilution on a periodic lattice, scalar path
+    shape = (6, 6, 4)
+    m2 = inputs.random_bond_mask(*shape, (1, 1, 1), seed=4, p_cut=0.3)
+    o, g = _pair(mods, shape, cone=1.0, Ku=0.1, bond_mask=m2)
+    g.set_spins(inputs.random_unit_spins(g.N, 6))
+    for colour in (0, 1):
+        _check_half_sweep(o, g, 0.8, colour, shape)
+    g.close()
+
+
+@pytest.mark.parametrize("T,spread,cone", [(0.1, 0.15, 0.25), (0.02, 0.06, 0.1), (0.5, 0.4, 0.6)])
+def test_low_temperature_decision_accuracy(mods, T, spread, cone):
+    """the fp32 decision variable must stay inside the 1e-5 band at low T on thermal-looking states."""
+    oracle, binding, inputs = mods
+    shape = (32, 32, 32)
+    o, g = _pair(mods, shape, cone=cone, sweep=5, Ku=0.01)
+    g.set_spins(inputs.thermal_like_spins(g.N, seed=11, spread=spread))
+    worst = 0.0
+    for colour in (0, 1):
+        f, dx = _check_half_sweep(o, g, T, colour, shape)
+        worst = max(worst, dx)
+    print(f"\nT={T}: max |x_gpu - x_oracle| = {worst:.2e}")
+    # T >= 0.1 is BASELINE's range: the GPU's fp32 x itself must stay inside the band.  T = 0.02 is outside it; there the
+    # fp32 resolution of dE/T (~1e-7 |h||d| / T) is the limit and only the decision rule (checked above) is required.
+    assert worst < (X_BAND if T >= 0.1 else 3e-5)
+    g.close()
+
+
+def test_sweep_equals_hooks_and_is_deterministic(mods):
+    oracle, binding, inputs = mods
+    shape = (24, 16, 8)
+    s0 = inputs.random_unit_spins(24 * 16 * 8, seed=1)
+    def run(kind):
+        g = binding.Lattice(*shape, Ku=0.01, cone0=0.5, adaptive=True, seed=42)
+        g.set_spins(s0)
+        if kind == "one":
+            g.sweep(1.0, 12)
+        elif kind == "split":
+            for n in (1, 5, 6): g.sweep(1.0, n)
+        else:
+            for _ in range(12):
+                g.half_sweep(1.0, 0); g.half_sweep(1.0, 1); g.end_sweep()
+        out = g.get_spins(), g.trace(), g.observables()
+        g.close()
+        return out
+    a, ta, oa = run("one"); b, tb, ob = run("split"); c, tc, oc = run("hooks"); d, td, od = run("one")
+    assert (a == b).all() and (a == c).all() and (a == d).all()          # P-20: bit-identical spins
+    assert (ta == tb).all() and (ta == tc).all() and (ta == td).all()    # bitwise reproducible reductions
+    assert oa.sweep == 12 and len(ta) == 12
+    assert np.allclose(np.abs(np.diff(ta[:, 1])), np.pi / 180, atol=1e-14)   # controller: exact 1 degree steps (P-19)
+
+
+def test_observables_match_oracle(mods):
+    oracle, binding, inputs = mods
+    shape = (16, 12, 6)
+    mask = inputs.boundary_mask(*shape, (1, 1, 0))
+    kw = dict(periodic=(1, 1, 0), J=0.8, Ku=0.3, eu=(0.2, 0.1, 0.9), Kc=0.4, B=(0.1, 0.2, -0.3))
+    o, g = _pair(mods, shape, **kw)
+    s = inputs.random_unit_spins(g.N, 3)
+    g.set_spins(s); o.set_spins(g.get_spins())
+    a, b = g.observables(), o.observables()
+    for name in ("m", "E_total", "E_exch", "E_aniso", "E_zeeman"):
+        assert abs(getattr(a, name) - getattr(b, name)) < 2e-6, name
+    assert np.allclose(list(a.M), list(b.M), atol=1e-6) and np.allclose(list(a.torque), list(b.torque), atol=1e-6)
+    # fused per-sweep values (trace) agree with a fresh measurement of the post-sweep state
+    g.sweep(0.9, 3)
+    tr = g.trace(); ob = g.observables()
+    assert np.allclose(tr[-1, 2:5], list(ob.M), atol=1e-6) and abs(tr[-1, 5] - ob.E_total) < 2e-6
+    assert ob.n_samples == 3 and abs(ob.sum_E - tr[:, 5].sum()) < 1e-12
+    g.close()
+
+
+def test_set_get_roundtrip_and_init(mods):
+    oracle, binding, inputs = mods
+    g = binding.Lattice(8, 6, 4, periodic=(1, 1, 1))
+    s = inputs.random_unit_spins(g.N, 9)
+    g.set_spins(s)
+    assert np.abs(g.get_spins() - s).max() < 1.2e-7
+    g.init_spins(1, (1, 1, 0))
+    assert np.allclose(g.get_spins(), np.array([1, 1, 0]) / np.sqrt(2), atol=1e-7)
+    assert abs(g.observables().m - 1) < 1e-6
+    g.close()
+
+
+def test_error_paths(mods):
+    oracle, binding, inputs = mods
+    g = binding.Lattice(8, 4, 4)
+    with pytest.raises(binding.McError): g.sweep(0.0, 1)                 # C-16
+    with pytest.raises(binding.McError): g.sweep(-1.0, 1)
+    with pytest.raises(binding.McError): g.set_cone(0.0)
+    g.set_spins(inputs.random_unit_spins(g.N, 1) * np.array([1, 1, 0], np.float32) + np.array([0, 0, 1e-9], np.float32))
+    bad = binding.Lattice(6, 3, 1, periodic=(1, 0, 0))                   # 9 sites per colour: odd (C-15)
+    with pytest.raises(binding.McError): bad.constrained_sweep(1.0, 0.0, 0.0, 1)
+    m = inputs.boundary_mask(8, 4, 4, (1, 1, 1)); m[0] &= 0xFE            # asymmetric mask
+    with pytest.raises(binding.McError): binding.Lattice(8, 4, 4, bond_mask=m)
+    g.close(); bad.close()
+
+
+# ------------------------------------------------------------------------------------------ constrained path
+CCASES = [
+    ((16, 16, 16), 0.8, 0.6, dict(Ku=0.05)),            # VEC=4, B=32
+    ((8, 8, 8), 1.0, 1.0, dict(Ku=0.05, Kc=0.02)),      # VEC=4, B=32, H=8
+    ((12, 4, 2), 0.9, 0.9, dict(Ku=0.1)),               # VEC=1, B=8
+    ((6, 6, 2), 0.9, 0.9, dict()),                      # VEC=1, B=2
+    ((32, 16, 8), 0.3, 0.3, dict(Ku=0.05)),             # lower T
+]
+
+
+@pytest.mark.parametrize("shape,T,cone,ham", CCASES)
+def test_constrained_half_sweep_parity(mods, shape, T, cone, ham):
+    oracle, binding, inputs = mods
+    theta, phi = 0.7, 0.4
+    e = np.array([np.sin(theta) * np.cos(phi), np.sin(theta) * np.sin(phi), np.cos(theta)])
+    o, g = _pair(mods, shape, cone=cone, sweep=77, **ham)
+    g.set_spins(inputs.thermal_like_spins(g.N, seed=2, spread=0.5, direction=e))
+    col = _colour(shape)
+    worst = 0.0
+    for colour in (0, 1):
+        before = g.get_spins()
+        o.set_spins(before)
+        ML = float((before.astype(np.float64) @ e).sum())
+        n_o, ml_o, x_o, acc_o = o.constrained_half_sweep(T, e, colour, ML, want_detail=True)
+        x_g, acc_g = g.constrained_half_sweep(T, theta, phi, colour, ML, want_detail=True)
+        after_g = g.get_spins().astype(np.float64); after_o = o.get_spins()
+        mine = col == colour
+        assert (after_g[~mine] == before[~mine].astype(np.float64)).all()
+        # same pairing: leaders are exactly the sites that carry a decision variable
+        partner, lead = o.pairing(77, colour)
+        lead_sites = np.array([o.site_of(colour, a) for a in np.nonzero(lead)[0]])
+        foll_sites = np.array([o.site_of(colour, partner[a]) for a in np.nonzero(lead)[0]])
+        assert not np.isnan(x_g[lead_sites]).any() and np.isnan(x_g[foll_sites]).all()
+        assert (acc_g[lead_sites] == acc_g[foll_sites]).all()
+        differ = acc_g[lead_sites] != acc_o[lead_sites]
+        xo = x_o[lead_sites]
+        assert (np.abs(xo[differ]) < X_BAND).all(), np.abs(xo[differ]).max()
+        ok_pairs = ~differ
+        for sites in (lead_sites[ok_pairs], foll_sites[ok_pairs]):
+            assert np.abs(after_g[sites] - after_o[sites]).max() < SPIN_TOL
+        fin = np.isfinite(xo) & np.isfinite(x_g[lead_sites])
+        assert (np.isfinite(xo) == np.isfinite(x_g[lead_sites])).mean() > 0.999
+        worst = max(worst, float(np.abs(x_g[lead_sites][fin] - xo[fin]).max()))
+        assert np.abs(np.linalg.norm(after_g, axis=1) - 1).max() < 3e-7
+        # transverse magnetisation is conserved by every accepted pair (P-16, fp32)
+        Mb = before.astype(np.float64).sum(axis=0); Ma = after_g.sum(axis=0)
+        perp = (Ma - Mb) - ((Ma - Mb) @ e) * e
+        assert np.abs(perp).max() < 1e-6 * np.sqrt(g.N) + 1e-5
+    print(f"\nconstrained {shape} T={T}: max |x_gpu - x_oracle| = {worst:.2e}")
+    g.close()
+
+
+def test_align_rotation_matches_oracle(mods):
+    oracle, binding, inputs = mods
+    shape = (16, 8, 8)
+    o, g = _pair(mods, shape, Ku=0.05)
+    s = inputs.thermal_like_spins(g.N, seed=4, spread=0.6, direction=(0.3, -0.2, 0.9))
+    g.set_spins(s); o.set_spins(g.get_spins())
+    theta, phi = 1.1, -0.7
+    e = np.array([np.sin(theta) * np.cos(phi), np.sin(theta) * np.sin(phi), np.cos(theta)])
+    g.align_to(theta, phi); assert o.align_to(e) == 0
+    assert np.abs(g.get_spins() - o.get_spins()).max() < 1e-6
+    ob = g.observables()
+    assert np.allclose(np.array(ob.M) / ob.m, e, atol=1e-6)
+    g.close()
