@@ -9,7 +9,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libmc_b200.so")
 SOURCES = [os.path.join(CSRC, "mc_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "mc_kernels.cuh"), os.path.join(CSRC, "mc_device.cuh"),
+DEPS = SOURCES + [os.path.join(CSRC, "mc_kernels.cuh"), os.path.join(CSRC, "mc_device.cuh"), os.path.join(CSRC, "mc_tile.cuh"),
                   os.path.join(os.path.dirname(_HERE), "include", "mc.h")]
 
 NVCC_FLAGS = [
@@ -31,7 +31,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
         return LIB
     tmp = f"{LIB}.{os.getpid()}.tmp"
-    cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
+    extra = os.environ.get("MC_B200_NVCC_EXTRA", "").split()      # experiments only (e.g. -DMC_TILE_MIN_BLOCKS=3)
+    cmd = [nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)
     return LIB

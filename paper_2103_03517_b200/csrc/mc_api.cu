@@ -3,6 +3,7 @@
 // of mc_kernels.cuh; there is no CPU fallback (without a device every entry point returns MC_ECUDA).
 #include "../../include/mc.h"
 #include "mc_kernels.cuh"
+#include "mc_tile.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -86,6 +87,8 @@ struct mc_ctx {
     Geom geom;
     PairGeom pgeom;
     bool pair_ok;
+    bool tile_ok; TileGeom tgeom; int tile_threads; size_t tile_smem;   // fast path of the colour pass (mc_tile.cuh)
+    bool field;
     int vec, aniso;
     bool masked;
     cudaStream_t stream;
@@ -132,6 +135,87 @@ template <int VEC> PairFn pick_pair(int aniso, bool masked)
     }
 }
 
+typedef void (*TileFn)(const Params, const TileGeom, int, float, int, float*, uint8_t*);
+template <int RT, bool DEBUG> TileFn pick_tile_rt(int aniso, bool field)
+{
+    switch (aniso * 2 + (field ? 1 : 0)) {
+        case 0: return tile_pass_kernel<0, false, RT, DEBUG>;  case 1: return tile_pass_kernel<0, true, RT, DEBUG>;
+        case 2: return tile_pass_kernel<1, false, RT, DEBUG>;  case 3: return tile_pass_kernel<1, true, RT, DEBUG>;
+        case 4: return tile_pass_kernel<2, false, RT, DEBUG>;  case 5: return tile_pass_kernel<2, true, RT, DEBUG>;
+        case 6: return tile_pass_kernel<3, false, RT, DEBUG>;  default: return tile_pass_kernel<3, true, RT, DEBUG>;
+    }
+}
+// Row lengths with a specialised instantiation (every shared-memory offset an immediate): R = nx/2 of BASELINE's
+// periodic configs c2 (64^3), c4 (128^3) and c3 (224^3).  Any other R runs the run-time-R instantiation.
+// The decision-variable debug outputs of the test hooks exist only in the run-time-R instantiation (same arithmetic).
+TileFn pick_tile(int R, int Ty, bool debug, int aniso, bool field)
+{
+    if (debug) return pick_tile_rt<0, true>(aniso, field);
+    if (getenv("MC_B200_NO_RT") || Ty != TILE_TY_RT) return pick_tile_rt<0, false>(aniso, field);
+    switch (R) {
+        case 32:  return pick_tile_rt<32, false>(aniso, field);
+        case 64:  return pick_tile_rt<64, false>(aniso, field);
+        case 112: return pick_tile_rt<112, false>(aniso, field);
+        default:  return pick_tile_rt<0, false>(aniso, field);
+    }
+}
+
+// Chooses the slab / segment decomposition of the tiled colour pass.  Returns false when the
+// lattice is not eligible (then the generic pass_kernel runs).
+bool plan_tile(mc_ctx* c)
+{
+    c->tile_ok = false;
+    const mc_lattice& lat = c->lat;
+    if (c->masked || c->P.region) return false;
+    if (!(lat.periodic[0] && lat.periodic[1] && lat.periodic[2])) return false;
+    const int R = lat.nx / 2;
+    if (R % 4) return false;                                    // TMA bulk copies move whole rows: 16-byte multiples
+    const int PR = R / 2;
+    int max_threads = TILE_MAX_THREADS, want_rp = 0, want_np = 0, want_segs = 0;
+    if (const char* env = getenv("MC_B200_TILE")) sscanf(env, "%d,%d,%d,%d", &want_rp, &want_np, &want_segs, &max_threads);
+    if (max_threads > TILE_MAX_THREADS) max_threads = TILE_MAX_THREADS;
+    if (PR > max_threads) return false;
+    TileGeom& G = c->tgeom;
+    G.R = R; G.PR = PR; G.nx = lat.nx; G.ny = lat.ny; G.nz = lat.nz;
+    int RP = 1;
+    for (int d = 1; d <= lat.ny; ++d) if (lat.ny % d == 0 && PR * d <= max_threads) RP = d;
+    if (want_rp > 0 && lat.ny % want_rp == 0 && PR * want_rp <= TILE_MAX_THREADS) RP = want_rp;
+    int NP = 1;
+    const size_t smem_cap = (size_t)(220 * 1024) / TILE_MIN_BLOCKS - 3 * 1024;   // TILE_MIN_BLOCKS CTAs per SM
+    auto slot_bytes = [&](int ty) { return (size_t)3 * (ty + 2) * R * sizeof(float); };
+    if (lat.ny % (2 * RP) == 0 && TILE_NSLOT * slot_bytes(2 * RP) <= smem_cap) NP = 2;
+    if (want_np > 0 && lat.ny % (want_np * RP) == 0) NP = want_np;
+    G.RP = RP; G.NPASS = NP; G.Ty = RP * NP;
+    G.n_slabs = lat.ny / G.Ty;
+    G.slot_floats = 3 * (G.Ty + 2) * R;
+    G.n_active = PR * RP;
+    c->tile_threads = (G.n_active + 31) / 32 * 32;
+    c->tile_smem = TILE_NSLOT * slot_bytes(G.Ty);
+    if (c->tile_smem > 200 * 1024) return false;
+    // every instantiation this handle can launch must be allowed its dynamic shared memory
+    TileFn fns[2] = { pick_tile(R, G.Ty, false, c->aniso, c->field), pick_tile(R, G.Ty, true, c->aniso, c->field) };
+    int per_sm = 1;
+    for (TileFn f : fns) {
+        if (cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tile_smem) != cudaSuccess) { cudaGetLastError(); return false; }
+    }
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fns[0], c->tile_threads, c->tile_smem) != cudaSuccess || per_sm < 1) { cudaGetLastError(); return false; }
+    // one wave of CTAs: n_segs z-segments per slab so that n_slabs * n_segs fills sm_count * per_sm slots
+    long long slots = (long long)c->sm_count * per_sm;
+    int n_segs = (int)(slots / G.n_slabs);
+    if (n_segs < 1) n_segs = 1;
+    if (n_segs > lat.nz) n_segs = lat.nz;
+    if (want_segs > 0 && want_segs <= lat.nz) n_segs = want_segs;
+    G.n_segs = n_segs; G.Lz = lat.nz / n_segs; G.Lz_rem = lat.nz % n_segs;
+    if ((long long)G.n_slabs * G.n_segs > c->P.max_blocks) return false;
+    c->tile_ok = true;
+    if (const char* env = getenv("MC_B200_PATH")) { if (!strcmp(env, "generic")) c->tile_ok = false; }
+    else if (c->P.Nc < 65536u) c->tile_ok = false;              // small lattices are launch-bound: the generic kernel has less prologue
+    if (getenv("MC_B200_VERBOSE"))
+        fprintf(stderr, "mc tile plan: ok=%d R=%d PR=%d RP=%d NPASS=%d Ty=%d slabs=%d segs=%d Lz=%d(+%d) threads=%d smem=%zu ctas/SM=%d\n",
+                (int)c->tile_ok, R, PR, RP, NP, G.Ty, G.n_slabs, G.n_segs, G.Lz, G.Lz_rem, c->tile_threads, c->tile_smem, per_sm);
+    return c->tile_ok;
+}
+
 int grid_for(const mc_ctx* c, uint32_t n_threads_needed)
 {
     const long long need = ((long long)n_threads_needed + BLOCK - 1) / BLOCK;
@@ -143,6 +227,14 @@ int grid_for(const mc_ctx* c, uint32_t n_threads_needed)
 
 int launch_pass(mc_ctx* ctx, int mode, int colour, float invT, int flags, float* dx, uint8_t* da)
 {
+    if (mode == MODE_SWEEP && ctx->tile_ok) {
+        TileFn fn = pick_tile(ctx->tgeom.R, ctx->tgeom.Ty, dx || da, ctx->aniso, ctx->field);
+        const int grid = ctx->tgeom.n_slabs * ctx->tgeom.n_segs;
+        fn<<<grid, ctx->tile_threads, ctx->tile_smem, ctx->stream>>>(ctx->P, ctx->tgeom, colour, invT, flags, dx, da);
+        ctx->launches += 1;
+        CU(cudaGetLastError());
+        return MC_OK;
+    }
     PassFn fn = (ctx->vec == 4) ? (mode == MODE_SWEEP ? pick_pass<4, MODE_SWEEP>(ctx->aniso, ctx->masked) : pick_pass<4, MODE_MEASURE>(ctx->aniso, ctx->masked))
                                 : (mode == MODE_SWEEP ? pick_pass<1, MODE_SWEEP>(ctx->aniso, ctx->masked) : pick_pass<1, MODE_MEASURE>(ctx->aniso, ctx->masked));
     const int grid = grid_for(ctx, ctx->geom.n_items);
@@ -243,10 +335,12 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     P.J = (float)ham->J; P.Ku = (float)ham->Ku; P.Kc = (float)ham->Kc;
     for (int a = 0; a < 3; ++a) { P.eu[a] = (float)ctx->eu[a]; P.B[a] = (float)ham->B[a]; }
     P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32);
+    P.key = philox_key(P.seed_lo, P.seed_hi);
     P.st = (DevState*)(ws + L.state); P.partials = (double*)(ws + L.partials); P.max_blocks = L.max_blocks;
     P.trace = (double*)(ws + L.trace);
 
     ctx->aniso = (ham->Ku != 0.0 ? 1 : 0) | (ham->Kc != 0.0 ? 2 : 0);
+    ctx->field = ham->B[0] != 0.0 || ham->B[1] != 0.0 || ham->B[2] != 0.0;
     ctx->masked = needs_mask(lat, ham);
     ctx->vec = (nx % 8 == 0) ? 4 : 1;
     ctx->geom.RV = R / ctx->vec; ctx->geom.n_items = Nc / ctx->vec;
@@ -323,6 +417,8 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
         P.region = (const uint16_t*)(ws + L.region);
         P.axis = (const float4*)(ws + L.axis);
     }
+
+    plan_tile(ctx);
 
     // ---- device state
     DevState st; memset(&st, 0, sizeof st);

@@ -21,7 +21,7 @@ struct PhiloxKey {            // the 10 round keys, precomputed once per thread 
     uint32_t k0[10], k1[10];
 };
 
-__device__ __forceinline__ PhiloxKey philox_key(uint32_t seed_lo, uint32_t seed_hi)
+__host__ __device__ __forceinline__ PhiloxKey philox_key(uint32_t seed_lo, uint32_t seed_hi)
 {
     PhiloxKey k;
 #pragma unroll

@@ -14,7 +14,8 @@
 namespace mc {
 
 constexpr int NQ = 9;          // fused sums: Mx My Mz E_exch E_aniso E_zeeman tq_x tq_y tq_z (extensive, fp64)
-constexpr int BLOCK = 256;     // threads per CTA of the pass kernels
+constexpr int BLOCK = 256;     // threads per CTA of the generic pass kernels
+constexpr int MAX_WARPS = 16;  // largest CTA any kernel that reduces uses (512 threads); block sizes are warp multiples
 constexpr int TRACE_CAP = 16384;
 
 // Controller / reduction state, resident in the workspace (no host round trip per sweep: P:165-171 runs on the device)
@@ -49,6 +50,7 @@ struct Params {
     float J, Ku, Kc;
     float eu[3], B[3];
     uint32_t seed_lo, seed_hi;
+    PhiloxKey key;                   // the 10 round keys of (seed_lo, seed_hi), filled by the host: constant-bank operands
     DevState* st;
     double* partials;                // [4][max_blocks][NQ]: slots 0,1 = sweep red/black, 2,3 = measurement red/black
     int max_blocks;
@@ -195,9 +197,9 @@ __device__ __forceinline__ double warp_sum(double v)
 
 __device__ __forceinline__ void block_partials(const double (&acc)[NQ], int cnt, const Params& P, int slot)
 {
-    __shared__ double sm[BLOCK / 32][NQ];
+    __shared__ double sm[MAX_WARPS][NQ];
     __shared__ int scnt;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = (int)(blockDim.x >> 5);
     if (threadIdx.x == 0) scnt = 0;
     __syncthreads();
     const int wc = __reduce_add_sync(0xffffffffu, cnt);
@@ -207,8 +209,7 @@ __device__ __forceinline__ void block_partials(const double (&acc)[NQ], int cnt,
     __syncthreads();
     if (threadIdx.x < NQ) {
         double v = 0.0;
-#pragma unroll
-        for (int w = 0; w < BLOCK / 32; ++w) v += sm[w][threadIdx.x];
+        for (int w = 0; w < nwarps; ++w) v += sm[w][threadIdx.x];
         P.partials[((long long)slot * P.max_blocks + blockIdx.x) * NQ + threadIdx.x] = v;
     }
     if (threadIdx.x == 0 && scnt) atomicAdd(&P.st->count, (unsigned long long)scnt);
@@ -218,14 +219,15 @@ __device__ __forceinline__ void block_partials(const double (&acc)[NQ], int cnt,
 // P:205-209; C-2, C-3, C-9), sweep counter, Eq. (6) accumulators, trace row.  mode 0: end of a sweep; 1: measurement.
 __device__ void final_reduce(const Params& P, int mode, int flags)
 {
-    __shared__ double red[BLOCK / 32][NQ];
+    __shared__ double red[MAX_WARPS][NQ];
     DevState* st = P.st;
+    const int nwarps = (int)(blockDim.x >> 5);
     double acc[NQ];
 #pragma unroll
     for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
     for (int slot = 2 * mode; slot < 2 * mode + 2; ++slot) {
         const unsigned nb = __ldcg(&st->nblocks[slot]);
-        for (unsigned b = threadIdx.x; b < nb; b += BLOCK) {
+        for (unsigned b = threadIdx.x; b < nb; b += blockDim.x) {
             const double* p = P.partials + ((long long)slot * P.max_blocks + b) * NQ;
 #pragma unroll
             for (int q = 0; q < NQ; ++q) acc[q] += __ldcg(p + q);
@@ -237,7 +239,7 @@ __device__ void final_reduce(const Params& P, int mode, int flags)
     __syncthreads();
     if (threadIdx.x == 0) {
         double s[NQ];
-        for (int q = 0; q < NQ; ++q) { double v = 0.0; for (int w = 0; w < BLOCK / 32; ++w) v += red[w][q]; s[q] = v; }
+        for (int q = 0; q < NQ; ++q) { double v = 0.0; for (int w = 0; w < nwarps; ++w) v += red[w][q]; s[q] = v; }
         st->ML = s[0] * st->eC[0] + s[1] * st->eC[1] + s[2] * st->eC[2];
         if (mode == 1) {
             for (int q = 0; q < NQ; ++q) st->meas[q] = s[q];
@@ -300,7 +302,7 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
     DevState* st = P.st;
     const unsigned long long sweep = st->sweep;
     const float omc = st->one_minus_cos;
-    const PhiloxKey key = philox_key(P.seed_lo, P.seed_hi);
+    const PhiloxKey& key = P.key;
     const uint32_t c1 = TAG_MOVE | ((uint32_t)colour << 8), c2 = (uint32_t)sweep, c3 = (uint32_t)(sweep >> 32);
     float* Sc = P.S + (long long)colour * 3 * P.plane;
     const Vec3 B = { P.B[0], P.B[1], P.B[2] };
@@ -418,7 +420,7 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
     const double ML = st->ML;
     const float invML = (float)(1.0 / ML);
     const Vec3 eC = { (float)st->eC[0], (float)st->eC[1], (float)st->eC[2] };
-    const PhiloxKey key = philox_key(P.seed_lo, P.seed_hi);
+    const PhiloxKey& key = P.key;
     const uint32_t c2 = (uint32_t)sweep, c3 = (uint32_t)(sweep >> 32);
     uint32_t p0, p1, p2, p3;
     philox4x32_10(key, 0u, TAG_PAIRING | ((uint32_t)colour << 8), c2, c3, p0, p1, p2, p3);

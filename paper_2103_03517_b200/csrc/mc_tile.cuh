@@ -1,0 +1,320 @@
+// mc_tile.cuh -- the sm_100a fast path of the colour pass (Table A1) for uniform, fully periodic lattices.
+//
+// Design:
+//   * One CTA owns a y-slab of Ty rows (all of x) and marches through a z-segment of Lz planes.  The three planes
+//     z-1, z, z+1 of the OTHER colour that a plane of this colour needs live in a 4-slot shared-memory ring; one warp
+//     streams plane z+2 into the free slot with TMA bulk copies (cp.async.bulk, one row per copy, completion on an
+//     mbarrier) while all warps update plane z.  Every other-colour value is therefore read from HBM/L2 once per
+//     (slab, segment) and then served 6 times from shared memory; the y-halo is 2 rows per slab and the z-halo 2
+//     planes per segment.
+//   * One thread owns a PAIR of x-adjacent sites of one colour in RP..RP*NPASS rows of the slab for the whole march:
+//     all its shared-memory and global offsets are loop invariants, the march only adds constants.
+//   * The fp32 arithmetic of the two sites is packed into Blackwell's two-wide FFMA2 / FADD2 / FMUL2 instructions
+//     (one issue slot for two sites); Philox, MUFU and the selects stay scalar.
+//   * Own colour: LDG.64 / STG.64 straight from/to the colour-split planes (read once, written once).
+//   * Fused sums (a-9) are carried per thread in fp32 over its <= 2*NPASS*Lz sites (a bounded, fixed set), converted to
+//     fp64 once, then reduced in a fixed order (deterministic two-pass reduction, pass 1).
+// Arithmetic contract: identical to pass_kernel / DESIGN.md section 3 (same Philox stream, same cone construction).
+#pragma once
+
+#include "mc_kernels.cuh"
+
+namespace mc {
+
+constexpr int TILE_NSLOT = 4;
+#ifndef MC_TILE_MAX_THREADS
+#define MC_TILE_MAX_THREADS 448
+#endif
+#ifndef MC_TILE_MIN_BLOCKS
+#define MC_TILE_MIN_BLOCKS 2
+#endif
+#ifndef MC_TILE_TY_RT
+#define MC_TILE_TY_RT 16
+#endif
+constexpr int TILE_MAX_THREADS = MC_TILE_MAX_THREADS;   // launch bounds of the tiled pass: threads per CTA ...
+constexpr int TILE_MIN_BLOCKS = MC_TILE_MIN_BLOCKS;     // ... and CTAs per SM the register allocation must allow
+constexpr int TILE_TY_RT = MC_TILE_TY_RT;               // slab height of the compile-time-R specialisations
+
+struct TileGeom {
+    int R, PR;                 // colour-sites per row, pairs per row
+    int nx, ny, nz;
+    int Ty, RP, NPASS;         // rows per slab = RP * NPASS, rows per pass
+    int n_slabs, n_segs;       // grid = n_slabs * n_segs
+    int Lz, Lz_rem;            // segment s covers Lz + (s < Lz_rem ? 1 : 0) planes
+    int slot_floats;           // 3 * (Ty + 2) * R
+    int n_active;              // PR * RP working threads (block size is this rounded up to a warp multiple)
+};
+
+// ---- packed two-wide fp32 helpers (FFMA2 / FADD2 / FMUL2 on sm_100a)
+typedef float2 f2;
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ f2 splat(float v) { return make_float2(v, v); }
+
+// ---- mbarrier / TMA bulk-copy primitives (PTX; CTA-local shared addresses)
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "MC_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra MC_DONE;\n"
+        "bra MC_WAIT;\n"
+        "MC_DONE:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+// One plane (Ty + 2 rows x 3 components, periodic wrap in y) of the other colour -> one ring slot, issued by ONE thread.
+// Rows that are consecutive in y are consecutive in HBM and in the slot, so a slab in the interior of the lattice
+// needs one bulk copy per component; a slab touching y = 0 or y = ny-1 needs one more per wrapped row.
+__device__ __forceinline__ void tile_issue_plane(const TileGeom& G, int R, const float* __restrict__ Oth, long long plane, int z, int y0,
+                                                 uint32_t slot_addr, uint32_t bar)
+{
+    const int nrows = G.Ty + 2;
+    const uint32_t row_bytes = (uint32_t)R * 4u;
+    mbar_arrive_expect_tx(bar, 3u * (uint32_t)nrows * row_bytes);
+    const float* zbase = Oth + (long long)z * G.ny * R;
+    int ry = 0;
+    while (ry < nrows) {
+        int y = y0 - 1 + ry;
+        if (y < 0) y += G.ny; else if (y >= G.ny) y -= G.ny;
+        int run = nrows - ry; if (run > G.ny - y) run = G.ny - y;
+#pragma unroll
+        for (int comp = 0; comp < 3; ++comp)
+            bulk_g2s(slot_addr + (uint32_t)(comp * nrows + ry) * row_bytes, zbase + (long long)comp * plane + (long long)y * R,
+                     (uint32_t)run * row_bytes, bar);
+        ry += run;
+    }
+}
+
+// ANISO: bit 0 uniaxial (uniform axis), bit 1 cubic.  FIELD: Zeeman term.  RT: colour-sites per row as a compile-time
+// constant (0 = run-time value; the specialisations turn every shared-memory offset into an immediate).
+// sum S.h is accumulated by the black pass only (every bond joins a red and a black site, so
+// E_exch = -J sum_{i black} S_i.h_i with h already in registers).
+template <int ANISO, bool FIELD, int RT, bool DEBUG>
+__global__ void __launch_bounds__(TILE_MAX_THREADS, TILE_MIN_BLOCKS)
+tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileGeom G, int colour, float invT, int flags,
+                 float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
+{
+    extern __shared__ __align__(128) float smem[];
+    __shared__ __align__(8) unsigned long long bars[TILE_NSLOT];
+
+    DevState* st = P.st;
+    const unsigned long long sweep = st->sweep;
+    const float omc = st->one_minus_cos;
+    const PhiloxKey& key = P.key;
+    const uint32_t c1 = TAG_MOVE | ((uint32_t)colour << 8), c2 = (uint32_t)sweep, c3 = (uint32_t)(sweep >> 32);
+
+    const int R = RT ? RT : G.R;
+    const int PR = R / 2;
+    const int tid = threadIdx.x;
+    const int slab = blockIdx.x % G.n_slabs, seg = blockIdx.x / G.n_slabs;
+    const int y0 = slab * G.Ty;
+    const int Lz = G.Lz + (seg < G.Lz_rem ? 1 : 0);
+    const int z0 = seg * G.Lz + (seg < G.Lz_rem ? seg : G.Lz_rem);
+    const int nrows = (RT ? TILE_TY_RT : G.Ty) + 2;          // the specialisations fix the slab height too
+    const int CS = nrows * R;                                // floats between components inside a slot
+    const int slot_floats = 3 * CS;
+
+    const float* Oth = P.S + (long long)(1 - colour) * 3 * P.plane;
+    float* Sc = P.S + (long long)colour * 3 * P.plane;
+    const uint32_t smem_base = smem_u32(smem), bar_base = smem_u32(bars);
+    const uint32_t slot_bytes = (uint32_t)slot_floats * 4u;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < TILE_NSLOT; ++s) mbar_init(bar_base + 8u * s, 1u);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        // prologue: planes z0-1 .. z0+2 (sequence index 0..3)
+        const int nseq = Lz + 2 < TILE_NSLOT ? Lz + 2 : TILE_NSLOT;
+        for (int k = 0; k < nseq; ++k) {
+            int z = z0 - 1 + k; if (z < 0) z += G.nz; else if (z >= G.nz) z -= G.nz;
+            tile_issue_plane(G, R, Oth, P.plane, z, y0, smem_base + (uint32_t)k * slot_bytes, bar_base + 8u * k);
+        }
+    }
+    __syncthreads();                                         // barriers initialised before anyone waits on them
+
+    // ---- per-thread invariants: a thread owns pair cp of rows r0, r0+RP, .. of the slab for the whole march
+    const bool active = tid < G.n_active;
+    const int r0 = tid / PR, cp = tid - r0 * PR;
+    const int exL = (cp == 0) ? R - 1 : 2 * cp - 1;          // x-neighbour outside the pair: left (row parity 0) ...
+    const int exR = (cp == PR - 1) ? 0 : 2 * cp + 2;         // ... or right (row parity 1), periodic in x
+    const int pbase = (y0 + r0 + z0 + colour) & 1;
+    const int soff0 = (r0 + 1) * R + 2 * cp;                 // centre element inside a component block of a slot
+    const int exo0 = (r0 + 1) * R;
+    const int pstride = G.RP * R;                            // floats between the rows of consecutive passes
+    const long long zstride = (long long)G.ny * R;
+    float* gS0 = Sc + ((long long)z0 * G.ny + y0 + r0) * R + 2 * cp;
+    const uint32_t site00 = (uint32_t)(((long long)z0 * G.ny + y0 + r0) * G.nx) + 4u * (uint32_t)cp;
+    const uint32_t zsite = (uint32_t)(G.ny * G.nx), psite = (uint32_t)(G.RP * G.nx);
+
+    f2 aMx = splat(0.f), aMy = splat(0.f), aMz = splat(0.f), aEx = splat(0.f), aAn = splat(0.f);
+    int cnt = 0;
+
+    const f2 two = splat(2.0f);
+    const float CU = 0.99999994f;                            // 1 - 2^-24: u = f - CU with f in [1,2) (C-8)
+    const f2 nomc2 = splat(-omc);
+    const f2 twopi2 = splat(6.2831853071795865f), angc2 = splat(-(CU * 6.2831853071795865f) - 3.1415926535897932f);
+    const f2 nCU2 = splat(-CU);
+    const f2 xscale2 = splat(invT * 1.4426950408889634f);    // decision in base 2: dE/T * log2(e) + log2(u2) < 0
+    const f2 nJ2 = splat(-P.J);
+    const f2 e2x = splat(P.eu[0]), e2y = splat(P.eu[1]), e2z = splat(P.eu[2]);
+    const f2 B2x = splat(P.B[0]), B2y = splat(P.B[1]), B2z = splat(P.B[2]);
+    const f2 nKu2 = splat(-P.Ku), nhKc2 = splat(-0.5f * P.Kc);
+
+    for (int j = 0; j < Lz; ++j) {
+        if (j == 0) { mbar_wait(bar_base, 0u); mbar_wait(bar_base + 8u, 0u); }
+        { const int k = j + 2; mbar_wait(bar_base + 8u * (k & 3), (uint32_t)(k >> 2) & 1u); }
+        const float* sM = smem + ((j) & 3) * slot_floats;          // plane z-1
+        const float* sC = smem + ((j + 1) & 3) * slot_floats;      // plane z
+        const float* sP = smem + ((j + 2) & 3) * slot_floats;      // plane z+1
+
+        if (active) {
+            float* gS = gS0 + (long long)j * zstride;
+            uint32_t siteb = site00 + (uint32_t)j * zsite;
+            int soff = soff0, exo = exo0, parj = pbase + j;
+            for (int pass = 0; pass < G.NPASS; ++pass, gS += pstride, siteb += psite, soff += pstride, exo += pstride, parj += G.RP) {
+                const int par = parj & 1;                             // (y + z + colour) & 1
+                const uint32_t site0 = siteb + (uint32_t)par;
+                const float* pC = sC + soff;
+                const float* pP = sP + soff;
+                const float* pM = sM + soff;
+                const float* pE = sC + exo + (par ? exR : exL);
+
+                // own colour: one LDG.64 per component
+                const f2 Sx = *reinterpret_cast<const f2*>(gS);
+                const f2 Sy = *reinterpret_cast<const f2*>(gS + P.plane);
+                const f2 Sz = *reinterpret_cast<const f2*>(gS + 2 * P.plane);
+
+                // exchange field h = sum of the 6 neighbours (first term of Eq. 2), J applied in dE
+                f2 h[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const f2 o  = *reinterpret_cast<const f2*>(pC + c * CS);
+                    const float ex = pE[c * CS];
+                    const f2 yp = *reinterpret_cast<const f2*>(pC + c * CS + R);
+                    const f2 ym = *reinterpret_cast<const f2*>(pC + c * CS - R);
+                    const f2 zp = *reinterpret_cast<const f2*>(pP + c * CS);
+                    const f2 zm = *reinterpret_cast<const f2*>(pM + c * CS);
+                    // par = 0: x-neighbours of the two sites are (ex, o.x) and (o.x, o.y);  par = 1: (o.x, o.y) and (o.y, ex)
+                    const f2 sh = par ? make_float2(o.y, ex) : make_float2(ex, o.x);
+                    h[c] = add2(add2(add2(o, sh), add2(yp, ym)), add2(zp, zm));
+                }
+
+                // random numbers: one Philox4x32-10 call per site (a-2)
+                uint32_t ra0, ra1, ra2, ra3, rb0, rb1, rb2, rb3;
+                philox4x32_10(key, site0, c1, c2, c3, ra0, ra1, ra2, ra3);
+                philox4x32_10(key, site0 + 2u, c1, c2, c3, rb0, rb1, rb2, rb3);
+                const f2 f0 = make_float2(__uint_as_float(__funnelshift_r(ra0, 0x7Fu, 9)), __uint_as_float(__funnelshift_r(rb0, 0x7Fu, 9)));
+                const f2 f1 = make_float2(__uint_as_float(__funnelshift_r(ra1, 0x7Fu, 9)), __uint_as_float(__funnelshift_r(rb1, 0x7Fu, 9)));
+                const f2 f2u = make_float2(__uint_as_float(__funnelshift_r(ra2, 0x7Fu, 9)), __uint_as_float(__funnelshift_r(rb2, 0x7Fu, 9)));
+
+                // cone move (a-4; C-6, C-7): d = sa (cos(phi) t1 + sin(phi) t2) - w S
+                const f2 nw = mul2(add2(f0, nCU2), nomc2);                           // -w,  w = u0 (1 - cos theta); u0 = f0 - CU exactly
+                const f2 t  = mul2(nw, fma2(nw, splat(-1.0f), splat(-2.0f)));        // w (2 - w) = sin^2(alpha)
+                const f2 sa = mul2(t, make_float2(rsqrtf(t.x), rsqrtf(t.y)));
+                const f2 ang = fma2(f1, twopi2, angc2);                              // phi - pi in (-pi, pi)
+                // cos(phi) = -cos(ang), sin(phi) = -sin(ang): the minus signs are folded into the frame (nt1 = -t1, nt2 = -t2)
+                const f2 Cc = mul2(sa, make_float2(__cosf(ang.x), __cosf(ang.y)));
+                const f2 Ss = mul2(sa, make_float2(__sinf(ang.x), __sinf(ang.y)));
+                const f2 sg = make_float2(copysignf(1.0f, Sz.x), copysignf(1.0f, Sz.y));
+                const f2 den = add2(sg, Sz);
+                const f2 ia = make_float2(__fdividef(1.0f, den.x), __fdividef(1.0f, den.y));   // -a of the frame construction
+                const f2 uu = mul2(Sx, ia), vv = mul2(Sy, ia);
+                const f2 q  = mul2(sg, Sx);
+                const f2 nt1x = fma2(q, uu, splat(-1.0f));      // -(1 + sg Sx^2 a)
+                const f2 nt1y = mul2(q, vv);                    // -(sg b),  b = Sx Sy a
+                const f2 nt2x = mul2(Sy, uu);                   // -b
+                const f2 nt2y = fma2(Sy, vv, make_float2(-sg.x, -sg.y));   // -(sg + Sy^2 a)
+                // nt1z = q = sg Sx,  nt2z = Sy
+                const f2 dx = fma2(Cc, nt1x, fma2(Ss, nt2x, mul2(nw, Sx)));
+                const f2 dy = fma2(Cc, nt1y, fma2(Ss, nt2y, mul2(nw, Sy)));
+                const f2 dz = fma2(Cc, q,    fma2(Ss, Sy,   mul2(nw, Sz)));
+                const f2 vx = add2(Sx, dx), vy = add2(Sy, dy), vz = add2(Sz, dz);
+                const f2 n2 = fma2(vx, vx, fma2(vy, vy, mul2(vz, vz)));
+                const f2 inv = fma2(n2, splat(-0.5f), splat(1.5f));                  // 1/|v| to O(eps^2), |v|^2 = 1 + O(1e-7)
+                const f2 Nx = mul2(vx, inv), Ny = mul2(vy, inv), Nz = mul2(vz, inv);
+
+                // energy difference (a-5), difference form: -J d.h - d.B - Ku (d.e)((2S+d).e) - Kc/2 sum_a (n_a^2 - S_a^2)(n_a^2 + S_a^2)
+                const f2 dh = fma2(dx, h[0], fma2(dy, h[1], mul2(dz, h[2])));
+                f2 dE = mul2(nJ2, dh);
+                if (FIELD) dE = fma2(splat(-1.0f), fma2(dx, B2x, fma2(dy, B2y, mul2(dz, B2z))), dE);
+                if (ANISO & 1) {
+                    const f2 de = fma2(dx, e2x, fma2(dy, e2y, mul2(dz, e2z)));
+                    const f2 se = fma2(Sx, e2x, fma2(Sy, e2y, mul2(Sz, e2z)));
+                    dE = fma2(nKu2, mul2(de, fma2(two, se, de)), dE);
+                }
+                if (ANISO & 2) {
+                    const f2 gx = mul2(dx, add2(Sx, vx)), gy = mul2(dy, add2(Sy, vy)), gz = mul2(dz, add2(Sz, vz));   // n_a^2 - S_a^2
+                    const f2 tx = fma2(vx, vx, mul2(Sx, Sx)), ty = fma2(vy, vy, mul2(Sy, Sy)), tz = fma2(vz, vz, mul2(Sz, Sz));
+                    const f2 qs = fma2(gx, tx, fma2(gy, ty, mul2(gz, tz)));
+                    dE = fma2(nhKc2, qs, dE);
+                }
+
+                // accept / reject (a-6; P:157-159 in log form, C-8)
+                const f2 u2 = add2(f2u, nCU2);
+                const f2 xd = fma2(dE, xscale2, make_float2(__log2f(u2.x), __log2f(u2.y)));
+                const bool ok0 = xd.x < 0.0f, ok1 = xd.y < 0.0f;
+                f2 Ox, Oy, Oz;
+                Ox.x = ok0 ? Nx.x : Sx.x; Oy.x = ok0 ? Ny.x : Sy.x; Oz.x = ok0 ? Nz.x : Sz.x;
+                Ox.y = ok1 ? Nx.y : Sx.y; Oy.y = ok1 ? Ny.y : Sy.y; Oz.y = ok1 ? Nz.y : Sz.y;
+                cnt += (int)ok0 + (int)ok1;
+                *reinterpret_cast<f2*>(gS) = Ox;
+                *reinterpret_cast<f2*>(gS + P.plane) = Oy;
+                *reinterpret_cast<f2*>(gS + 2 * P.plane) = Oz;
+                if (DEBUG) {
+                    if (dbg_x)   { dbg_x[site0] = xd.x * 0.69314718055994531f; dbg_x[site0 + 2u] = xd.y * 0.69314718055994531f; }
+                    if (dbg_acc) { dbg_acc[site0] = (uint8_t)ok0; dbg_acc[site0 + 2u] = (uint8_t)ok1; }
+                }
+
+                // fused sums of the final spins (a-9)
+                aMx = add2(aMx, Ox); aMy = add2(aMy, Oy); aMz = add2(aMz, Oz);
+                if (colour) aEx = fma2(Ox, h[0], fma2(Oy, h[1], fma2(Oz, h[2], aEx)));
+                if (ANISO & 1) { const f2 se = fma2(Ox, e2x, fma2(Oy, e2y, mul2(Oz, e2z))); aAn = fma2(mul2(nKu2, se), se, aAn); }
+                if (ANISO & 2) {
+                    const f2 x2 = mul2(Ox, Ox), y2 = mul2(Oy, Oy), z2 = mul2(Oz, Oz);
+                    const f2 cub = fma2(x2, y2, fma2(x2, z2, mul2(y2, z2)));
+                    aAn = fma2(splat(P.Kc), cub, aAn);
+                }
+            }
+        }
+        __syncthreads();                                     // every warp is done with plane z-1's slot
+        if (tid == 0 && j + TILE_NSLOT < Lz + 2) {
+            const int k = j + TILE_NSLOT;
+            int zn = z0 - 1 + k; if (zn >= G.nz) zn -= G.nz;
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            tile_issue_plane(G, R, Oth, P.plane, zn, y0, smem_base + (uint32_t)(k & 3) * slot_bytes, bar_base + 8u * (k & 3));
+        }
+    }
+
+    // ---- deterministic block reduction (pass 1) + election of the finalising block
+    double acc[NQ];
+    acc[0] = (double)aMx.x + (double)aMx.y; acc[1] = (double)aMy.x + (double)aMy.y; acc[2] = (double)aMz.x + (double)aMz.y;
+    acc[3] = colour ? -(double)P.J * ((double)aEx.x + (double)aEx.y) : 0.0;
+    acc[4] = (double)aAn.x + (double)aAn.y;
+    acc[5] = FIELD ? -(acc[0] * (double)P.B[0] + acc[1] * (double)P.B[1] + acc[2] * (double)P.B[2]) : 0.0;
+    acc[6] = acc[7] = acc[8] = 0.0;
+    block_partials(acc, cnt, P, colour);
+    if (threadIdx.x == 0) st->nblocks[colour] = gridDim.x;
+    if (flags & F_FINALIZE) {
+        if (last_block_done(st)) final_reduce(P, 0, flags);
+    }
+}
+
+}  // namespace mc
