@@ -141,7 +141,7 @@ def test_c2_temperature_sweep_tc_from_susceptibility_peak(mods):
     for T, v in zip(Ts[:12], m[:12]):
         assert abs(v - (1 - T / 1.4451) ** 0.340) < 0.03, (T, v)
     ipk = int(np.argmax(chi))
-    assert Ts[ipk] in (1.4, 1.5)                                    # chi_l peaks at T_c = 1.443 on a 0.1 grid (P-14, C-19)
+    assert ipk in (13, 14)                                          # chi_l peaks at T = 1.4 or 1.5: T_c = 1.443 on a 0.1 grid (P-14, C-19)
     a, b, c = np.polyfit(Ts[ipk - 1: ipk + 2], chi[ipk - 1: ipk + 2], 2)
     assert abs(-b / (2 * a) - 1.443) < 0.06
     assert chi[0] < 0.05 * chi[ipk]                                 # chi_l -> 0 as T -> 0
