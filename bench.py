@@ -52,12 +52,16 @@ def measured_peaks():
 
 
 def recorded_traffic():
-    """dram bytes per colour-pass launch from the committed ncu --set full capture, if any (profiles/traffic.json)."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
+    """dram bytes per colour-pass launch from the committed ncu --set full capture, if any (profiles/traffic.txt)."""
+    path = os.path.join(ROOT, "profiles", "traffic.txt")
     try:
-        return float(json.load(open(path))["pass_kernel_dram_bytes_per_launch"])
+        for line in open(path):
+            t = line.split()
+            if t and t[0] == "pass_kernel_dram_bytes_per_launch":
+                return float(t[1])
     except Exception:
-        return None
+        pass
+    return None
 
 
 class ClockSampler:
