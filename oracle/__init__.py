@@ -53,6 +53,8 @@ def lib():
     vp, i32, i64, u64, dbl = C.c_void_p, C.c_int, C.c_int64, C.c_uint64, C.c_double
     L.orc_philox4x32_10.argtypes = [vp, vp, vp]; L.orc_philox4x32_10.restype = None
     L.orc_uniform.argtypes = [C.c_uint32]; L.orc_uniform.restype = dbl
+    L.orc_uniform_azimuth.argtypes = [C.c_uint32, C.c_uint32]; L.orc_uniform_azimuth.restype = dbl
+    L.orc_site_uniforms.argtypes = [vp, i32, i32, i32, i32, u64, vp, vp, vp]; L.orc_site_uniforms.restype = None
     L.orc_cone_move.argtypes = [vp, dbl, dbl, dbl, vp]; L.orc_cone_move.restype = None
     L.orc_create.argtypes = [i32, i32, i32, vp, dbl, dbl, vp, dbl, vp, vp, vp, vp, i32, dbl, i32, u64]
     L.orc_create.restype = vp
@@ -96,6 +98,10 @@ def uniform(r: int) -> float:
     return lib().orc_uniform(int(r) & 0xFFFFFFFF)
 
 
+def uniform_azimuth(w0: int, w1: int) -> float:
+    return lib().orc_uniform_azimuth(int(w0) & 0xFFFFFFFF, int(w1) & 0xFFFFFFFF)
+
+
 def cone_move(S, theta, u0, u1):
     s = np.ascontiguousarray(S, dtype=np.float64); o = np.zeros(3)
     lib().orc_cone_move(_p(s), float(theta), float(u0), float(u1), _p(o))
@@ -125,6 +131,12 @@ class Oracle:
     def __del__(self):
         if getattr(self, "h", None):
             self.L.orc_destroy(self.h); self.h = None
+
+    def site_uniforms(self, x, y, z, colour, sweep):
+        """(u0, u1, u2) of the unconstrained update of site (x,y,z) in the given sweep (reading C-26)."""
+        u = [C.c_double(), C.c_double(), C.c_double()]
+        self.L.orc_site_uniforms(self.h, int(x), int(y), int(z), int(colour), int(sweep), C.byref(u[0]), C.byref(u[1]), C.byref(u[2]))
+        return tuple(v.value for v in u)
 
     # ---- state
     def set_spins(self, xyz):

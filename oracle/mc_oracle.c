@@ -63,6 +63,14 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
 /* u = ((r>>9) + 0.5) * 2^-23: 24 significant bits, so identical in fp32 and fp64 (pin P-2, reading C-8). */
 double orc_uniform(uint32_t r) { return ((double)(r >> 9) + 0.5) * (1.0 / 8388608.0); }
 
+/* Azimuth uniform of the unconstrained move (reading C-26): the 9 low bits of the two words whose 23 high bits
+ * make u0 and u2, 18 bits in all, u1 = k 2^-18 in [0,1) (an angle needs no open interval). */
+double orc_uniform_azimuth(uint32_t w0, uint32_t w1)
+{
+    uint32_t k = ((w0 & 0x1FFu) << 9) | (w1 & 0x1FFu);
+    return (double)k * (1.0 / 262144.0);
+}
+
 static void draw(const orc_ctx* c, uint32_t site, uint32_t tag, int colour, uint64_t sweep, uint32_t r[4])
 {
     uint32_t ctr[4] = { site, tag | ((uint32_t)colour << 8), (uint32_t)sweep, (uint32_t)(sweep >> 32) };
@@ -224,13 +232,31 @@ void orc_set_sweep(orc_ctx* c, uint64_t s) { c->sweep = s; }
 void orc_set_adaptive(orc_ctx* c, int a) { c->adaptive = a; }
 void orc_set_sampling(orc_ctx* c, int on) { c->sampling = on; }
 
+/* ------------------------------------------------------------------ the three uniforms of one unconstrained update
+ * Reading C-26: two same-colour sites that are neighbours along x in their colour's row,
+ * x and x ^ 2, share ONE Philox4x32-10 block, counter word 0 = lexicographic index of the one with bit 1 of x clear;
+ * that site takes words (0,1), the other takes words (2,3).  From its words (w0,w1) a site forms
+ *   u0 = ((w0 >> 9) + 0.5) 2^-23   (cone polar draw),     u2 = ((w1 >> 9) + 0.5) 2^-23   (acceptance draw),
+ *   u1 = (((w0 & 511) << 9) | (w1 & 511)) 2^-18            (cone azimuth).
+ * 64 random bits per update, every bit used once. */
+void orc_site_uniforms(const orc_ctx* c, int x, int y, int z, int colour, uint64_t sweep, double* u0, double* u1, double* u2)
+{
+    int64_t first = site_index(c, x & ~2, y, z);
+    int half = (x >> 1) & 1;
+    uint32_t r[4];
+    draw(c, (uint32_t)first, TAG_MOVE, colour, sweep, r);
+    uint32_t w0 = r[2 * half], w1 = r[2 * half + 1];
+    *u0 = orc_uniform(w0);
+    *u1 = orc_uniform_azimuth(w0, w1);
+    *u2 = orc_uniform(w1);
+}
+
 /* ------------------------------------------------------------------ Table A1: one colour pass */
 static int metropolis_update(orc_ctx* c, int x, int y, int z, int colour, double T, double* xdec)
 {
     int64_t i = site_index(c, x, y, z);                       /* P:155  i = Get_Red(Black)SpinIndex(index) */
-    uint32_t r[4];
-    draw(c, (uint32_t)i, TAG_MOVE, colour, c->sweep, r);
-    double u0 = orc_uniform(r[0]), u1 = orc_uniform(r[1]), u2 = orc_uniform(r[2]);
+    double u0, u1, u2;
+    orc_site_uniforms(c, x, y, z, colour, c->sweep, &u0, &u1, &u2);   /* P:156-157 UniformRandom() x 3 (C-8, C-26) */
     double* S = &c->S[3 * i], Sn[3], h[3];
     orc_cone_move(S, c->cone, u0, u1, Sn);                    /* P:156  S_new = UniformRandom_RotateSpin(S_i, theta) */
     exchange_field(c, x, y, z, h);

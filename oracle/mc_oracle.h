@@ -41,6 +41,10 @@ typedef struct {
 void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
 /* Uniform in (0,1): ((r >> 9) + 0.5) * 2^-23. */
 double orc_uniform(uint32_t r);
+double orc_uniform_azimuth(uint32_t w0, uint32_t w1);
+/* The three uniforms of the unconstrained update of site (x,y,z): one Philox block per pair of x-neighbours of one
+ * colour (x, x^2), 64 bits per site (reading C-26 in DESIGN.md section 4). */
+void orc_site_uniforms(const orc_ctx* c, int x, int y, int z, int colour, uint64_t sweep, double* u0, double* u1, double* u2);
 /* Cone trial move: S unit, theta = cone half-angle, u0,u1 in (0,1). */
 void orc_cone_move(const double S[3], double theta, double u0, double u1, double Snew[3]);
 

@@ -329,7 +329,7 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     const uint32_t N = (uint32_t)nx * ny * nz, R = nx / 2, Nc = N / 2;
     char* ws = (char*)dev_workspace;
     Params& P = ctx->P;
-    P.nx = nx; P.ny = ny; P.nz = nz; P.R = (int)R; P.Nc = Nc; P.N = N;
+    P.nx = nx; P.ny = ny; P.nz = nz; P.R = (int)R; P.Nc = Nc; P.N = N; P.invN = 1.0 / (double)N;
     P.plane = L.plane; P.S = (float*)(ws + L.spins);
     P.mask = nullptr; P.mask_plane = L.mask_plane; P.region = nullptr; P.region_plane = L.region_plane; P.axis = nullptr;
     P.J = (float)ham->J; P.Ku = (float)ham->Ku; P.Kc = (float)ham->Kc;

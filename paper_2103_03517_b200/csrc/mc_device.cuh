@@ -53,6 +53,21 @@ __device__ __forceinline__ float uniform01(uint32_t r)
     return __uint_as_float((r >> 9) | 0x3f800000u) - 0.99999994f;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// The uniforms of one unconstrained update (C-26).  Two same-colour x-neighbours of a row (x and x ^ 2) share one
+// Philox block whose counter word 0 is the lexicographic index of the one with bit 1 of x clear; that site takes
+// words (0,1), the other words (2,3).  From its words (w0,w1):
+//   u0 = ((w0 >> 9) + 0.5) 2^-23,  u2 = ((w1 >> 9) + 0.5) 2^-23,  u1 = (((w0 & 511) << 9) | (w1 & 511)) 2^-18.
+// Why: IMAD.WIDE.U32 issues once per ~6 cycles per SM sub-partition on sm_100a (measured), so the 20 wide multiplies
+// of a Philox call cost as much as all the fp32 arithmetic of an update; 64 bits per update halve that.
+// ---------------------------------------------------------------------------------------------------------------
+// 1 + u1 as a float in [1,2): exponent | 9 low bits of w0 | 9 low bits of w1 | 00000   (one LOP3, one SHF.L, one SHF.R.W)
+__device__ __forceinline__ float azimuth_1p(uint32_t w0, uint32_t w1)
+{
+    return __uint_as_float(__funnelshift_r(w1 << 23, (w0 & 0x1FFu) | 0xFE00u, 18));
+}
+__device__ __forceinline__ float uniform_azimuth(uint32_t w0, uint32_t w1) { return azimuth_1p(w0, w1) - 1.0f; }
+
 struct Vec3 { float x, y, z; };
 
 __device__ __forceinline__ float dot3(const Vec3& a, const Vec3& b) { return fmaf(a.x, b.x, fmaf(a.y, b.y, a.z * b.z)); }

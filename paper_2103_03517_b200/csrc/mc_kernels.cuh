@@ -15,7 +15,7 @@ namespace mc {
 
 constexpr int NQ = 9;          // fused sums: Mx My Mz E_exch E_aniso E_zeeman tq_x tq_y tq_z (extensive, fp64)
 constexpr int BLOCK = 256;     // threads per CTA of the generic pass kernels
-constexpr int MAX_WARPS = 16;  // largest CTA any kernel that reduces uses (512 threads); block sizes are warp multiples
+constexpr int MAX_WARPS = 32;  // largest CTA any kernel that reduces uses (1024 threads); block sizes are warp multiples
 constexpr int TRACE_CAP = 16384;
 
 // Controller / reduction state, resident in the workspace (no host round trip per sweep: P:165-171 runs on the device)
@@ -42,6 +42,7 @@ struct Params {
     int nx, ny, nz, R;               // R = nx/2 sites of one colour per row
     uint32_t Nc;                     // sites per colour
     uint32_t N;
+    double invN;                     // 1 / N (host-computed: keeps an fp64 division off the finalising thread)
     long long plane;                 // floats between component planes
     float* S;                        // 6 planes: colour-major, then component
     const uint8_t* mask;   long long mask_plane;     // [2][mask_plane] colour-split bond masks (or null)
@@ -96,6 +97,7 @@ struct ItemPos {
     uint32_t par;       // (y + z + colour) & 1
     uint32_t o_yp, o_ym, o_zp, o_zm;   // colour-linear index of the same column in the 4 neighbouring rows
     uint32_t o_x;       // colour-linear index of the one extra x-neighbour outside the item's own column range
+    uint32_t xh0;       // in-row colour index of the first site (x = 2 xh0 + par)
 };
 
 template <int VEC>
@@ -108,6 +110,7 @@ __device__ __forceinline__ ItemPos locate(const Params& P, const Geom& G, uint32
     const uint32_t R = (uint32_t)P.R, ny = (uint32_t)P.ny, nz = (uint32_t)P.nz;
     const uint32_t xh0 = xq * VEC;
     q.par = (y + z + (uint32_t)colour) & 1u;
+    q.xh0 = xh0;
     q.a0 = row * R + xh0;
     q.site0 = row * (uint32_t)P.nx + 2u * xh0 + q.par;
     const uint32_t yp = (y + 1 == ny) ? 0u : y + 1, ym = (y == 0) ? ny - 1 : y - 1;
@@ -217,11 +220,22 @@ __device__ __forceinline__ void block_partials(const double (&acc)[NQ], int cnt,
 
 // Pass 2 of the reduction (one block, fixed order) + what follows a sweep: cone controller (P:168-171 read with
 // P:205-209; C-2, C-3, C-9), sweep counter, Eq. (6) accumulators, trace row.  mode 0: end of a sweep; 1: measurement.
+// This block runs alone at the tail of the black pass, so its latency is exposed: the controller state is staged
+// through shared memory with one coalesced read and one coalesced write (two L2 round trips instead of a chain of
+// dependent ones), and thread 0 does the scalar work on the shared copy.
+static_assert(sizeof(DevState) % 4 == 0, "DevState is staged as 32-bit words");
 __device__ void final_reduce(const Params& P, int mode, int flags)
 {
     __shared__ double red[MAX_WARPS][NQ];
+    __shared__ double tot[NQ];
+    __shared__ double cone_next[2];
+    __shared__ float omc_next[2];
+    __shared__ DevState sst;
     DevState* st = P.st;
+    constexpr int NWORDS = (int)(sizeof(DevState) / 4);
     const int nwarps = (int)(blockDim.x >> 5);
+    for (int i = threadIdx.x; i < NWORDS; i += blockDim.x)
+        reinterpret_cast<uint32_t*>(&sst)[i] = __ldcg(reinterpret_cast<const uint32_t*>(st) + i);
     double acc[NQ];
 #pragma unroll
     for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
@@ -237,42 +251,57 @@ __device__ void final_reduce(const Params& P, int mode, int flags)
 #pragma unroll
     for (int q = 0; q < NQ; ++q) { const double v = warp_sum(acc[q]); if (lane == 0) red[warp][q] = v; }
     __syncthreads();
+    // warps in a fixed order, one thread per quantity; another thread meanwhile evaluates both possible next cone angles
+    const int cone_thread = blockDim.x > 32 ? 32 : NQ;
+    if (threadIdx.x < NQ) {
+        double v = 0.0;
+        for (int w = 0; w < nwarps; ++w) v += red[w][threadIdx.x];
+        tot[threadIdx.x] = v;
+    } else if ((int)threadIdx.x == cone_thread && mode == 0) {
+        const double deg = 3.14159265358979323846 / 180.0, pi = 3.14159265358979323846;
+        double up = sst.cone + deg; if (up > pi) up = pi;
+        double dn = sst.cone - deg; if (dn < deg) dn = deg;
+        cone_next[0] = up; cone_next[1] = dn;
+        omc_next[0] = (float)(1.0 - cos(up)); omc_next[1] = (float)(1.0 - cos(dn));
+    }
+    __syncthreads();
     if (threadIdx.x == 0) {
+        DevState& S = sst;
         double s[NQ];
-        for (int q = 0; q < NQ; ++q) { double v = 0.0; for (int w = 0; w < nwarps; ++w) v += red[w][q]; s[q] = v; }
-        st->ML = s[0] * st->eC[0] + s[1] * st->eC[1] + s[2] * st->eC[2];
+        for (int q = 0; q < NQ; ++q) s[q] = tot[q];
+        S.ML = s[0] * S.eC[0] + s[1] * S.eC[1] + s[2] * S.eC[2];
         if (mode == 1) {
-            for (int q = 0; q < NQ; ++q) st->meas[q] = s[q];
+            for (int q = 0; q < NQ; ++q) S.meas[q] = s[q];
         } else {
-            const double N = (double)P.N, invN = 1.0 / N;
-            const unsigned long long cnt = __ldcg(&st->count);
-            const double cone_used = st->cone;
-            st->last_acceptance = (double)cnt * invN;
-            if (st->adaptive) {
-                const double deg = 3.14159265358979323846 / 180.0, pi = 3.14159265358979323846;
-                double c = st->cone;
-                if (2ull * cnt > (unsigned long long)P.N) { c += deg; if (c > pi) c = pi; }
-                else                                      { c -= deg; if (c < deg) c = deg; }
-                st->cone = c;
-                st->one_minus_cos = (float)(1.0 - cos(c));
+            const double invN = P.invN;
+            const unsigned long long cnt = S.count;
+            const double cone_used = S.cone;
+            S.last_acceptance = (double)cnt * invN;
+            if (S.adaptive) {
+                const int k = (2ull * cnt > (unsigned long long)P.N) ? 0 : 1;     // C-9: equality decreases
+                S.cone = cone_next[k];
+                S.one_minus_cos = omc_next[k];
             }
-            st->count = 0ull;
-            st->sweep += 1ull;
-            for (int q = 0; q < NQ; ++q) st->sums[q] = s[q];
+            S.count = 0ull;
+            S.sweep += 1ull;
+            for (int q = 0; q < NQ; ++q) S.sums[q] = s[q];
             const double mx = s[0] * invN, my = s[1] * invN, mz = s[2] * invN;
             const double ml = sqrt(mx * mx + my * my + mz * mz);
             const double E = (s[3] + s[4] + s[5]) * invN;
             const double mv[4] = { ml, mx, my, mz };
-            for (int a = 0; a < 4; ++a) { st->sum_m[a] += mv[a]; st->sum_m2[a] += mv[a] * mv[a]; }
-            st->sum_E += E; st->sum_E2 += E * E;
-            if (flags & F_SAMPLE_TORQUE) for (int a = 0; a < 3; ++a) st->sum_torque[a] += s[6 + a] * invN;
-            st->n_samples += 1ull;
-            double* row = P.trace + (st->trace_rows % (unsigned long long)TRACE_CAP) * 6;
-            row[0] = st->last_acceptance; row[1] = cone_used; row[2] = mx; row[3] = my; row[4] = mz; row[5] = E;
-            st->trace_rows += 1ull;
+            for (int a = 0; a < 4; ++a) { S.sum_m[a] += mv[a]; S.sum_m2[a] += mv[a] * mv[a]; }
+            S.sum_E += E; S.sum_E2 += E * E;
+            if (flags & F_SAMPLE_TORQUE) for (int a = 0; a < 3; ++a) S.sum_torque[a] += s[6 + a] * invN;
+            S.n_samples += 1ull;
+            double* row = P.trace + (S.trace_rows % (unsigned long long)TRACE_CAP) * 6;
+            row[0] = S.last_acceptance; row[1] = cone_used; row[2] = mx; row[3] = my; row[4] = mz; row[5] = E;
+            S.trace_rows += 1ull;
         }
-        st->ticket = 0u;
+        S.ticket = 0u;
     }
+    __syncthreads();
+    for (int i = threadIdx.x; i < NWORDS; i += blockDim.x)
+        reinterpret_cast<uint32_t*>(st)[i] = reinterpret_cast<const uint32_t*>(&sst)[i];
 }
 
 // Last-block election: returns true in every thread of the block that arrives last.
@@ -324,17 +353,29 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
 #pragma unroll
         for (int k = 0; k < NQ; ++k) f[k] = 0.0f;
 #pragma unroll
+        // random words: one Philox4x32-10 block per pair of x-neighbours (x, x ^ 2) of this colour, two words per site (C-26)
+        uint32_t w0[VEC], w1[VEC];
+        if (MODE == MODE_SWEEP) {
+            if (VEC == 1) {
+                const uint32_t half = q.xh0 & 1u;
+                uint32_t r0, r1, r2, r3;
+                philox4x32_10(key, q.site0 - 2u * half, c1, c2, c3, r0, r1, r2, r3);
+                w0[0] = half ? r2 : r0; w1[0] = half ? r3 : r1;
+            } else {
+#pragma unroll
+                for (int k = 0; k + 1 < VEC; k += 2) philox4x32_10(key, q.site0 + 2u * k, c1, c2, c3, w0[k], w1[k], w0[k + 1], w1[k + 1]);
+            }
+        }
+#pragma unroll
         for (int k = 0; k < VEC; ++k) {
             Vec3 S = { sx.v[k], sy.v[k], sz.v[k] };
             const Vec3 hJ = { P.J * h[k].x, P.J * h[k].y, P.J * h[k].z };
             if (MODE == MODE_SWEEP) {
-                uint32_t r0, r1, r2, r3;
-                philox4x32_10(key, q.site0 + 2u * k, c1, c2, c3, r0, r1, r2, r3);
                 Vec3 d, Sn;
-                cone_move(S, omc, uniform01(r0), uniform01(r1), d, Sn);
+                cone_move(S, omc, uniform01(w0[k]), uniform_azimuth(w0[k], w1[k]), d, Sn);
                 const Vec3 hB = { hJ.x + B.x, hJ.y + B.y, hJ.z + B.z };
                 const float dE = delta_energy<ANISO>(S, d, hB, P.Ku, e[(ANISO & 1) ? k : 0], P.Kc);
-                const float x = fmaf(dE, invT, __logf(uniform01(r2)));       // P:157-158 in log form (C-8)
+                const float x = fmaf(dE, invT, __logf(uniform01(w1[k])));    // P:157-158 in log form (C-8)
                 const bool ok = x < 0.0f;
                 if (ok) { S = Sn; nxv.v[k] = Sn.x; nyv.v[k] = Sn.y; nzv.v[k] = Sn.z; }
                 cnt += ok;

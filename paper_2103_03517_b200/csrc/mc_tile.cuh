@@ -103,14 +103,22 @@ __device__ __forceinline__ void tile_issue_plane(const TileGeom& G, int R, const
     }
 }
 
+// u = f - (1 - 2^-24) with f = 1 + (w >> 9) 2^-23 in [1,2): one funnel shift builds f (C-8)
+__device__ __forceinline__ float mantissa_1p(uint32_t w) { return __uint_as_float(__funnelshift_r(w, 0x7Fu, 9)); }
+// a with the sign of s folded in: a * copysign(1, s), on the integer pipe
+__device__ __forceinline__ float xor_sign(float a, float s) { return __uint_as_float(__float_as_uint(a) ^ (__float_as_uint(s) & 0x80000000u)); }
+
 // ANISO: bit 0 uniaxial (uniform axis), bit 1 cubic.  FIELD: Zeeman term.  RT: colour-sites per row as a compile-time
 // constant (0 = run-time value; the specialisations turn every shared-memory offset into an immediate).
 // sum S.h is accumulated by the black pass only (every bond joins a red and a black site, so
 // E_exch = -J sum_{i black} S_i.h_i with h already in registers).
+// On-site energies of the FINAL spin reuse what dE needs: cubic through s4 = sum_a S_a^4 (on the unit sphere
+// Sx^2Sy^2 + Sx^2Sz^2 + Sy^2Sz^2 = (1 - s4)/2, so dE_c = -Kc/2 (s4' - s4) and E_c = Kc/2 (1 - s4)), uniaxial through
+// (S.e)^2 and its difference form.
 template <int ANISO, bool FIELD, int RT, bool DEBUG>
 __global__ void __launch_bounds__(TILE_MAX_THREADS, TILE_MIN_BLOCKS)
 tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileGeom G, int colour, float invT, int flags,
-                 float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
+                  float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
 {
     extern __shared__ __align__(128) float smem[];
     __shared__ __align__(8) unsigned long long bars[TILE_NSLOT];
@@ -128,8 +136,8 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
     const int y0 = slab * G.Ty;
     const int Lz = G.Lz + (seg < G.Lz_rem ? 1 : 0);
     const int z0 = seg * G.Lz + (seg < G.Lz_rem ? seg : G.Lz_rem);
-    const int nrows = (RT ? TILE_TY_RT : G.Ty) + 2;          // the specialisations fix the slab height too
-    const int CS = nrows * R;                                // floats between components inside a slot
+    const int nrows = (RT ? TILE_TY_RT : G.Ty) + 2;
+    const int CS = nrows * R;
     const int slot_floats = 3 * CS;
 
     const float* Oth = P.S + (long long)(1 - colour) * 3 * P.plane;
@@ -141,68 +149,63 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
 #pragma unroll
         for (int s = 0; s < TILE_NSLOT; ++s) mbar_init(bar_base + 8u * s, 1u);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        // prologue: planes z0-1 .. z0+2 (sequence index 0..3)
         const int nseq = Lz + 2 < TILE_NSLOT ? Lz + 2 : TILE_NSLOT;
         for (int k = 0; k < nseq; ++k) {
             int z = z0 - 1 + k; if (z < 0) z += G.nz; else if (z >= G.nz) z -= G.nz;
             tile_issue_plane(G, R, Oth, P.plane, z, y0, smem_base + (uint32_t)k * slot_bytes, bar_base + 8u * k);
         }
     }
-    __syncthreads();                                         // barriers initialised before anyone waits on them
+    __syncthreads();
 
-    // ---- per-thread invariants: a thread owns pair cp of rows r0, r0+RP, .. of the slab for the whole march
     const bool active = tid < G.n_active;
     const int r0 = tid / PR, cp = tid - r0 * PR;
-    const int exL = (cp == 0) ? R - 1 : 2 * cp - 1;          // x-neighbour outside the pair: left (row parity 0) ...
-    const int exR = (cp == PR - 1) ? 0 : 2 * cp + 2;         // ... or right (row parity 1), periodic in x
-    const int pbase = (y0 + r0 + z0 + colour) & 1;
-    const int soff0 = (r0 + 1) * R + 2 * cp;                 // centre element inside a component block of a slot
+    const int exL = (cp == 0) ? R - 1 : 2 * cp - 1;
+    const int exR = (cp == PR - 1) ? 0 : 2 * cp + 2;
+    const int soff0 = (r0 + 1) * R + 2 * cp;
     const int exo0 = (r0 + 1) * R;
-    const int pstride = G.RP * R;                            // floats between the rows of consecutive passes
+    const int pstride = G.RP * R;
     const long long zstride = (long long)G.ny * R;
-    float* gS0 = Sc + ((long long)z0 * G.ny + y0 + r0) * R + 2 * cp;
-    const uint32_t site00 = (uint32_t)(((long long)z0 * G.ny + y0 + r0) * G.nx) + 4u * (uint32_t)cp;
+    float* gS = Sc + ((long long)z0 * G.ny + y0 + r0) * R + 2 * cp;
+    uint32_t siteb = (uint32_t)(((long long)z0 * G.ny + y0 + r0) * G.nx) + 4u * (uint32_t)cp;
     const uint32_t zsite = (uint32_t)(G.ny * G.nx), psite = (uint32_t)(G.RP * G.nx);
+    int parz = (y0 + r0 + z0 + colour) & 1;
 
     f2 aMx = splat(0.f), aMy = splat(0.f), aMz = splat(0.f), aEx = splat(0.f), aAn = splat(0.f);
     int cnt = 0;
 
-    const f2 two = splat(2.0f);
-    const float CU = 0.99999994f;                            // 1 - 2^-24: u = f - CU with f in [1,2) (C-8)
+    const float CU = 0.99999994f;
     const f2 nomc2 = splat(-omc);
-    const f2 twopi2 = splat(6.2831853071795865f), angc2 = splat(-(CU * 6.2831853071795865f) - 3.1415926535897932f);
+    const f2 twopi2 = splat(6.2831853071795865f), angc2 = splat(-9.4247779607693797f);     // phi - pi = 2 pi (f1 - 1) - pi
     const f2 nCU2 = splat(-CU);
-    const f2 xscale2 = splat(invT * 1.4426950408889634f);    // decision in base 2: dE/T * log2(e) + log2(u2) < 0
+    const f2 xscale2 = splat(invT * 1.4426950408889634f);
     const f2 nJ2 = splat(-P.J);
     const f2 e2x = splat(P.eu[0]), e2y = splat(P.eu[1]), e2z = splat(P.eu[2]);
     const f2 B2x = splat(P.B[0]), B2y = splat(P.B[1]), B2z = splat(P.B[2]);
-    const f2 nKu2 = splat(-P.Ku), nhKc2 = splat(-0.5f * P.Kc);
+    const f2 nKu2 = splat(-P.Ku), nhKc2 = splat(-0.5f * P.Kc), two = splat(2.0f);
 
-    for (int j = 0; j < Lz; ++j) {
-        if (j == 0) { mbar_wait(bar_base, 0u); mbar_wait(bar_base + 8u, 0u); }
+    mbar_wait(bar_base, 0u); mbar_wait(bar_base + 8u, 0u);
+    for (int j = 0; j < Lz; ++j, gS += zstride, siteb += zsite, parz ^= 1) {
         { const int k = j + 2; mbar_wait(bar_base + 8u * (k & 3), (uint32_t)(k >> 2) & 1u); }
-        const float* sM = smem + ((j) & 3) * slot_floats;          // plane z-1
-        const float* sC = smem + ((j + 1) & 3) * slot_floats;      // plane z
-        const float* sP = smem + ((j + 2) & 3) * slot_floats;      // plane z+1
+        const float* sM = smem + ((j) & 3) * slot_floats;
+        const float* sC = smem + ((j + 1) & 3) * slot_floats;
+        const float* sP = smem + ((j + 2) & 3) * slot_floats;
 
         if (active) {
-            float* gS = gS0 + (long long)j * zstride;
-            uint32_t siteb = site00 + (uint32_t)j * zsite;
-            int soff = soff0, exo = exo0, parj = pbase + j;
-            for (int pass = 0; pass < G.NPASS; ++pass, gS += pstride, siteb += psite, soff += pstride, exo += pstride, parj += G.RP) {
-                const int par = parj & 1;                             // (y + z + colour) & 1
-                const uint32_t site0 = siteb + (uint32_t)par;
+            float* g = gS;
+            uint32_t sb = siteb;
+            int soff = soff0, exo = exo0, parj = parz;
+            for (int pass = 0; pass < G.NPASS; ++pass, g += pstride, sb += psite, soff += pstride, exo += pstride, parj += G.RP) {
+                const int par = parj & 1;
+                const uint32_t site0 = sb + (uint32_t)par;
                 const float* pC = sC + soff;
                 const float* pP = sP + soff;
                 const float* pM = sM + soff;
                 const float* pE = sC + exo + (par ? exR : exL);
 
-                // own colour: one LDG.64 per component
-                const f2 Sx = *reinterpret_cast<const f2*>(gS);
-                const f2 Sy = *reinterpret_cast<const f2*>(gS + P.plane);
-                const f2 Sz = *reinterpret_cast<const f2*>(gS + 2 * P.plane);
+                const f2 Sx = *reinterpret_cast<const f2*>(g);
+                const f2 Sy = *reinterpret_cast<const f2*>(g + P.plane);
+                const f2 Sz = *reinterpret_cast<const f2*>(g + 2 * P.plane);
 
-                // exchange field h = sum of the 6 neighbours (first term of Eq. 2), J applied in dE
                 f2 h[3];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
@@ -212,72 +215,71 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
                     const f2 ym = *reinterpret_cast<const f2*>(pC + c * CS - R);
                     const f2 zp = *reinterpret_cast<const f2*>(pP + c * CS);
                     const f2 zm = *reinterpret_cast<const f2*>(pM + c * CS);
-                    // par = 0: x-neighbours of the two sites are (ex, o.x) and (o.x, o.y);  par = 1: (o.x, o.y) and (o.y, ex)
                     const f2 sh = par ? make_float2(o.y, ex) : make_float2(ex, o.x);
                     h[c] = add2(add2(add2(o, sh), add2(yp, ym)), add2(zp, zm));
                 }
 
-                // random numbers: one Philox4x32-10 call per site (a-2)
-                uint32_t ra0, ra1, ra2, ra3, rb0, rb1, rb2, rb3;
-                philox4x32_10(key, site0, c1, c2, c3, ra0, ra1, ra2, ra3);
-                philox4x32_10(key, site0 + 2u, c1, c2, c3, rb0, rb1, rb2, rb3);
-                const f2 f0 = make_float2(__uint_as_float(__funnelshift_r(ra0, 0x7Fu, 9)), __uint_as_float(__funnelshift_r(rb0, 0x7Fu, 9)));
-                const f2 f1 = make_float2(__uint_as_float(__funnelshift_r(ra1, 0x7Fu, 9)), __uint_as_float(__funnelshift_r(rb1, 0x7Fu, 9)));
-                const f2 f2u = make_float2(__uint_as_float(__funnelshift_r(ra2, 0x7Fu, 9)), __uint_as_float(__funnelshift_r(rb2, 0x7Fu, 9)));
+                // random numbers (a-2): one Philox4x32-10 block per x-adjacent pair: words 0,1 -> first site, words 2,3 -> second site (C-26)
+                uint32_t r0w, r1w, r2w, r3w;
+                philox4x32_10(key, site0, c1, c2, c3, r0w, r1w, r2w, r3w);
+                const f2 f0 = make_float2(mantissa_1p(r0w), mantissa_1p(r2w));
+                const f2 f2u = make_float2(mantissa_1p(r1w), mantissa_1p(r3w));
+                const f2 f1 = make_float2(azimuth_1p(r0w, r1w), azimuth_1p(r2w, r3w));
 
-                // cone move (a-4; C-6, C-7): d = sa (cos(phi) t1 + sin(phi) t2) - w S
-                const f2 nw = mul2(add2(f0, nCU2), nomc2);                           // -w,  w = u0 (1 - cos theta); u0 = f0 - CU exactly
-                const f2 t  = mul2(nw, fma2(nw, splat(-1.0f), splat(-2.0f)));        // w (2 - w) = sin^2(alpha)
+                const f2 nw = mul2(add2(f0, nCU2), nomc2);
+                const f2 t  = mul2(nw, fma2(nw, splat(-1.0f), splat(-2.0f)));
                 const f2 sa = mul2(t, make_float2(rsqrtf(t.x), rsqrtf(t.y)));
-                const f2 ang = fma2(f1, twopi2, angc2);                              // phi - pi in (-pi, pi)
-                // cos(phi) = -cos(ang), sin(phi) = -sin(ang): the minus signs are folded into the frame (nt1 = -t1, nt2 = -t2)
+                const f2 ang = fma2(f1, twopi2, angc2);
                 const f2 Cc = mul2(sa, make_float2(__cosf(ang.x), __cosf(ang.y)));
                 const f2 Ss = mul2(sa, make_float2(__sinf(ang.x), __sinf(ang.y)));
                 const f2 sg = make_float2(copysignf(1.0f, Sz.x), copysignf(1.0f, Sz.y));
                 const f2 den = add2(sg, Sz);
-                const f2 ia = make_float2(__fdividef(1.0f, den.x), __fdividef(1.0f, den.y));   // -a of the frame construction
+                const f2 ia = make_float2(__fdividef(1.0f, den.x), __fdividef(1.0f, den.y));
                 const f2 uu = mul2(Sx, ia), vv = mul2(Sy, ia);
-                const f2 q  = mul2(sg, Sx);
-                const f2 nt1x = fma2(q, uu, splat(-1.0f));      // -(1 + sg Sx^2 a)
-                const f2 nt1y = mul2(q, vv);                    // -(sg b),  b = Sx Sy a
-                const f2 nt2x = mul2(Sy, uu);                   // -b
-                const f2 nt2y = fma2(Sy, vv, make_float2(-sg.x, -sg.y));   // -(sg + Sy^2 a)
-                // nt1z = q = sg Sx,  nt2z = Sy
+                const f2 q  = make_float2(xor_sign(Sx.x, Sz.x), xor_sign(Sx.y, Sz.y));      // sg * Sx
+                const f2 nt1x = fma2(q, uu, splat(-1.0f));
+                const f2 nt1y = mul2(q, vv);
+                const f2 nt2x = mul2(Sy, uu);
+                const f2 nt2y = fma2(Sy, vv, make_float2(-sg.x, -sg.y));
                 const f2 dx = fma2(Cc, nt1x, fma2(Ss, nt2x, mul2(nw, Sx)));
                 const f2 dy = fma2(Cc, nt1y, fma2(Ss, nt2y, mul2(nw, Sy)));
                 const f2 dz = fma2(Cc, q,    fma2(Ss, Sy,   mul2(nw, Sz)));
                 const f2 vx = add2(Sx, dx), vy = add2(Sy, dy), vz = add2(Sz, dz);
-                const f2 n2 = fma2(vx, vx, fma2(vy, vy, mul2(vz, vz)));
-                const f2 inv = fma2(n2, splat(-0.5f), splat(1.5f));                  // 1/|v| to O(eps^2), |v|^2 = 1 + O(1e-7)
+                const f2 V2x = mul2(vx, vx), V2y = mul2(vy, vy), V2z = mul2(vz, vz);
+                const f2 n2 = add2(add2(V2x, V2y), V2z);
+                const f2 inv = fma2(n2, splat(-0.5f), splat(1.5f));
                 const f2 Nx = mul2(vx, inv), Ny = mul2(vy, inv), Nz = mul2(vz, inv);
 
-                // energy difference (a-5), difference form: -J d.h - d.B - Ku (d.e)((2S+d).e) - Kc/2 sum_a (n_a^2 - S_a^2)(n_a^2 + S_a^2)
                 const f2 dh = fma2(dx, h[0], fma2(dy, h[1], mul2(dz, h[2])));
                 f2 dE = mul2(nJ2, dh);
                 if (FIELD) dE = fma2(splat(-1.0f), fma2(dx, B2x, fma2(dy, B2y, mul2(dz, B2z))), dE);
+                f2 eu_old = splat(0.f), eu_new = splat(0.f);
                 if (ANISO & 1) {
                     const f2 de = fma2(dx, e2x, fma2(dy, e2y, mul2(dz, e2z)));
                     const f2 se = fma2(Sx, e2x, fma2(Sy, e2y, mul2(Sz, e2z)));
-                    dE = fma2(nKu2, mul2(de, fma2(two, se, de)), dE);
+                    const f2 du = mul2(de, fma2(two, se, de));                  // (v.e)^2 - (S.e)^2, difference form
+                    dE = fma2(nKu2, du, dE);
+                    eu_old = mul2(se, se); eu_new = add2(eu_old, du);
                 }
+                f2 s4S = splat(0.f), s4v = splat(0.f);
                 if (ANISO & 2) {
-                    const f2 gx = mul2(dx, add2(Sx, vx)), gy = mul2(dy, add2(Sy, vy)), gz = mul2(dz, add2(Sz, vz));   // n_a^2 - S_a^2
-                    const f2 tx = fma2(vx, vx, mul2(Sx, Sx)), ty = fma2(vy, vy, mul2(Sy, Sy)), tz = fma2(vz, vz, mul2(Sz, Sz));
-                    const f2 qs = fma2(gx, tx, fma2(gy, ty, mul2(gz, tz)));
-                    dE = fma2(nhKc2, qs, dE);
+                    // on the unit sphere Sx^2Sy^2 + Sx^2Sz^2 + Sy^2Sz^2 = (1 - s4)/2 with s4 = sum_a S_a^4
+                    const f2 S2x = mul2(Sx, Sx), S2y = mul2(Sy, Sy), S2z = mul2(Sz, Sz);
+                    s4S = fma2(S2x, S2x, fma2(S2y, S2y, mul2(S2z, S2z)));
+                    s4v = fma2(V2x, V2x, fma2(V2y, V2y, mul2(V2z, V2z)));
+                    dE = fma2(nhKc2, add2(s4v, make_float2(-s4S.x, -s4S.y)), dE);
                 }
 
-                // accept / reject (a-6; P:157-159 in log form, C-8)
                 const f2 u2 = add2(f2u, nCU2);
                 const f2 xd = fma2(dE, xscale2, make_float2(__log2f(u2.x), __log2f(u2.y)));
                 const bool ok0 = xd.x < 0.0f, ok1 = xd.y < 0.0f;
                 f2 Ox, Oy, Oz;
                 Ox.x = ok0 ? Nx.x : Sx.x; Oy.x = ok0 ? Ny.x : Sy.x; Oz.x = ok0 ? Nz.x : Sz.x;
                 Ox.y = ok1 ? Nx.y : Sx.y; Oy.y = ok1 ? Ny.y : Sy.y; Oz.y = ok1 ? Nz.y : Sz.y;
-                cnt += (int)ok0 + (int)ok1;                                          // P:160
-                *reinterpret_cast<f2*>(gS) = Ox;
-                *reinterpret_cast<f2*>(gS + P.plane) = Oy;
-                *reinterpret_cast<f2*>(gS + 2 * P.plane) = Oz;
+                cnt += (int)ok0 + (int)ok1;
+                *reinterpret_cast<f2*>(g) = Ox;
+                *reinterpret_cast<f2*>(g + P.plane) = Oy;
+                *reinterpret_cast<f2*>(g + 2 * P.plane) = Oz;
                 if (DEBUG) {
                     if (dbg_x)   { dbg_x[site0] = xd.x * 0.69314718055994531f; dbg_x[site0 + 2u] = xd.y * 0.69314718055994531f; }
                     if (dbg_acc) { dbg_acc[site0] = (uint8_t)ok0; dbg_acc[site0 + 2u] = (uint8_t)ok1; }
@@ -286,15 +288,11 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
                 // fused sums of the final spins (a-9)
                 aMx = add2(aMx, Ox); aMy = add2(aMy, Oy); aMz = add2(aMz, Oz);
                 if (colour) aEx = fma2(Ox, h[0], fma2(Oy, h[1], fma2(Oz, h[2], aEx)));
-                if (ANISO & 1) { const f2 se = fma2(Ox, e2x, fma2(Oy, e2y, mul2(Oz, e2z))); aAn = fma2(mul2(nKu2, se), se, aAn); }
-                if (ANISO & 2) {
-                    const f2 x2 = mul2(Ox, Ox), y2 = mul2(Oy, Oy), z2 = mul2(Oz, Oz);
-                    const f2 cub = fma2(x2, y2, fma2(x2, z2, mul2(y2, z2)));
-                    aAn = fma2(splat(P.Kc), cub, aAn);
-                }
+                if (ANISO & 1) aAn = fma2(nKu2, make_float2(ok0 ? eu_new.x : eu_old.x, ok1 ? eu_new.y : eu_old.y), aAn);
+                if (ANISO & 2) aAn = fma2(nhKc2, make_float2(ok0 ? s4v.x : s4S.x, ok1 ? s4v.y : s4S.y), aAn);
             }
         }
-        __syncthreads();                                     // every warp is done with plane z-1's slot
+        __syncthreads();
         if (tid == 0 && j + TILE_NSLOT < Lz + 2) {
             const int k = j + TILE_NSLOT;
             int zn = z0 - 1 + k; if (zn >= G.nz) zn -= G.nz;
@@ -303,11 +301,11 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
         }
     }
 
-    // ---- deterministic block reduction (pass 1) + election of the finalising block
     double acc[NQ];
     acc[0] = (double)aMx.x + (double)aMx.y; acc[1] = (double)aMy.x + (double)aMy.y; acc[2] = (double)aMz.x + (double)aMz.y;
     acc[3] = colour ? -(double)P.J * ((double)aEx.x + (double)aEx.y) : 0.0;
     acc[4] = (double)aAn.x + (double)aAn.y;
+    if ((ANISO & 2) && active) acc[4] += 0.5 * (double)P.Kc * (double)(2 * G.NPASS * Lz);     // the "1" of (1 - s4)/2, once per site
     acc[5] = FIELD ? -(acc[0] * (double)P.B[0] + acc[1] * (double)P.B[1] + acc[2] * (double)P.B[2]) : 0.0;
     acc[6] = acc[7] = acc[8] = 0.0;
     block_partials(acc, cnt, P, colour);
@@ -316,5 +314,4 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
         if (last_block_done(st)) final_reduce(P, 0, flags);
     }
 }
-
 }  // namespace mc

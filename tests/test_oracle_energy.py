@@ -101,7 +101,9 @@ def test_torque_is_minus_dE_by_rotation_angle():
 
 @pytest.mark.parametrize("case", CASES[:4])
 def test_half_sweep_wiring_decision_variable_and_stream(case):
-    """x = dE/T + ln u2 with (u0,u1,u2) = words 0,1,2 of Philox(key=seed, ctr=(site, colour<<8, sweep)); S' = cone(S,u0,u1)."""
+    """x = dE/T + ln u2; S' = cone(S,u0,u1); the uniforms follow reading C-26: sites x and x^2 of a row share the block
+    Philox(key=seed, ctr=(index of the one with bit 1 of x clear, colour<<8, sweep)), two words each:
+    u0 = top 23 bits of w0, u2 = top 23 bits of w1 (+ half), u1 = the 9 + 9 low bits (retyped here in integer arithmetic)."""
     seed = (7 << 32) | 123
     o = _make(case, seed=seed, cone0=0.9, adaptive=False)
     o.set_sweep((5 << 32) | 17)
@@ -120,8 +122,12 @@ def test_half_sweep_wiring_decision_variable_and_stream(case):
                             B=(0.05, -0.02, 0.13), bond_mask=o._mask)
         chk.set_spins(before)
         for site in np.nonzero(col == colour)[0][:40]:
-            r = oracle.philox4x32_10([site, colour << 8, 17, 5], [123, 7])
-            u = [oracle.uniform(int(v)) for v in r]
+            x_site = int(xs[site])
+            first = int(site) - (x_site & 2)
+            r = [int(v) for v in oracle.philox4x32_10([first, colour << 8, 17, 5], [123, 7])]
+            w0, w1 = (r[2], r[3]) if (x_site & 2) else (r[0], r[1])
+            u = [((w0 >> 9) + 0.5) / 2**23, (((w0 & 511) << 9) | (w1 & 511)) / 2**18, ((w1 >> 9) + 0.5) / 2**23]
+            assert u == list(o.site_uniforms(x_site, int(ys[site]), int(zs[site]), colour, (5 << 32) | 17))
             Sn = oracle.cone_move(before[site], 0.9, u[0], u[1])
             xd = (chk.site_energy(site, Sn) - chk.site_energy(site, before[site])) / T + np.log(u[2])
             assert abs(xd - x[site]) < 1e-12

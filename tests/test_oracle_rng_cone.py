@@ -68,6 +68,48 @@ def test_p2_uniform_moments():
     assert abs(us.var() - 1 / 12) < 4 * np.sqrt(1 / 180 / n)
 
 
+def test_p2_site_uniforms_use_every_bit_of_their_two_words_once():
+    """Reading C-26: u0 <- bits 31..9 of w0, u2 <- bits 31..9 of w1, u1 <- bits 8..0 of w0 then bits 8..0 of w1."""
+    rng = np.random.default_rng(1)
+    for _ in range(300):
+        w0, w1 = (int(v) for v in rng.integers(0, 2**32, size=2, dtype=np.uint64))
+        u1 = oracle.uniform_azimuth(w0, w1)
+        assert 0.0 <= u1 < 1.0 and float(np.float32(u1)) == u1 and float(np.float32(1.0 + u1)) == 1.0 + u1
+        assert u1 == (((w0 & 511) << 9) | (w1 & 511)) / 2**18
+        bit = int(rng.integers(0, 32))
+        for which in (0, 1):
+            v0, v1 = (w0 ^ (1 << bit), w1) if which == 0 else (w0, w1 ^ (1 << bit))
+            changed = [oracle.uniform(v0) != oracle.uniform(w0), oracle.uniform_azimuth(v0, v1) != u1, oracle.uniform(v1) != oracle.uniform(w1)]
+            expect = [which == 0 and bit >= 9, bit < 9, which == 1 and bit >= 9]
+            assert changed == expect
+    assert oracle.uniform_azimuth(0, 0) == 0.0 and oracle.uniform_azimuth(0x1FF, 0x1FF) == 1.0 - 2.0**-18
+
+
+def test_p2_site_uniforms_pair_sharing_and_moments():
+    """Sites x and x^2 of a row read the two halves of one block; different rows, colours and sweeps read other blocks;
+    all three uniforms of a site are flat and mutually uncorrelated over the lattice."""
+    o = oracle.Oracle(16, 8, 8, seed=99)
+    key = [99, 0]
+    u = {}
+    for z in range(8):
+        for y in range(8):
+            for x in range(16):
+                u[(x, y, z)] = o.site_uniforms(x, y, z, (x + y + z) & 1, 7)
+    for (x, y, z), got in list(u.items())[::17]:
+        first = (x & ~2) + 16 * (y + 8 * z)
+        r = [int(v) for v in oracle.philox4x32_10([first, ((x + y + z) & 1) << 8, 7, 0], key)]
+        w0, w1 = (r[2], r[3]) if x & 2 else (r[0], r[1])
+        assert got == (oracle.uniform(w0), oracle.uniform_azimuth(w0, w1), oracle.uniform(w1))
+    assert len({v for v in u.values()}) == len(u)                      # no two sites share their numbers
+    assert o.site_uniforms(0, 0, 0, 0, 8) != u[(0, 0, 0)]             # the sweep moves the stream
+    a = np.array(list(u.values())); n = len(a)
+    for k in range(3):
+        assert abs(a[:, k].mean() - 0.5) < 4 * np.sqrt(1 / 12 / n)
+        assert abs(a[:, k].var() - 1 / 12) < 5 * np.sqrt(1 / 180 / n)
+    c = np.corrcoef(a.T)
+    assert np.abs(c - np.eye(3)).max() < 4 / np.sqrt(n)
+
+
 # ---------------------------------------------------------------------------------------- P-3 cone move
 def _spins():
     rng = np.random.default_rng(5)
