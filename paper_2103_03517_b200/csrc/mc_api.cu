@@ -19,12 +19,12 @@ constexpr size_t ALIGN = 256;
 inline size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {            // byte offsets into the caller's workspace
-    size_t spins, mask, region, axis, state, partials, trace, total;
+    size_t spins, mask, region, axis, state, trace, total;
     long long plane, mask_plane, region_plane;
     int max_blocks;
 };
 
-constexpr int MAX_BLOCKS = 148 * 32;     // upper bound on the grid of a pass kernel (partials are sized for it)
+constexpr int MAX_BLOCKS = 148 * 32;     // upper bound on the grid of a pass kernel
 
 bool needs_mask(const mc_lattice* lat, const mc_hamiltonian* ham)
 {
@@ -58,7 +58,6 @@ Layout make_layout(const mc_lattice* lat, const mc_hamiltonian* ham)
     L.region = off;   if (ham->region) off += round_up((size_t)2 * L.region_plane * sizeof(uint16_t), ALIGN);
     L.axis = off;     if (ham->region) off += round_up((size_t)ham->n_regions * sizeof(float4), ALIGN);
     L.state = off;    off += round_up(sizeof(DevState), ALIGN);
-    L.partials = off; off += round_up((size_t)4 * L.max_blocks * NQ * sizeof(double), ALIGN);
     L.trace = off;    off += round_up((size_t)TRACE_CAP * 6 * sizeof(double), ALIGN);
     L.total = off;
     return L;
@@ -336,7 +335,14 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     for (int a = 0; a < 3; ++a) { P.eu[a] = (float)ctx->eu[a]; P.B[a] = (float)ham->B[a]; }
     P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32);
     P.key = philox_key(P.seed_lo, P.seed_hi);
-    P.st = (DevState*)(ws + L.state); P.partials = (double*)(ws + L.partials); P.max_blocks = L.max_blocks;
+    P.st = (DevState*)(ws + L.state); P.max_blocks = L.max_blocks;
+    {   // fixed-point unit 2^-k of the fused sums: the largest k <= 40 with N * (largest per-site term) * 2^k < 2^61
+        const double bmag = sqrt(ham->B[0] * ham->B[0] + ham->B[1] * ham->B[1] + ham->B[2] * ham->B[2]);
+        const double mag = 1.0 + 6.0 * fabs(ham->J) + 2.0 * fabs(ham->Ku) + 2.0 * fabs(ham->Kc) + bmag;
+        int lg = 0; while (ldexp(1.0, lg) < (double)N * mag) ++lg;
+        int k = 61 - lg; if (k > 40) k = 40;
+        P.fx_scale = (float)ldexp(1.0, k); P.fx_inv = ldexp(1.0, -k);
+    }
     P.trace = (double*)(ws + L.trace);
 
     ctx->aniso = (ham->Ku != 0.0 ? 1 : 0) | (ham->Kc != 0.0 ? 2 : 0);

@@ -17,6 +17,7 @@ constexpr int NQ = 9;          // fused sums: Mx My Mz E_exch E_aniso E_zeeman t
 constexpr int BLOCK = 256;     // threads per CTA of the generic pass kernels
 constexpr int MAX_WARPS = 32;  // largest CTA any kernel that reduces uses (1024 threads); block sizes are warp multiples
 constexpr int TRACE_CAP = 16384;
+constexpr int FLUSH_ITEMS = 8;  // items a thread sums in fp32 before the sums go to 64-bit fixed point
 
 // Controller / reduction state, resident in the workspace (no host round trip per sweep: P:165-171 runs on the device)
 struct DevState {
@@ -26,7 +27,7 @@ struct DevState {
     int adaptive;
     unsigned long long count;        // accepted moves of the sweep in flight (integer atomics: order independent)
     unsigned int ticket;             // last-block election
-    unsigned int nblocks[4];         // grid size of the pass whose partials wait in slot: 0,1 sweep red/black; 2,3 measurement
+    unsigned int pad4_[4];
     unsigned int pad_;
     double last_acceptance;
     double sums[NQ];                 // fused sums of the last completed sweep
@@ -36,6 +37,7 @@ struct DevState {
     unsigned long long n_samples;
     double sum_m[4], sum_m2[4], sum_E, sum_E2, sum_torque[3];
     unsigned long long trace_rows;   // rows ever written to the trace ring
+    long long isum[2][NQ];           // exact fixed-point sums in flight: [0] the sweep (both colour passes), [1] the measurement
 };
 
 struct Params {
@@ -53,7 +55,8 @@ struct Params {
     uint32_t seed_lo, seed_hi;
     PhiloxKey key;                   // the 10 round keys of (seed_lo, seed_hi), filled by the host: constant-bank operands
     DevState* st;
-    double* partials;                // [4][max_blocks][NQ]: slots 0,1 = sweep red/black, 2,3 = measurement red/black
+    float fx_scale;                  // 2^k: fixed-point unit of the fused sums is 2^-k (k chosen by the host so that N * 8 * 2^k < 2^62)
+    double fx_inv;                   // 2^-k
     int max_blocks;
     double* trace;                   // [TRACE_CAP][6]
 };
@@ -191,16 +194,31 @@ __device__ __forceinline__ void easy_axes(const Params& P, const ItemPos& q, int
 // Block reduction of the per-thread fused sums in a FIXED order (deterministic two-pass fp64 reduction, pass 1):
 // lanes by xor-shuffle, warps sequentially; thread 0 writes the block partial.
 // --------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ double warp_sum(double v)
+
+// --------------------------------------------------------------------------------------------------------------
+// Fused sums (a-9), pass 1.  A thread carries fp32 partial sums over a small bounded set of sites, converts them ONCE to
+// 64-bit fixed point (unit 2^-k) and from there on every addition is an integer addition: exact, hence independent of
+// the order (warp shuffles, warps of a block, one 64-bit atomic per block and quantity) and bitwise reproducible.
+// fp64 enters in pass 2 only (final_reduce).  Why not fp64 partials: fp64 adds issue an order of magnitude slower than
+// integer adds on this part, and the chain of them sat on the exposed tail of every colour pass.
+// --------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void fx_flush(long long (&acc)[NQ], float (&f)[NQ], float scale)
+{
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) { acc[q] += __float2ll_rn(f[q] * scale); f[q] = 0.0f; }
+}
+
+__device__ __forceinline__ long long warp_sum_i64(long long v)
 {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
 }
 
-__device__ __forceinline__ void block_partials(const double (&acc)[NQ], int cnt, const Params& P, int slot)
+// mode 0: sums of a sweep in flight; mode 1: standalone measurement
+__device__ __forceinline__ void block_reduce(const long long (&acc)[NQ], int cnt, const Params& P, int mode)
 {
-    __shared__ double sm[MAX_WARPS][NQ];
+    __shared__ long long sm[MAX_WARPS][NQ];
     __shared__ int scnt;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = (int)(blockDim.x >> 5);
     if (threadIdx.x == 0) scnt = 0;
@@ -208,67 +226,49 @@ __device__ __forceinline__ void block_partials(const double (&acc)[NQ], int cnt,
     const int wc = __reduce_add_sync(0xffffffffu, cnt);
     if (lane == 0 && wc) atomicAdd(&scnt, wc);
 #pragma unroll
-    for (int q = 0; q < NQ; ++q) { const double v = warp_sum(acc[q]); if (lane == 0) sm[warp][q] = v; }
+    for (int q = 0; q < NQ; ++q) { const long long v = warp_sum_i64(acc[q]); if (lane == 0) sm[warp][q] = v; }
     __syncthreads();
     if (threadIdx.x < NQ) {
-        double v = 0.0;
+        long long v = 0;
         for (int w = 0; w < nwarps; ++w) v += sm[w][threadIdx.x];
-        P.partials[((long long)slot * P.max_blocks + blockIdx.x) * NQ + threadIdx.x] = v;
+        if (v) atomicAdd(reinterpret_cast<unsigned long long*>(&P.st->isum[mode][threadIdx.x]), (unsigned long long)v);
     }
     if (threadIdx.x == 0 && scnt) atomicAdd(&P.st->count, (unsigned long long)scnt);
 }
 
 // Pass 2 of the reduction (one block, fixed order) + what follows a sweep: cone controller (P:168-171 read with
 // P:205-209; C-2, C-3, C-9), sweep counter, Eq. (6) accumulators, trace row.  mode 0: end of a sweep; 1: measurement.
-// This block runs alone at the tail of the black pass, so its latency is exposed: the controller state is staged
-// through shared memory with one coalesced read and one coalesced write (two L2 round trips instead of a chain of
-// dependent ones), and thread 0 does the scalar work on the shared copy.
+// Pass 1 left exact fixed-point totals in DevState.isum; here they become fp64.  This block runs alone at the tail of
+// the black pass, so its latency is exposed: the controller state is staged through shared memory with one coalesced
+// read and one coalesced write (two L2 round trips instead of a chain of dependent ones), thread 0 does the scalar
+// work on the shared copy.
 static_assert(sizeof(DevState) % 4 == 0, "DevState is staged as 32-bit words");
 __device__ void final_reduce(const Params& P, int mode, int flags)
 {
-    __shared__ double red[MAX_WARPS][NQ];
-    __shared__ double tot[NQ];
     __shared__ double cone_next[2];
     __shared__ float omc_next[2];
     __shared__ DevState sst;
     DevState* st = P.st;
     constexpr int NWORDS = (int)(sizeof(DevState) / 4);
-    const int nwarps = (int)(blockDim.x >> 5);
     for (int i = threadIdx.x; i < NWORDS; i += blockDim.x)
         reinterpret_cast<uint32_t*>(&sst)[i] = __ldcg(reinterpret_cast<const uint32_t*>(st) + i);
-    double acc[NQ];
-#pragma unroll
-    for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
-    for (int slot = 2 * mode; slot < 2 * mode + 2; ++slot) {
-        const unsigned nb = __ldcg(&st->nblocks[slot]);
-        for (unsigned b = threadIdx.x; b < nb; b += blockDim.x) {
-            const double* p = P.partials + ((long long)slot * P.max_blocks + b) * NQ;
-#pragma unroll
-            for (int q = 0; q < NQ; ++q) acc[q] += __ldcg(p + q);
-        }
-    }
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-    for (int q = 0; q < NQ; ++q) { const double v = warp_sum(acc[q]); if (lane == 0) red[warp][q] = v; }
     __syncthreads();
-    // warps in a fixed order, one thread per quantity; another thread meanwhile evaluates both possible next cone angles
-    const int cone_thread = blockDim.x > 32 ? 32 : NQ;
-    if (threadIdx.x < NQ) {
-        double v = 0.0;
-        for (int w = 0; w < nwarps; ++w) v += red[w][threadIdx.x];
-        tot[threadIdx.x] = v;
-    } else if ((int)threadIdx.x == cone_thread && mode == 0) {
+    // one thread evaluates both possible next cone angles while thread 0 does the rest
+    const int cone_thread = blockDim.x > 32 ? 32 : 1;
+    if ((int)threadIdx.x == cone_thread && mode == 0) {
         const double deg = 3.14159265358979323846 / 180.0, pi = 3.14159265358979323846;
         double up = sst.cone + deg; if (up > pi) up = pi;
         double dn = sst.cone - deg; if (dn < deg) dn = deg;
         cone_next[0] = up; cone_next[1] = dn;
         omc_next[0] = (float)(1.0 - cos(up)); omc_next[1] = (float)(1.0 - cos(dn));
     }
+    double s[NQ];
+    if (threadIdx.x == 0) {
+        for (int q = 0; q < NQ; ++q) { s[q] = (double)sst.isum[mode][q] * P.fx_inv; sst.isum[mode][q] = 0; }
+    }
     __syncthreads();
     if (threadIdx.x == 0) {
         DevState& S = sst;
-        double s[NQ];
-        for (int q = 0; q < NQ; ++q) s[q] = tot[q];
         S.ML = s[0] * S.eC[0] + s[1] * S.eC[1] + s[2] * S.eC[2];
         if (mode == 1) {
             for (int q = 0; q < NQ; ++q) S.meas[q] = s[q];
@@ -336,10 +336,11 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
     float* Sc = P.S + (long long)colour * 3 * P.plane;
     const Vec3 B = { P.B[0], P.B[1], P.B[2] };
 
-    double acc[NQ];
+    long long acc[NQ];               // exact fixed-point sums of this thread (fx_flush)
+    float fs[NQ];                    // fp32 running sums of at most FLUSH_ITEMS items
 #pragma unroll
-    for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
-    int cnt = 0;
+    for (int q = 0; q < NQ; ++q) { acc[q] = 0; fs[q] = 0.0f; }
+    int cnt = 0, pending = 0;
 
     const uint32_t stride = gridDim.x * BLOCK;
     for (uint32_t item = blockIdx.x * BLOCK + threadIdx.x; item < G.n_items; item += stride) {
@@ -352,7 +353,6 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
         float f[NQ];
 #pragma unroll
         for (int k = 0; k < NQ; ++k) f[k] = 0.0f;
-#pragma unroll
         // random words: one Philox4x32-10 block per pair of x-neighbours (x, x ^ 2) of this colour, two words per site (C-26)
         uint32_t w0[VEC], w1[VEC];
         if (MODE == MODE_SWEEP) {
@@ -395,12 +395,12 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
             st_rw<VEC>(Sc + q.a0, nxv); st_rw<VEC>(Sc + P.plane + q.a0, nyv); st_rw<VEC>(Sc + 2 * P.plane + q.a0, nzv);
         }
 #pragma unroll
-        for (int k = 0; k < NQ; ++k) acc[k] += (double)f[k];
+        for (int k = 0; k < NQ; ++k) fs[k] += f[k];
+        if (++pending == FLUSH_ITEMS) { fx_flush(acc, fs, P.fx_scale); pending = 0; }
     }
+    fx_flush(acc, fs, P.fx_scale);
 
-    const int slot = (MODE == MODE_MEASURE ? 2 : 0) + colour;
-    block_partials(acc, cnt, P, slot);
-    if (threadIdx.x == 0) st->nblocks[slot] = gridDim.x;
+    block_reduce(acc, cnt, P, MODE == MODE_MEASURE ? 1 : 0);
     if (flags & F_FINALIZE) {
         if (last_block_done(st)) final_reduce(P, MODE == MODE_MEASURE ? 1 : 0, flags);
     }
@@ -472,10 +472,11 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
     float* Sc = P.S + (long long)colour * 3 * P.plane;
     const Vec3 B = { P.B[0], P.B[1], P.B[2] };
 
-    double acc[NQ];
+    long long acc[NQ];               // exact fixed-point sums of this thread (fx_flush)
+    float fs[NQ];                    // fp32 running sums of at most FLUSH_ITEMS items
 #pragma unroll
-    for (int q = 0; q < NQ; ++q) acc[q] = 0.0;
-    int cnt = 0;
+    for (int q = 0; q < NQ; ++q) { acc[q] = 0; fs[q] = 0.0f; }
+    int cnt = 0, pending = 0;
 
     const uint32_t stride = gridDim.x * BLOCK;
     for (uint32_t t = blockIdx.x * BLOCK + threadIdx.x; t < G.n_threads; t += stride) {
@@ -591,11 +592,12 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
         st_rw<VEC>(Sc + aL, nlx); st_rw<VEC>(Sc + P.plane + aL, nly); st_rw<VEC>(Sc + 2 * P.plane + aL, nlz);
         st_rw<VEC>(Sc + aF, nfx); st_rw<VEC>(Sc + P.plane + aF, nfy); st_rw<VEC>(Sc + 2 * P.plane + aF, nfz);
 #pragma unroll
-        for (int k = 0; k < NQ; ++k) acc[k] += (double)f[k];
+        for (int k = 0; k < NQ; ++k) fs[k] += f[k];
+        if (++pending == FLUSH_ITEMS) { fx_flush(acc, fs, P.fx_scale); pending = 0; }
     }
+    fx_flush(acc, fs, P.fx_scale);
 
-    block_partials(acc, cnt, P, colour);
-    if (threadIdx.x == 0) st->nblocks[colour] = gridDim.x;
+    block_reduce(acc, cnt, P, 0);
     if (flags & F_FINALIZE) {
         if (last_block_done(st)) final_reduce(P, 0, flags);
     }

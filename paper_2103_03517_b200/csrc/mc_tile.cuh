@@ -301,15 +301,19 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
         }
     }
 
-    double acc[NQ];
-    acc[0] = (double)aMx.x + (double)aMx.y; acc[1] = (double)aMy.x + (double)aMy.y; acc[2] = (double)aMz.x + (double)aMz.y;
-    acc[3] = colour ? -(double)P.J * ((double)aEx.x + (double)aEx.y) : 0.0;
-    acc[4] = (double)aAn.x + (double)aAn.y;
-    if ((ANISO & 2) && active) acc[4] += 0.5 * (double)P.Kc * (double)(2 * G.NPASS * Lz);     // the "1" of (1 - s4)/2, once per site
-    acc[5] = FIELD ? -(acc[0] * (double)P.B[0] + acc[1] * (double)P.B[1] + acc[2] * (double)P.B[2]) : 0.0;
-    acc[6] = acc[7] = acc[8] = 0.0;
-    block_partials(acc, cnt, P, colour);
-    if (threadIdx.x == 0) st->nblocks[colour] = gridDim.x;
+    // ---- pass 1 of the fused sums: this thread's fp32 sums (<= 2 NPASS Lz sites) -> 64-bit fixed point -> exact block sums
+    float f[NQ];
+    f[0] = aMx.x + aMx.y; f[1] = aMy.x + aMy.y; f[2] = aMz.x + aMz.y;
+    f[3] = colour ? -P.J * (aEx.x + aEx.y) : 0.0f;
+    f[4] = aAn.x + aAn.y;
+    if ((ANISO & 2) && active) f[4] += 0.5f * P.Kc * (float)(2 * G.NPASS * Lz);      // the "1" of (1 - s4)/2, once per site
+    f[5] = FIELD ? -(f[0] * P.B[0] + f[1] * P.B[1] + f[2] * P.B[2]) : 0.0f;
+    f[6] = f[7] = f[8] = 0.0f;
+    long long acc[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) acc[q] = 0;
+    fx_flush(acc, f, P.fx_scale);
+    block_reduce(acc, cnt, P, 0);
     if (flags & F_FINALIZE) {
         if (last_block_done(st)) final_reduce(P, 0, flags);
     }
