@@ -147,10 +147,10 @@ template <int RT, bool DEBUG> TileFn pick_tile_rt(int aniso, bool field)
 // Row lengths with a specialised instantiation (every shared-memory offset an immediate): R = nx/2 of BASELINE's
 // periodic configs c2 (64^3), c4 (128^3) and c3 (224^3).  Any other R runs the run-time-R instantiation.
 // The decision-variable debug outputs of the test hooks exist only in the run-time-R instantiation (same arithmetic).
-TileFn pick_tile(int R, int Ty, bool debug, int aniso, bool field)
+TileFn pick_tile(int R, int Ty, int npass, bool debug, int aniso, bool field)
 {
     if (debug) return pick_tile_rt<0, true>(aniso, field);
-    if (getenv("MC_B200_NO_RT") || Ty != TILE_TY_RT) return pick_tile_rt<0, false>(aniso, field);
+    if (getenv("MC_B200_NO_RT") || Ty != TILE_TY_RT || npass != TILE_NPASS_RT) return pick_tile_rt<0, false>(aniso, field);
     switch (R) {
         case 32:  return pick_tile_rt<32, false>(aniso, field);
         case 64:  return pick_tile_rt<64, false>(aniso, field);
@@ -192,7 +192,7 @@ bool plan_tile(mc_ctx* c)
     c->tile_smem = TILE_NSLOT * slot_bytes(G.Ty);
     if (c->tile_smem > 200 * 1024) return false;
     // every instantiation this handle can launch must be allowed its dynamic shared memory
-    TileFn fns[2] = { pick_tile(R, G.Ty, false, c->aniso, c->field), pick_tile(R, G.Ty, true, c->aniso, c->field) };
+    TileFn fns[2] = { pick_tile(R, G.Ty, G.NPASS, false, c->aniso, c->field), pick_tile(R, G.Ty, G.NPASS, true, c->aniso, c->field) };
     int per_sm = 1;
     for (TileFn f : fns) {
         if (cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tile_smem) != cudaSuccess) { cudaGetLastError(); return false; }
@@ -224,23 +224,38 @@ int grid_for(const mc_ctx* c, uint32_t n_threads_needed)
     return (int)(g < 1 ? 1 : g);
 }
 
+// Launch of a pass kernel with programmatic dependent launch: the grid may be scheduled while the previous kernel of the
+// stream drains (every pass kernel starts with grid_dependency_sync(), so it reads nothing early).  Hides the launch
+// gap between the 2n back-to-back colour passes of mc_sweep(T, n).
+template <class Fn, class Geo>
+cudaError_t launch_dependent(Fn fn, int grid, int block, size_t smem, cudaStream_t stream, const Params& P, const Geo& G,
+                             int colour, float invT, int flags, float* dx, uint8_t* da)
+{
+    static const bool no_pdl = getenv("MC_B200_NO_PDL") != nullptr;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = no_pdl ? 0 : 1;
+    return cudaLaunchKernelEx(&cfg, fn, P, G, colour, invT, flags, dx, da);
+}
+
 int launch_pass(mc_ctx* ctx, int mode, int colour, float invT, int flags, float* dx, uint8_t* da)
 {
     if (mode == MODE_SWEEP && ctx->tile_ok) {
-        TileFn fn = pick_tile(ctx->tgeom.R, ctx->tgeom.Ty, dx || da, ctx->aniso, ctx->field);
+        TileFn fn = pick_tile(ctx->tgeom.R, ctx->tgeom.Ty, ctx->tgeom.NPASS, dx || da, ctx->aniso, ctx->field);
         const int grid = ctx->tgeom.n_slabs * ctx->tgeom.n_segs;
-        fn<<<grid, ctx->tile_threads, ctx->tile_smem, ctx->stream>>>(ctx->P, ctx->tgeom, colour, invT, flags, dx, da);
+        CU(launch_dependent(fn, grid, ctx->tile_threads, ctx->tile_smem, ctx->stream, ctx->P, ctx->tgeom, colour, invT, flags, dx, da));
         ctx->launches += 1;
-        CU(cudaGetLastError());
         return MC_OK;
     }
     PassFn fn = (ctx->vec == 4) ? (mode == MODE_SWEEP ? pick_pass<4, MODE_SWEEP>(ctx->aniso, ctx->masked) : pick_pass<4, MODE_MEASURE>(ctx->aniso, ctx->masked))
                                 : (mode == MODE_SWEEP ? pick_pass<1, MODE_SWEEP>(ctx->aniso, ctx->masked) : pick_pass<1, MODE_MEASURE>(ctx->aniso, ctx->masked));
     const int grid = grid_for(ctx, ctx->geom.n_items);
     // measurement uses partial slots 2,3 so that it never disturbs a sweep assembled from the half-sweep hooks
-    fn<<<grid, BLOCK, 0, ctx->stream>>>(ctx->P, ctx->geom, colour, invT, flags, dx, da);
+    CU(launch_dependent(fn, grid, BLOCK, 0, ctx->stream, ctx->P, ctx->geom, colour, invT, flags, dx, da));
     ctx->launches += 1;
-    CU(cudaGetLastError());
     return MC_OK;
 }
 
@@ -248,9 +263,8 @@ int launch_pair(mc_ctx* ctx, int colour, float invT, int flags, float* dx, uint8
 {
     PairFn fn = (ctx->vec == 4) ? pick_pair<4>(ctx->aniso, ctx->masked) : pick_pair<1>(ctx->aniso, ctx->masked);
     const int grid = grid_for(ctx, ctx->pgeom.n_threads);
-    fn<<<grid, BLOCK, 0, ctx->stream>>>(ctx->P, ctx->pgeom, colour, invT, flags, dx, da);
+    CU(launch_dependent(fn, grid, BLOCK, 0, ctx->stream, ctx->P, ctx->pgeom, colour, invT, flags, dx, da));
     ctx->launches += 1;
-    CU(cudaGetLastError());
     return MC_OK;
 }
 

@@ -9,6 +9,16 @@
 
 namespace mc {
 
+// Programmatic dependent launch (sm_90+): a grid launched with the programmatic-stream-serialization attribute may be
+// scheduled while its predecessor drains; griddepcontrol.wait blocks until the predecessor has completed and its writes
+// are visible, launch_dependents lets the successor be scheduled in turn.  Both are no-ops in an ordinary launch.
+// Every pass kernel calls this before it touches anything a previous kernel wrote.
+__device__ __forceinline__ void grid_dependency_sync()
+{
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;");
+}
+
 // Stream tags (counter word 1, low byte); colour goes to bits 8..
 constexpr uint32_t TAG_MOVE = 0u, TAG_PAIR = 1u, TAG_PAIRING = 2u;
 

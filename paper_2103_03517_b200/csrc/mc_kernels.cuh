@@ -329,6 +329,7 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
             float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
 {
     DevState* st = P.st;
+    grid_dependency_sync();
     const unsigned long long sweep = st->sweep;
     const float omc = st->one_minus_cos;
     const PhiloxKey& key = P.key;
@@ -456,6 +457,7 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
             float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
 {
     DevState* st = P.st;
+    grid_dependency_sync();
     const unsigned long long sweep = st->sweep;
     const float omc = st->one_minus_cos;
     const double ML = st->ML;

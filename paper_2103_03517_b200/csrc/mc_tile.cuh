@@ -34,6 +34,7 @@ constexpr int TILE_NSLOT = 4;
 constexpr int TILE_MAX_THREADS = MC_TILE_MAX_THREADS;   // launch bounds of the tiled pass: threads per CTA ...
 constexpr int TILE_MIN_BLOCKS = MC_TILE_MIN_BLOCKS;     // ... and CTAs per SM the register allocation must allow
 constexpr int TILE_TY_RT = MC_TILE_TY_RT;               // slab height of the compile-time-R specialisations
+constexpr int TILE_NPASS_RT = 2;                        // ... which a thread covers in this many passes (unrolled)
 
 struct TileGeom {
     int R, PR;                 // colour-sites per row, pairs per row
@@ -124,6 +125,7 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
     __shared__ __align__(8) unsigned long long bars[TILE_NSLOT];
 
     DevState* st = P.st;
+    grid_dependency_sync();          // nothing a previous pass wrote (spins, controller state) is touched before this point
     const unsigned long long sweep = st->sweep;
     const float omc = st->one_minus_cos;
     const PhiloxKey& key = P.key;
@@ -136,7 +138,8 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
     const int y0 = slab * G.Ty;
     const int Lz = G.Lz + (seg < G.Lz_rem ? 1 : 0);
     const int z0 = seg * G.Lz + (seg < G.Lz_rem ? seg : G.Lz_rem);
-    const int nrows = (RT ? TILE_TY_RT : G.Ty) + 2;
+    const int nrows = (RT ? TILE_TY_RT : G.Ty) + 2;                 // the specialisations fix the slab height ...
+    const int NPASS = RT ? TILE_NPASS_RT : G.NPASS, RP = RT ? TILE_TY_RT / TILE_NPASS_RT : G.RP;   // ... and its split into passes
     const int CS = nrows * R;
     const int slot_floats = 3 * CS;
 
@@ -163,11 +166,11 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
     const int exR = (cp == PR - 1) ? 0 : 2 * cp + 2;
     const int soff0 = (r0 + 1) * R + 2 * cp;
     const int exo0 = (r0 + 1) * R;
-    const int pstride = G.RP * R;
+    const int pstride = RP * R;
     const long long zstride = (long long)G.ny * R;
     float* gS = Sc + ((long long)z0 * G.ny + y0 + r0) * R + 2 * cp;
     uint32_t siteb = (uint32_t)(((long long)z0 * G.ny + y0 + r0) * G.nx) + 4u * (uint32_t)cp;
-    const uint32_t zsite = (uint32_t)(G.ny * G.nx), psite = (uint32_t)(G.RP * G.nx);
+    const uint32_t zsite = (uint32_t)(G.ny * G.nx), psite = (uint32_t)(RP * G.nx);
     int parz = (y0 + r0 + z0 + colour) & 1;
 
     f2 aMx = splat(0.f), aMy = splat(0.f), aMz = splat(0.f), aEx = splat(0.f), aAn = splat(0.f);
@@ -194,7 +197,8 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
             float* g = gS;
             uint32_t sb = siteb;
             int soff = soff0, exo = exo0, parj = parz;
-            for (int pass = 0; pass < G.NPASS; ++pass, g += pstride, sb += psite, soff += pstride, exo += pstride, parj += G.RP) {
+#pragma unroll (RT ? TILE_NPASS_RT : 1)
+            for (int pass = 0; pass < NPASS; ++pass, g += pstride, sb += psite, soff += pstride, exo += pstride, parj += RP) {
                 const int par = parj & 1;
                 const uint32_t site0 = sb + (uint32_t)par;
                 const float* pC = sC + soff;
@@ -306,7 +310,7 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
     f[0] = aMx.x + aMx.y; f[1] = aMy.x + aMy.y; f[2] = aMz.x + aMz.y;
     f[3] = colour ? -P.J * (aEx.x + aEx.y) : 0.0f;
     f[4] = aAn.x + aAn.y;
-    if ((ANISO & 2) && active) f[4] += 0.5f * P.Kc * (float)(2 * G.NPASS * Lz);      // the "1" of (1 - s4)/2, once per site
+    if ((ANISO & 2) && active) f[4] += 0.5f * P.Kc * (float)(2 * NPASS * Lz);      // the "1" of (1 - s4)/2, once per site
     f[5] = FIELD ? -(f[0] * P.B[0] + f[1] * P.B[1] + f[2] * P.B[2]) : 0.0f;
     f[6] = f[7] = f[8] = 0.0f;
     long long acc[NQ];
