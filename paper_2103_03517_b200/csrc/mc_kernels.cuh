@@ -199,8 +199,10 @@ __device__ __forceinline__ void easy_axes(const Params& P, const ItemPos& q, int
 // Fused sums (a-9), pass 1.  A thread carries fp32 partial sums over a small bounded set of sites, converts them ONCE to
 // 64-bit fixed point (unit 2^-k) and from there on every addition is an integer addition: exact, hence independent of
 // the order (warp shuffles, warps of a block, one 64-bit atomic per block and quantity) and bitwise reproducible.
-// fp64 enters in pass 2 only (final_reduce).  Why not fp64 partials: fp64 adds issue an order of magnitude slower than
-// integer adds on this part, and the chain of them sat on the exposed tail of every colour pass.
+// fp64 enters in pass 2 only (final_reduce).  Why not fp64 block partials re-read by the last block: their order had to
+// be fixed to be reproducible, so they went through an array in HBM that the finalising block re-read behind a chain of
+// dependent loads -- 7 us alone on the GPU at the tail of every black pass (224^3).  Exact sums need no order, so one
+// atomic per block and quantity replaces the array and the tail is 2.5 us.
 // --------------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void fx_flush(long long (&acc)[NQ], float (&f)[NQ], float scale)
 {
