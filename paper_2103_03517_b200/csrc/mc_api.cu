@@ -363,6 +363,7 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     ctx->field = ham->B[0] != 0.0 || ham->B[1] != 0.0 || ham->B[2] != 0.0;
     ctx->masked = needs_mask(lat, ham);
     ctx->vec = (nx % 8 == 0) ? 4 : 1;
+    if (const char* env = getenv("MC_B200_VEC")) { if (atoi(env) == 1) ctx->vec = 1; }     // experiments
     ctx->geom.RV = R / ctx->vec; ctx->geom.n_items = Nc / ctx->vec;
     ctx->geom.div_rv = make_div(ctx->geom.RV); ctx->geom.div_ny = make_div((uint32_t)ny);
 

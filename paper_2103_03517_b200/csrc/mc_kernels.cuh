@@ -453,8 +453,11 @@ __device__ __forceinline__ ItemPos locate_linear(const Params& P, const PairGeom
     return q;
 }
 
+#ifndef MC_PAIR_MIN_BLOCKS
+#define MC_PAIR_MIN_BLOCKS 1
+#endif
 template <int VEC, int ANISO, bool MASKED>
-__global__ void __launch_bounds__(BLOCK)
+__global__ void __launch_bounds__(BLOCK, MC_PAIR_MIN_BLOCKS)
 pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G, int colour, float invT, int flags,
             float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
 {
