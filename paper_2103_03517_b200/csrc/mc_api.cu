@@ -365,7 +365,8 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     ctx->vec = (nx % 8 == 0) ? 4 : 1;
     if (const char* env = getenv("MC_B200_VEC")) { if (atoi(env) == 1) ctx->vec = 1; }     // experiments
     ctx->geom.RV = R / ctx->vec; ctx->geom.n_items = Nc / ctx->vec;
-    ctx->geom.div_rv = make_div(ctx->geom.RV); ctx->geom.div_ny = make_div((uint32_t)ny);
+    ctx->geom.div_rv = make_div(ctx->geom.RV); ctx->geom.div_nz = make_div((uint32_t)nz);
+    { uint32_t sh = 0; while (sh < 5 && ny % (2 << sh) == 0) ++sh; ctx->geom.yb_shift = sh; }      // up to 32 rows per block
 
     // pairing geometry (C-11); the constrained path needs an even colour population (C-15)
     ctx->pair_ok = (Nc % 2 == 0) && Nc >= 2;

@@ -63,7 +63,8 @@ struct Params {
 
 struct Geom {                        // per-VEC decomposition of the colour-linear index space into items of VEC sites
     uint32_t n_items, RV;            // RV = items per row
-    FastDiv div_rv, div_ny;
+    FastDiv div_rv, div_nz;
+    uint32_t yb_shift;               // rows are visited in blocks of 2^yb_shift rows, z fastest between blocks (see locate)
 };
 
 enum : int { F_FINALIZE = 1, F_TORQUE = 2, F_SAMPLE_TORQUE = 4 };
@@ -106,11 +107,18 @@ struct ItemPos {
 template <int VEC>
 __device__ __forceinline__ ItemPos locate(const Params& P, const Geom& G, uint32_t item, int colour)
 {
-    uint32_t row, xq, y, z;
-    G.div_rv.divmod(item, row, xq);
-    G.div_ny.divmod(row, z, y);
-    ItemPos q;
+    // Visiting order of the rows (which thread takes which site; the result does not depend on it): blocks of 2^yb_shift
+    // consecutive y-rows, all nz planes of a block before the next block.  The grid-stride window of a pass then holds a
+    // site's +-z neighbours together with it, so every other-colour value comes from HBM once; in plain (y, then z) order
+    // a thin film (c5: a z-plane is 25 MB per colour) re-read them up to three times.
+    uint32_t rowp, xq, t, yb, y, z;
+    G.div_rv.divmod(item, rowp, xq);
+    t = rowp >> G.yb_shift;
+    G.div_nz.divmod(t, yb, z);
+    y = (yb << G.yb_shift) + (rowp & ((1u << G.yb_shift) - 1u));
     const uint32_t R = (uint32_t)P.R, ny = (uint32_t)P.ny, nz = (uint32_t)P.nz;
+    const uint32_t row = y + ny * z;
+    ItemPos q;
     const uint32_t xh0 = xq * VEC;
     q.par = (y + z + (uint32_t)colour) & 1u;
     q.xh0 = xh0;
