@@ -337,6 +337,16 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return bail(MC_ECUDA, "no CUDA device");
     if (cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return bail(MC_ECUDA, "cannot query the device");
+    {   // mc_set_spins / mc_get_spins borrow stream-ordered scratch (cudaMallocAsync) and return it before they end; keep
+        // what they return cached in the device's default pool instead of handing it back to the driver at every
+        // synchronisation (the default threshold of 0 makes every upload pay a fresh 135 MB allocation at c3)
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            unsigned long long keep = ~0ull;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+        cudaGetLastError();
+    }
 
     const int nx = lat->nx, ny = lat->ny, nz = lat->nz;
     const uint32_t N = (uint32_t)nx * ny * nz, R = nx / 2, Nc = N / 2;
