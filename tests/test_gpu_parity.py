@@ -78,6 +78,8 @@ CASES = [
     ((8, 6, 5), 0.9, 1.0, dict(periodic=(1, 0, 0), Ku=0.05, Kc=0.1)),      # open faces, odd open dims, both anisotropies
     ((2, 1, 1), 1.0, 1.5, dict(periodic=(0, 0, 0))),                       # the dimer
     ((64, 64, 64), 0.1, 0.3, dict(Ku=0.01)),                               # c2 first T-point (low T, random state = worst case)
+    ((96, 40, 36), 1.2, 0.9, dict(Kc=0.2, Ku=0.1, eu=(0.5, 0.5, 0.7), B=(0.05, 0.1, -0.2))),   # tiled pass, run-time row length (R = 48), two slabs, ragged z-segments, every term
+    ((80, 30, 58), 0.6, 0.4, dict(Ku=0.05)),                               # tiled pass, one slab = all of y (halo wraps on both sides), R = 40
 ]
 
 
@@ -177,6 +179,28 @@ def test_observables_match_oracle(mods):
     tr = g.trace(); ob = g.observables()
     assert np.allclose(tr[-1, 2:5], list(ob.M), atol=1e-6) and abs(tr[-1, 5] - ob.E_total) < 2e-6
     assert ob.n_samples == 3 and abs(ob.sum_E - tr[:, 5].sum()) < 1e-12
+    g.close()
+
+
+def test_tiled_pass_fused_sums_match_a_fresh_measurement(mods):
+    """The tiled pass forms the on-site energies of the final spin from the dE terms (s4 identity, (S.e)^2 difference form)
+    and sums in 64-bit fixed point: its per-sweep M and E must equal a standalone measurement of the same state, and the
+    oracle's energy of that state."""
+    oracle, binding, inputs = mods
+    shape = (64, 64, 64)
+    kw = dict(J=0.9, Ku=0.3, eu=(0.2, 0.1, 0.9), Kc=0.4, B=(0.1, 0.2, -0.3))
+    g = binding.Lattice(*shape, seed=5, cone0=0.7, adaptive=True, **kw)
+    g.set_spins(inputs.random_unit_spins(g.N, 11))
+    g.sweep(0.8, 4)
+    tr = g.trace()
+    fused = g.observables()                                   # what the black pass left
+    g.set_spins(g.get_spins())                                # invalidates the fused sums: the next call measures afresh
+    fresh = g.observables()
+    o = oracle.Oracle(*shape, seed=5, **kw); o.set_spins(g.get_spins()); ref = o.observables()
+    for name in ("m", "E_total", "E_exch", "E_aniso", "E_zeeman"):
+        assert abs(getattr(fused, name) - getattr(fresh, name)) < 2e-6, name
+        assert abs(getattr(fresh, name) - getattr(ref, name)) < 2e-6, name
+    assert np.allclose(tr[-1, 2:5], list(fresh.M), atol=1e-6) and abs(tr[-1, 5] - fresh.E_total) < 2e-6
     g.close()
 
 
