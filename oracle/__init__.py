@@ -80,6 +80,7 @@ def lib():
     L.orc_trace.argtypes = [vp, i64, vp]; L.orc_trace.restype = i64
     L.orc_site_energy.argtypes = [vp, i64, vp]; L.orc_site_energy.restype = dbl
     L.orc_total_energy.argtypes = [vp]; L.orc_total_energy.restype = dbl
+    L.orc_profile_x.argtypes = [vp, vp]; L.orc_profile_x.restype = None
     _lib = L
     return L
 
@@ -137,6 +138,10 @@ class Oracle:
         u = [C.c_double(), C.c_double(), C.c_double()]
         self.L.orc_site_uniforms(self.h, int(x), int(y), int(z), int(colour), int(sweep), C.byref(u[0]), C.byref(u[1]), C.byref(u[2]))
         return tuple(v.value for v in u)
+
+    def profile_x(self):
+        """[nx, 3] slice-averaged magnetisation along x (Fig. 2)."""
+        out = np.zeros((self.shape[0], 3)); self.L.orc_profile_x(self.h, _p(out)); return out
 
     # ---- state
     def set_spins(self, xyz):

@@ -104,16 +104,20 @@ void orc_cone_move(const double S[3], double theta, double u0, double u1, double
 /* ------------------------------------------------------------------ lattice helpers */
 static inline int64_t site_index(const orc_ctx* c, int x, int y, int z) { return x + (int64_t)c->nx * (y + (int64_t)c->ny * z); }
 
-/* neighbour of (x,y,z) in direction k = (+x,-x,+y,-y,+z,-z); -1 if there is no bond (open face or masked). */
-static int64_t neighbour(const orc_ctx* c, int x, int y, int z, int k)
+/* neighbour of (x,y,z) in direction k = (+x,-x,+y,-y,+z,-z); -1 if there is no bond (open face or masked).
+ * *sign = -1 when the bond crosses an ANTI-periodic wrap (periodic[axis] == 2): the spin on the other side enters
+ * Eq. (2) as -S_j, which is how a domain wall is held in the box ("anti-periodic along x direction"). */
+static int64_t neighbour(const orc_ctx* c, int x, int y, int z, int k, double* sign)
 {
     int p[3] = { x, y, z }, dim[3] = { c->nx, c->ny, c->nz };
     int axis = k >> 1, step = (k & 1) ? -1 : +1;
     int64_t self = site_index(c, x, y, z);
+    *sign = 1.0;
     if (c->mask && !((c->mask[self] >> k) & 1)) return -1;
     p[axis] += step;
     if (p[axis] < 0 || p[axis] >= dim[axis]) {
         if (!c->periodic[axis]) return -1;
+        if (c->periodic[axis] == 2) *sign = -1.0;
         p[axis] = (p[axis] + dim[axis]) % dim[axis];
     }
     return site_index(c, p[0], p[1], p[2]);
@@ -124,9 +128,10 @@ static void exchange_field(const orc_ctx* c, int x, int y, int z, double h[3])
 {
     h[0] = h[1] = h[2] = 0.0;
     for (int k = 0; k < 6; ++k) {
-        int64_t j = neighbour(c, x, y, z, k);
+        double sg;
+        int64_t j = neighbour(c, x, y, z, k, &sg);
         if (j < 0) continue;
-        for (int a = 0; a < 3; ++a) h[a] += c->J * c->S[3 * j + a];
+        for (int a = 0; a < 3; ++a) h[a] += sg * c->J * c->S[3 * j + a];
     }
 }
 
@@ -164,10 +169,11 @@ double orc_total_energy(const orc_ctx* c)
         int64_t i = site_index(c, x, y, z);
         const double* S = &c->S[3 * i];
         for (int k = 0; k < 6; k += 2) {          /* +x, +y, +z only */
-            int64_t j = neighbour(c, x, y, z, k);
+            double sg;
+            int64_t j = neighbour(c, x, y, z, k, &sg);
             if (j < 0) continue;
             const double* Sj = &c->S[3 * j];
-            E -= c->J * (S[0] * Sj[0] + S[1] * Sj[1] + S[2] * Sj[2]);
+            E -= sg * c->J * (S[0] * Sj[0] + S[1] * Sj[1] + S[2] * Sj[2]);
         }
         const double* e = easy_axis(c, i);
         double se = S[0] * e[0] + S[1] * e[1] + S[2] * e[2];
@@ -188,6 +194,7 @@ orc_ctx* orc_create(int nx, int ny, int nz, const int periodic[3],
     if (nx < 1 || ny < 1 || nz < 1) return NULL;
     int dim[3] = { nx, ny, nz };
     for (int a = 0; a < 3; ++a) if (periodic[a] && (dim[a] & 1)) return NULL;   /* two-colouring needs even periodic dims */
+    for (int a = 0; a < 3; ++a) if (periodic[a] < 0 || periodic[a] > 2) return NULL;   /* 0 open, 1 periodic, 2 anti-periodic */
     orc_ctx* c = (orc_ctx*)calloc(1, sizeof(orc_ctx));
     c->nx = nx; c->ny = ny; c->nz = nz;
     for (int a = 0; a < 3; ++a) c->periodic[a] = periodic[a];
@@ -277,6 +284,21 @@ int64_t orc_half_sweep(orc_ctx* c, double T, int colour, double* xdec, uint8_t* 
         count += a;                                           /* P:160 */
     }
     return count;
+}
+
+/* ------------------------------------------------------------------ domain-wall profile (P:66, Fig. 2)
+ * "the normalized magnetization z component is obtained for each profile point by averaging over the respective
+ * cross-section slice": out[3*x + a] = mean over (y,z) of S_a at that x. */
+void orc_profile_x(const orc_ctx* c, double* out)
+{
+    for (int x = 0; x < c->nx; ++x) {
+        double s[3] = { 0, 0, 0 };
+        for (int z = 0; z < c->nz; ++z) for (int y = 0; y < c->ny; ++y) {
+            const double* S = &c->S[3 * site_index(c, x, y, z)];
+            s[0] += S[0]; s[1] += S[1]; s[2] += S[2];
+        }
+        for (int a = 0; a < 3; ++a) out[3 * x + a] = s[a] / ((double)c->ny * c->nz);
+    }
 }
 
 /* ------------------------------------------------------------------ observables (Eq. 6 P:94; P:52; P:54) */

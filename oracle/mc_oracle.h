@@ -55,6 +55,9 @@ orc_ctx* orc_create(int nx, int ny, int nz, const int periodic[3],
                     const double* region_axis, int n_regions,
                     double cone0_rad, int adaptive, uint64_t seed);
 void orc_destroy(orc_ctx*);
+/* periodic[a]: 0 open faces, 1 periodic, 2 anti-periodic (the spin across the wrap enters as -S_j). */
+/* Slice-averaged magnetisation along x: out[3*x + a], a = x,y,z component. */
+void orc_profile_x(const orc_ctx*, double* out);
 
 void orc_set_spins(orc_ctx*, const double* xyz /* [N][3] lexicographic */);
 void orc_set_spins_f32(orc_ctx*, const float* xyz);

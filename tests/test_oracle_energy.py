@@ -21,6 +21,9 @@ CASES = [
     dict(shape=(6, 5, 3), periodic=(1, 0, 0)),          # odd open dims
     dict(shape=(8, 4, 4), periodic=(1, 1, 0), masked=True),
     dict(shape=(2, 1, 1), periodic=(0, 0, 0)),          # the dimer
+    dict(shape=(6, 4, 4), periodic=(2, 1, 1)),          # anti-periodic along x (domain-wall box)
+    dict(shape=(2, 2, 2), periodic=(2, 1, 1)),          # L = 2 with an anti-periodic wrap: the two x-bonds cancel
+    dict(shape=(8, 4, 4), periodic=(2, 1, 0), masked=True),
 ]
 
 
