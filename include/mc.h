@@ -37,7 +37,9 @@ extern "C" {
 typedef struct mc_ctx mc_ctx;      /* opaque handle (host memory, freed by mc_destroy) */
 
 /* Simple-cubic lattice, nearest neighbours.  nx must be even (colour-split rows); every periodic
- * dimension must be even (two-colourability); N = nx*ny*nz < 2^31.  periodic[a] = 1: wrap; 0: open faces. */
+ * dimension must be even (two-colourability); N = nx*ny*nz < 2^31.  periodic[a] = 1: wrap; 0: open faces;
+ * periodic[0] = 2: ANTI-periodic along x, the spin across the wrap enters Eq. (2) as -S_j, which holds a domain wall in
+ * the box ("anti-periodic along x direction"; x only: 2 on another axis is MC_EINVAL). */
 typedef struct {
     int32_t nx, ny, nz;
     int32_t periodic[3];
@@ -130,6 +132,12 @@ int mc_reset_accumulators(mc_ctx* ctx);                      /* asynchronous */
  * rows[k][6] = acceptance, cone used, Mx, My, Mz (per site), E_total (per site).  Synchronous. */
 #define MC_TRACE_CAPACITY 16384
 int mc_trace(mc_ctx* ctx, int64_t max_rows, double* host_rows, int64_t* n_rows);
+
+/* Domain-wall profile (Fig. 2: "the normalized magnetization z component is obtained for each profile point by
+ * averaging over the respective cross-section slice"): host_profile[3*x + a] = mean over (y,z) of component a of the spins
+ * at that x, x = 0..nx-1 (HOST pointer to 3*nx doubles, caller-owned).  Exact fixed-point sums on the device, so the
+ * result is reproducible.  Borrows 24*nx bytes of stream-ordered scratch; synchronous. */
+int mc_profile_x(mc_ctx* ctx, double* host_profile);
 
 /* Number of kernel launches this handle has enqueued since creation (bench.py's gpu_launches). */
 int64_t mc_launch_count(const mc_ctx* ctx);

@@ -21,7 +21,7 @@ MC_TRACE_CAPACITY = 16384
 SYMBOLS = [
     "mc_workspace_bytes", "mc_create", "mc_destroy", "mc_init_spins", "mc_set_spins", "mc_get_spins", "mc_set_cone",
     "mc_set_sweep", "mc_sweep", "mc_constrained_sweep", "mc_half_sweep", "mc_constrained_half_sweep", "mc_end_sweep",
-    "mc_align_to", "mc_observables", "mc_reset_accumulators", "mc_trace", "mc_launch_count", "mc_last_error", "mc_version",
+    "mc_align_to", "mc_observables", "mc_reset_accumulators", "mc_trace", "mc_profile_x", "mc_launch_count", "mc_last_error", "mc_version",
 ]
 
 
@@ -84,6 +84,7 @@ def load():
     L.mc_observables.argtypes = [vp, vp]; L.mc_observables.restype = i32
     L.mc_reset_accumulators.argtypes = [vp]; L.mc_reset_accumulators.restype = i32
     L.mc_trace.argtypes = [vp, i64, vp, vp]; L.mc_trace.restype = i32
+    L.mc_profile_x.argtypes = [vp, vp]; L.mc_profile_x.restype = i32
     L.mc_launch_count.argtypes = [vp]; L.mc_launch_count.restype = i64
     L.mc_last_error.argtypes = [vp]; L.mc_last_error.restype = C.c_char_p
     L.mc_version.argtypes = []; L.mc_version.restype = C.c_char_p
@@ -98,7 +99,7 @@ def _p(a):
 def make_structs(shape, periodic=(1, 1, 1), J=1.0, Ku=0.0, eu=(0, 0, 1), Kc=0.0, B=(0, 0, 0),
                  bond_mask=None, region=None, region_axis=None, cone0=0.5, adaptive=True):
     """Fills mc_lattice / mc_hamiltonian; returns them plus the arrays that must stay alive during mc_create."""
-    lat = McLattice(int(shape[0]), int(shape[1]), int(shape[2]), (C.c_int32 * 3)(*[int(bool(p)) for p in periodic]))
+    lat = McLattice(int(shape[0]), int(shape[1]), int(shape[2]), (C.c_int32 * 3)(*[int(p) for p in periodic]))   # 0 open, 1 periodic, 2 anti-periodic (x)
     keep = []
     def arr(a, dt):
         if a is None:
@@ -200,6 +201,10 @@ class Lattice:
         o = McObs(); self._chk(self.L.mc_observables(self.h, C.byref(o))); return o
 
     def reset_accumulators(self): self._chk(self.L.mc_reset_accumulators(self.h))
+
+    def profile_x(self):
+        """[nx, 3] slice-averaged magnetisation along x (mc_profile_x; Fig. 2)."""
+        out = np.empty((self.shape[0], 3)); self._chk(self.L.mc_profile_x(self.h, _p(out))); return out
 
     def trace(self, max_rows=MC_TRACE_CAPACITY):
         rows = np.empty((int(max_rows), 6)); k = C.c_int64(0)

@@ -38,6 +38,7 @@ bool valid_lattice(const mc_lattice* lat)
     for (int a = 0; a < 3; ++a) {
         if (dim[a] < 1) return false;
         if (lat->periodic[a] && (dim[a] & 1)) return false;
+        if (lat->periodic[a] < 0 || lat->periodic[a] > (a == 0 ? 2 : 1)) return false;     // anti-periodic (2) along x only
     }
     if (lat->nx & 1) return false;
     const double N = (double)lat->nx * lat->ny * lat->nz;
@@ -166,7 +167,7 @@ bool plan_tile(mc_ctx* c)
     c->tile_ok = false;
     const mc_lattice& lat = c->lat;
     if (c->masked || c->P.region) return false;
-    if (!(lat.periodic[0] && lat.periodic[1] && lat.periodic[2])) return false;
+    if (!(lat.periodic[0] == 1 && lat.periodic[1] == 1 && lat.periodic[2] == 1)) return false;   // anti-periodic x: generic pass
     const int R = lat.nx / 2;
     if (R % 4) return false;                                    // TMA bulk copies move whole rows: 16-byte multiples
     const int PR = R / 2;
@@ -353,6 +354,7 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     char* ws = (char*)dev_workspace;
     Params& P = ctx->P;
     P.nx = nx; P.ny = ny; P.nz = nz; P.R = (int)R; P.Nc = Nc; P.N = N; P.invN = 1.0 / (double)N;
+    P.anti_x = lat->periodic[0] == 2 ? 1 : 0;
     P.plane = L.plane; P.S = (float*)(ws + L.spins);
     P.mask = nullptr; P.mask_plane = L.mask_plane; P.region = nullptr; P.region_plane = L.region_plane; P.axis = nullptr;
     P.J = (float)ham->J; P.Ku = (float)ham->Ku; P.Kc = (float)ham->Kc;
@@ -705,6 +707,29 @@ int mc_observables(mc_ctx* ctx, mc_obs* out)
     for (int a = 0; a < 4; ++a) { out->sum_m[a] = st.sum_m[a]; out->sum_m2[a] = st.sum_m2[a]; }
     out->sum_E = st.sum_E; out->sum_E2 = st.sum_E2;
     for (int a = 0; a < 3; ++a) out->sum_torque[a] = st.sum_torque[a];
+    return MC_OK;
+}
+
+int mc_profile_x(mc_ctx* ctx, double* host_profile)
+{
+    CHECK_CTX();
+    if (!host_profile) return fail(ctx, MC_EINVAL, "mc_profile_x: null pointer");
+    const int nx = ctx->P.nx;
+    const size_t bytes = (size_t)nx * 3 * sizeof(long long);
+    long long* tmp = nullptr;
+    CU(cudaMallocAsync((void**)&tmp, bytes, ctx->stream));        // stream-ordered scratch, returned before the call ends
+    CU(cudaMemsetAsync(tmp, 0, bytes, ctx->stream));
+    const uint32_t rows = (uint32_t)ctx->P.ny * (uint32_t)ctx->P.nz;
+    const uint32_t n_threads = (uint32_t)ctx->P.R * ((rows + PROFILE_ROWS - 1) / PROFILE_ROWS);
+    profile_x_kernel<<<(n_threads + BLOCK - 1) / BLOCK, BLOCK, 0, ctx->stream>>>(ctx->P, tmp);
+    ctx->launches += 1;
+    CU(cudaGetLastError());
+    std::vector<long long> sums((size_t)nx * 3);
+    CU(cudaMemcpyAsync(sums.data(), tmp, bytes, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaFreeAsync(tmp, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    const double scale = ctx->P.fx_inv / ((double)ctx->P.ny * (double)ctx->P.nz);
+    for (size_t i = 0; i < sums.size(); ++i) host_profile[i] = (double)sums[i] * scale;
     return MC_OK;
 }
 

@@ -42,6 +42,7 @@ struct DevState {
 
 struct Params {
     int nx, ny, nz, R;               // R = nx/2 sites of one colour per row
+    int anti_x;                      // 1: anti-periodic boundary along x (domain-wall box); the wrap bond sees -S_j
     uint32_t Nc;                     // sites per colour
     uint32_t N;
     double invN;                     // 1 / N (host-computed: keeps an fp64 division off the finalising thread)
@@ -102,6 +103,7 @@ struct ItemPos {
     uint32_t o_yp, o_ym, o_zp, o_zm;   // colour-linear index of the same column in the 4 neighbouring rows
     uint32_t o_x;       // colour-linear index of the one extra x-neighbour outside the item's own column range
     uint32_t xh0;       // in-row colour index of the first site (x = 2 xh0 + par)
+    float xs;           // -1 if the bond to the extra x-neighbour crosses an anti-periodic x wrap, else +1
 };
 
 template <int VEC>
@@ -128,8 +130,10 @@ __device__ __forceinline__ ItemPos locate(const Params& P, const Geom& G, uint32
     const uint32_t zp = (z + 1 == nz) ? 0u : z + 1, zm = (z == 0) ? nz - 1 : z - 1;
     q.o_yp = (z * ny + yp) * R + xh0;  q.o_ym = (z * ny + ym) * R + xh0;
     q.o_zp = (zp * ny + y) * R + xh0;  q.o_zm = (zm * ny + y) * R + xh0;
-    const uint32_t xe = q.par ? ((xh0 + VEC == R) ? 0u : xh0 + VEC) : ((xh0 == 0) ? R - 1 : xh0 - 1);
+    const bool wraps = q.par ? (xh0 + VEC == R) : (xh0 == 0);      // only the item's outermost x-bond can cross the wrap
+    const uint32_t xe = q.par ? (wraps ? 0u : xh0 + VEC) : (wraps ? R - 1 : xh0 - 1);
     q.o_x = row * R + xe;
+    q.xs = (wraps && P.anti_x) ? -1.0f : 1.0f;
     return q;
 }
 
@@ -158,7 +162,7 @@ __device__ __forceinline__ void exchange_field(const Params& P, const ItemPos& q
         const Pack<VEC> o  = ld_nc<VEC>(Oc + q.a0);
         const Pack<VEC> yp = ld_nc<VEC>(Oc + q.o_yp), ym = ld_nc<VEC>(Oc + q.o_ym);
         const Pack<VEC> zp = ld_nc<VEC>(Oc + q.o_zp), zm = ld_nc<VEC>(Oc + q.o_zm);
-        const float ex = __ldg(Oc + q.o_x);
+        const float ex = q.xs * __ldg(Oc + q.o_x);               // the spin across an anti-periodic wrap enters as -S_j
 #pragma unroll
         for (int k = 0; k < VEC; ++k) {
             // the second x-neighbour: next column if par = 1, previous column if par = 0
@@ -459,8 +463,10 @@ __device__ __forceinline__ ItemPos locate_linear(const Params& P, const PairGeom
     const uint32_t zp = (z + 1 == nz) ? 0u : z + 1, zm = (z == 0) ? nz - 1 : z - 1;
     q.o_yp = (z * ny + yp) * R + xh0;  q.o_ym = (z * ny + ym) * R + xh0;
     q.o_zp = (zp * ny + y) * R + xh0;  q.o_zm = (zm * ny + y) * R + xh0;
-    const uint32_t xe = q.par ? ((xh0 + VEC == R) ? 0u : xh0 + VEC) : ((xh0 == 0) ? R - 1 : xh0 - 1);
+    const bool wraps = q.par ? (xh0 + VEC == R) : (xh0 == 0);      // only the item's outermost x-bond can cross the wrap
+    const uint32_t xe = q.par ? (wraps ? 0u : xh0 + VEC) : (wraps ? R - 1 : xh0 - 1);
     q.o_x = row * R + xe;
+    q.xs = (wraps && P.anti_x) ? -1.0f : 1.0f;
     return q;
 }
 
@@ -619,6 +625,38 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
     if (flags & F_FINALIZE) {
         if (last_block_done(st)) final_reduce(P, 0, flags);
     }
+}
+
+// --------------------------------------------------------------------------------------------------------------
+// Slice profile along x (Fig. 2): sum over (y, z) of the three spin components at every x, in exact fixed point.
+// One thread = one colour column xh of a chunk of PROFILE_ROWS rows (coalesced along xh); a colour-c site of row (y,z)
+// sits at x = 2 xh + ((y + z + c) & 1), so the thread feeds two x positions.  out[3 x + a] (int64, unit P.fx_inv).
+// --------------------------------------------------------------------------------------------------------------
+constexpr int PROFILE_ROWS = 32;
+__global__ void __launch_bounds__(BLOCK) profile_x_kernel(const __grid_constant__ Params P, long long* __restrict__ out)
+{
+    const uint32_t R = (uint32_t)P.R, rows = (uint32_t)P.ny * (uint32_t)P.nz;
+    const uint32_t n_chunks = (rows + PROFILE_ROWS - 1) / PROFILE_ROWS;
+    const uint32_t t = blockIdx.x * BLOCK + threadIdx.x;
+    if (t >= R * n_chunks) return;
+    const uint32_t chunk = t / R, xh = t - chunk * R;
+    float acc[2][3] = { { 0.f, 0.f, 0.f }, { 0.f, 0.f, 0.f } };
+    const uint32_t r1 = min(rows, (chunk + 1) * PROFILE_ROWS);
+    for (uint32_t row = chunk * PROFILE_ROWS; row < r1; ++row) {
+        const uint32_t y = row % (uint32_t)P.ny, z = row / (uint32_t)P.ny;
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            const uint32_t p = (y + z + (uint32_t)c) & 1u;
+            const float* S = P.S + (long long)c * 3 * P.plane + (long long)row * R + xh;
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { const float v = S[(long long)a * P.plane]; acc[0][a] += p ? 0.f : v; acc[1][a] += p ? v : 0.f; }
+        }
+    }
+#pragma unroll
+    for (int p = 0; p < 2; ++p)
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+            atomicAdd(reinterpret_cast<unsigned long long*>(out + 3 * (2 * xh + p) + a), (unsigned long long)__float2ll_rn(acc[p][a] * P.fx_scale));
 }
 
 // --------------------------------------------------------------------------------------------------------------

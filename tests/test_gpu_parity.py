@@ -78,6 +78,9 @@ CASES = [
     ((8, 6, 5), 0.9, 1.0, dict(periodic=(1, 0, 0), Ku=0.05, Kc=0.1)),      # open faces, odd open dims, both anisotropies
     ((2, 1, 1), 1.0, 1.5, dict(periodic=(0, 0, 0))),                       # the dimer
     ((64, 64, 64), 0.1, 0.3, dict(Ku=0.01)),                               # c2 first T-point (low T, random state = worst case)
+    ((24, 8, 6), 0.8, 0.7, dict(periodic=(2, 1, 1), Ku=0.1)),              # anti-periodic x (domain-wall box), VEC=4
+    ((6, 4, 4), 1.1, 1.0, dict(periodic=(2, 1, 0), Kc=0.2)),               # anti-periodic x, VEC=1 path, open z
+    ((2, 2, 2), 2.0, 2.5, dict(periodic=(2, 1, 1), Ku=0.1)),               # L = 2 with an anti-periodic wrap: the x-bonds cancel
     ((96, 40, 36), 1.2, 0.9, dict(Kc=0.2, Ku=0.1, eu=(0.5, 0.5, 0.7), B=(0.05, 0.1, -0.2))),   # tiled pass, run-time row length (R = 48), two slabs, ragged z-segments, every term
     ((80, 30, 58), 0.6, 0.4, dict(Ku=0.05)),                               # tiled pass, one slab = all of y (halo wraps on both sides), R = 40
 ]
@@ -204,6 +207,35 @@ def test_tiled_pass_fused_sums_match_a_fresh_measurement(mods):
     g.close()
 
 
+def test_domain_wall_box_profile_and_energy_match_oracle(mods):
+    """anti-periodic x + slice profile.  A tanh wall (Eq. 5) with thermal scatter: mc_profile_x against the
+    oracle's slice average, the exchange energy (wrap bonds counted with -S_j) against the oracle's, then whole sweeps
+    keep the wall in the box (m_z changes sign once along x and the total M_z stays near 0)."""
+    oracle, binding, inputs = mods
+    shape = (48, 16, 12)
+    kw = dict(periodic=(2, 1, 1), J=1.0, Ku=0.05)
+    o, g = _pair(mods, shape, **kw)
+    nx, ny, nz = shape
+    x = np.arange(nx * ny * nz) % nx
+    rng = np.random.default_rng(4)
+    S = np.zeros((nx * ny * nz, 3)); S[:, 2] = np.tanh(-(x - 23.5) / np.sqrt(1.0 / (2 * 0.05))); S[:, 1] = np.sqrt(1 - S[:, 2] ** 2)
+    S += 0.15 * rng.standard_normal(S.shape); S /= np.linalg.norm(S, axis=1, keepdims=True)
+    g.set_spins(S.astype(np.float32)); o.set_spins(g.get_spins())
+    pg, po = g.profile_x(), o.profile_x()
+    assert pg.shape == (nx, 3) and np.abs(pg - po).max() < 1e-6
+    a, b = g.observables(), o.observables()
+    for name in ("E_total", "E_exch", "E_aniso", "m"):
+        assert abs(getattr(a, name) - getattr(b, name)) < 2e-6, name
+    assert (g.profile_x() == pg).all()                       # exact fixed-point sums: bitwise reproducible
+    for colour in (0, 1):
+        _check_half_sweep(o, g, 0.5, colour, shape)
+    g2 = binding.Lattice(*shape, seed=9, cone0=0.4, adaptive=True, **kw)
+    g2.set_spins(g.get_spins()); g2.sweep(0.4, 300)
+    mz = g2.profile_x()[:, 2]
+    assert mz[:8].mean() > 0.8 and mz[-8:].mean() < -0.8 and (np.diff(np.sign(mz)) != 0).sum() == 1
+    g.close(); g2.close()
+
+
 def test_set_get_roundtrip_and_init(mods):
     oracle, binding, inputs = mods
     g = binding.Lattice(8, 6, 4, periodic=(1, 1, 1))
@@ -227,6 +259,7 @@ def test_error_paths(mods):
     with pytest.raises(binding.McError): bad.constrained_sweep(1.0, 0.0, 0.0, 1)
     m = inputs.boundary_mask(8, 4, 4, (1, 1, 1)); m[0] &= 0xFE            # asymmetric mask
     with pytest.raises(binding.McError): binding.Lattice(8, 4, 4, bond_mask=m)
+    with pytest.raises(binding.McError): binding.Lattice(8, 4, 4, periodic=(1, 2, 1))     # anti-periodic along x only
     g.close(); bad.close()
 
 
@@ -237,6 +270,7 @@ CCASES = [
     ((12, 4, 2), 0.9, 0.9, dict(Ku=0.1)),               # VEC=1, B=8
     ((6, 6, 2), 0.9, 0.9, dict()),                      # VEC=1, B=2
     ((32, 16, 8), 0.3, 0.3, dict(Ku=0.05)),             # lower T
+    ((16, 8, 8), 0.7, 0.6, dict(periodic=(2, 1, 1), Ku=0.1)),              # pair pass in the domain-wall box (anti-periodic x)
 ]
 
 
