@@ -184,6 +184,11 @@ bool plan_tile(mc_ctx* c)
     const size_t smem_cap = (size_t)(220 * 1024) / TILE_MIN_BLOCKS - 3 * 1024;   // TILE_MIN_BLOCKS CTAs per SM
     auto slot_bytes = [&](int ty) { return (size_t)3 * (ty + 2) * R * sizeof(float); };
     if (lat.ny % (2 * RP) == 0 && TILE_NSLOT * slot_bytes(2 * RP) <= smem_cap) NP = 2;
+    // row lengths with a compile-time specialisation (R = 32, 64, 112) take its slab shape when it fits: 64^3 13.3 -> 11.3 us per sweep
+    if ((R == 32 || R == 64 || R == 112) && lat.ny % TILE_TY_RT == 0 && PR * (TILE_TY_RT / TILE_NPASS_RT) <= max_threads) {
+        RP = TILE_TY_RT / TILE_NPASS_RT; NP = TILE_NPASS_RT;
+    }
+    if (want_rp > 0 && lat.ny % want_rp == 0 && PR * want_rp <= TILE_MAX_THREADS) { RP = want_rp; NP = 1; if (lat.ny % (2 * RP) == 0 && TILE_NSLOT * slot_bytes(2 * RP) <= smem_cap) NP = 2; }
     if (want_np > 0 && lat.ny % (want_np * RP) == 0) NP = want_np;
     G.RP = RP; G.NPASS = NP; G.Ty = RP * NP;
     G.n_slabs = lat.ny / G.Ty;
