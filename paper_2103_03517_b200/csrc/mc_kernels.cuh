@@ -404,7 +404,7 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
             if (colour == 1) f[3] -= dot3(S, hJ);
             if (ANISO) f[4] += aniso_energy<ANISO>(S, P.Ku, e[(ANISO & 1) ? k : 0], P.Kc);
             f[5] -= dot3(S, B);
-            if (flags & F_TORQUE) {
+            if (MODE == MODE_MEASURE && (flags & F_TORQUE)) {        // the unconstrained sweep never samples the torque
                 const Vec3 t = onsite_torque<ANISO>(S, P.Ku, e[(ANISO & 1) ? k : 0], P.Kc, B);
                 f[6] += t.x; f[7] += t.y; f[8] += t.z;
             }
