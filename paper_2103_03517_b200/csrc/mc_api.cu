@@ -136,20 +136,21 @@ template <int VEC> PairFn pick_pair(int aniso, bool masked)
 }
 
 typedef void (*TileFn)(const Params, const TileGeom, int, float, int, float*, uint8_t*);
-template <int RT, bool DEBUG> TileFn pick_tile_rt(int aniso, bool field)
+template <int RT, bool DEBUG, bool ANTI = false> TileFn pick_tile_rt(int aniso, bool field)
 {
     switch (aniso * 2 + (field ? 1 : 0)) {
-        case 0: return tile_pass_kernel<0, false, RT, DEBUG>;  case 1: return tile_pass_kernel<0, true, RT, DEBUG>;
-        case 2: return tile_pass_kernel<1, false, RT, DEBUG>;  case 3: return tile_pass_kernel<1, true, RT, DEBUG>;
-        case 4: return tile_pass_kernel<2, false, RT, DEBUG>;  case 5: return tile_pass_kernel<2, true, RT, DEBUG>;
-        case 6: return tile_pass_kernel<3, false, RT, DEBUG>;  default: return tile_pass_kernel<3, true, RT, DEBUG>;
+        case 0: return tile_pass_kernel<0, false, RT, DEBUG, ANTI>;  case 1: return tile_pass_kernel<0, true, RT, DEBUG, ANTI>;
+        case 2: return tile_pass_kernel<1, false, RT, DEBUG, ANTI>;  case 3: return tile_pass_kernel<1, true, RT, DEBUG, ANTI>;
+        case 4: return tile_pass_kernel<2, false, RT, DEBUG, ANTI>;  case 5: return tile_pass_kernel<2, true, RT, DEBUG, ANTI>;
+        case 6: return tile_pass_kernel<3, false, RT, DEBUG, ANTI>;  default: return tile_pass_kernel<3, true, RT, DEBUG, ANTI>;
     }
 }
 // Row lengths with a specialised instantiation (every shared-memory offset an immediate): R = nx/2 of BASELINE's
 // periodic configs c2 (64^3), c4 (128^3) and c3 (224^3).  Any other R runs the run-time-R instantiation.
 // The decision-variable debug outputs of the test hooks exist only in the run-time-R instantiation (same arithmetic).
-TileFn pick_tile(int R, int Ty, int npass, bool debug, int aniso, bool field)
+TileFn pick_tile(int R, int Ty, int npass, bool debug, int aniso, bool field, bool anti)
 {
+    if (anti) return debug ? pick_tile_rt<0, true, true>(aniso, field) : pick_tile_rt<0, false, true>(aniso, field);
     if (debug) return pick_tile_rt<0, true>(aniso, field);
     if (getenv("MC_B200_NO_RT") || Ty != TILE_TY_RT || npass != TILE_NPASS_RT) return pick_tile_rt<0, false>(aniso, field);
     switch (R) {
@@ -167,7 +168,7 @@ bool plan_tile(mc_ctx* c)
     c->tile_ok = false;
     const mc_lattice& lat = c->lat;
     if (c->masked || c->P.region) return false;
-    if (!(lat.periodic[0] == 1 && lat.periodic[1] == 1 && lat.periodic[2] == 1)) return false;   // anti-periodic x: generic pass
+    if (!(lat.periodic[0] >= 1 && lat.periodic[1] == 1 && lat.periodic[2] == 1)) return false;   // x may be anti-periodic (ANTI instantiation)
     const int R = lat.nx / 2;
     if (R % 4) return false;                                    // TMA bulk copies move whole rows: 16-byte multiples
     const int PR = R / 2;
@@ -198,7 +199,7 @@ bool plan_tile(mc_ctx* c)
     c->tile_smem = TILE_NSLOT * slot_bytes(G.Ty);
     if (c->tile_smem > 200 * 1024) return false;
     // every instantiation this handle can launch must be allowed its dynamic shared memory
-    TileFn fns[2] = { pick_tile(R, G.Ty, G.NPASS, false, c->aniso, c->field), pick_tile(R, G.Ty, G.NPASS, true, c->aniso, c->field) };
+    TileFn fns[2] = { pick_tile(R, G.Ty, G.NPASS, false, c->aniso, c->field, c->P.anti_x != 0), pick_tile(R, G.Ty, G.NPASS, true, c->aniso, c->field, c->P.anti_x != 0) };
     int per_sm = 1;
     for (TileFn f : fns) {
         if (cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tile_smem) != cudaSuccess) { cudaGetLastError(); return false; }
@@ -250,7 +251,7 @@ cudaError_t launch_dependent(Fn fn, int grid, int block, size_t smem, cudaStream
 int launch_pass(mc_ctx* ctx, int mode, int colour, float invT, int flags, float* dx, uint8_t* da)
 {
     if (mode == MODE_SWEEP && ctx->tile_ok) {
-        TileFn fn = pick_tile(ctx->tgeom.R, ctx->tgeom.Ty, ctx->tgeom.NPASS, dx || da, ctx->aniso, ctx->field);
+        TileFn fn = pick_tile(ctx->tgeom.R, ctx->tgeom.Ty, ctx->tgeom.NPASS, dx || da, ctx->aniso, ctx->field, ctx->P.anti_x != 0);
         const int grid = ctx->tgeom.n_slabs * ctx->tgeom.n_segs;
         CU(launch_dependent(fn, grid, ctx->tile_threads, ctx->tile_smem, ctx->stream, ctx->P, ctx->tgeom, colour, invT, flags, dx, da));
         ctx->launches += 1;

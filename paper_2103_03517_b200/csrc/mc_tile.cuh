@@ -116,7 +116,9 @@ __device__ __forceinline__ float xor_sign(float a, float s) { return __uint_as_f
 // On-site energies of the FINAL spin reuse what dE needs: cubic through s4 = sum_a S_a^4 (on the unit sphere
 // Sx^2Sy^2 + Sx^2Sz^2 + Sy^2Sz^2 = (1 - s4)/2, so dE_c = -Kc/2 (s4' - s4) and E_c = Kc/2 (1 - s4)), uniaxial through
 // (S.e)^2 and its difference form.
-template <int ANISO, bool FIELD, int RT, bool DEBUG>
+// ANTI: anti-periodic boundary along x (domain-wall box; C-27): the one x-neighbour a pair reads across the row
+// end enters with the opposite sign.  Instantiated for the run-time row length only.
+template <int ANISO, bool FIELD, int RT, bool DEBUG, bool ANTI = false>
 __global__ void __launch_bounds__(TILE_MAX_THREADS, TILE_MIN_BLOCKS)
 tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileGeom G, int colour, float invT, int flags,
                   float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
@@ -164,6 +166,7 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
     const int r0 = tid / PR, cp = tid - r0 * PR;
     const int exL = (cp == 0) ? R - 1 : 2 * cp - 1;
     const int exR = (cp == PR - 1) ? 0 : 2 * cp + 2;
+    const float sgL = (ANTI && cp == 0) ? -1.0f : 1.0f, sgR = (ANTI && cp == PR - 1) ? -1.0f : 1.0f;   // wrap-bond signs
     const int soff0 = (r0 + 1) * R + 2 * cp;
     const int exo0 = (r0 + 1) * R;
     const int pstride = RP * R;
@@ -214,7 +217,7 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
                     const f2 o  = *reinterpret_cast<const f2*>(pC + c * CS);
-                    const float ex = pE[c * CS];
+                    const float ex = ANTI ? pE[c * CS] * (par ? sgR : sgL) : pE[c * CS];
                     const f2 yp = *reinterpret_cast<const f2*>(pC + c * CS + R);
                     const f2 ym = *reinterpret_cast<const f2*>(pC + c * CS - R);
                     const f2 zp = *reinterpret_cast<const f2*>(pP + c * CS);

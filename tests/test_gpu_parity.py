@@ -82,6 +82,7 @@ CASES = [
     ((6, 4, 4), 1.1, 1.0, dict(periodic=(2, 1, 0), Kc=0.2)),               # anti-periodic x, VEC=1 path, open z
     ((2, 2, 2), 2.0, 2.5, dict(periodic=(2, 1, 1), Ku=0.1)),               # L = 2 with an anti-periodic wrap: the x-bonds cancel
     ((96, 40, 36), 1.2, 0.9, dict(Kc=0.2, Ku=0.1, eu=(0.5, 0.5, 0.7), B=(0.05, 0.1, -0.2))),   # tiled pass, run-time row length (R = 48), two slabs, ragged z-segments, every term
+    ((96, 40, 36), 0.9, 0.8, dict(periodic=(2, 1, 1), Ku=0.1, Kc=0.05)),     # tiled pass with the anti-periodic x wrap (ANTI instantiation)
     ((80, 30, 58), 0.6, 0.4, dict(Ku=0.05)),                               # tiled pass, one slab = all of y (halo wraps on both sides), R = 40
 ]
 
