@@ -88,7 +88,8 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
               void* dev_workspace, size_t workspace_bytes, void* cuda_stream, mc_ctx** out);
 int mc_destroy(mc_ctx* ctx);     /* frees the host handle only; the workspace stays the caller's */
 
-/* mode 0: all spins +z; mode 1: all spins along dir (normalised).  Asynchronous. */
+/* mode 0: all spins +z; mode 1: all spins along dir (normalised); mode 2: uniform on the sphere, seeded (site i takes
+ * Philox(ctr = (i, 3, 0, 0), key = seed): z = 2 u0 - 1, phi = 2 pi u1; BASELINE.json configs[2]).  Asynchronous. */
 int mc_init_spins(mc_ctx* ctx, int mode, const double dir[3]);
 /* Upload / download the spin state as [N][3] fp32 in lexicographic site order (x fastest).  mc_set_spins
  * normalises every spin.  Both synchronise the stream. */

@@ -61,6 +61,7 @@ def lib():
     L.orc_destroy.argtypes = [vp]; L.orc_destroy.restype = None
     for name in ("orc_set_spins", "orc_set_spins_f32", "orc_get_spins", "orc_init_uniform"):
         getattr(L, name).argtypes = [vp, vp]; getattr(L, name).restype = None
+    L.orc_init_random.argtypes = [vp]; L.orc_init_random.restype = None
     L.orc_set_cone.argtypes = [vp, dbl]; L.orc_set_cone.restype = None
     L.orc_set_sweep.argtypes = [vp, u64]; L.orc_set_sweep.restype = None
     L.orc_set_adaptive.argtypes = [vp, i32]; L.orc_set_adaptive.restype = None
@@ -138,6 +139,8 @@ class Oracle:
         u = [C.c_double(), C.c_double(), C.c_double()]
         self.L.orc_site_uniforms(self.h, int(x), int(y), int(z), int(colour), int(sweep), C.byref(u[0]), C.byref(u[1]), C.byref(u[2]))
         return tuple(v.value for v in u)
+
+    def init_random(self): self.L.orc_init_random(self.h)
 
     def profile_x(self):
         """[nx, 3] slice-averaged magnetisation along x (Fig. 2)."""

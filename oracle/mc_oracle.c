@@ -19,6 +19,7 @@
 #define TAG_MOVE     0u   /* unconstrained trial move, keyed on the site                 */
 #define TAG_PAIR     1u   /* constrained pair move, keyed on the leader's site           */
 #define TAG_PAIRING  2u   /* pairing parameters of one (sweep, colour); site word = 0    */
+#define TAG_INIT     3u   /* random initial state, keyed on the site (sweep words = 0)    */
 #define TAG_ORACLE  16u   /* oracle-only cross-check modes (random order, Fisher-Yates)  */
 
 static const double PI = 3.14159265358979323846;
@@ -232,6 +233,18 @@ void orc_init_uniform(orc_ctx* c, const double dir[3])
 {
     double n = sqrt(dir[0] * dir[0] + dir[1] * dir[1] + dir[2] * dir[2]);
     for (int64_t i = 0; i < c->N; ++i) for (int a = 0; a < 3; ++a) c->S[3 * i + a] = dir[a] / n;
+    c->aligned = 0;
+}
+/* Random start (BASELINE.json configs[2] "spins start uniformly random on the sphere (seeded)"): site i takes
+ * (r0,r1,..) = Philox(ctr = (i, TAG_INIT, 0, 0), key = seed), z = 2 u(r0) - 1, phi = 2 pi u(r1) (Archimedes: z uniform). */
+void orc_init_random(orc_ctx* c)
+{
+    for (int64_t i = 0; i < c->N; ++i) {
+        uint32_t r[4];
+        draw(c, (uint32_t)i, TAG_INIT, 0, 0, r);
+        double z = 2.0 * orc_uniform(r[0]) - 1.0, phi = 2.0 * PI * orc_uniform(r[1]), s = sqrt(1.0 - z * z);
+        c->S[3 * i] = s * cos(phi); c->S[3 * i + 1] = s * sin(phi); c->S[3 * i + 2] = z;
+    }
     c->aligned = 0;
 }
 void orc_set_cone(orc_ctx* c, double cone) { c->cone = cone; }

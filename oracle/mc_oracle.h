@@ -63,6 +63,7 @@ void orc_set_spins(orc_ctx*, const double* xyz /* [N][3] lexicographic */);
 void orc_set_spins_f32(orc_ctx*, const float* xyz);
 void orc_get_spins(const orc_ctx*, double* xyz);
 void orc_init_uniform(orc_ctx*, const double dir[3]);
+void orc_init_random(orc_ctx*);   /* uniform on the sphere, Philox tag 3 keyed on the site */
 void orc_set_cone(orc_ctx*, double cone_rad);
 void orc_set_sweep(orc_ctx*, uint64_t sweep);
 void orc_set_adaptive(orc_ctx*, int adaptive);

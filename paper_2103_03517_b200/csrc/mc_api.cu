@@ -491,6 +491,12 @@ int mc_init_spins(mc_ctx* ctx, int mode, const double dir[3])
         const double n = sqrt(dir[0] * dir[0] + dir[1] * dir[1] + dir[2] * dir[2]);
         if (!(n > 0)) return fail(ctx, MC_EINVAL, "mc_init_spins: zero direction");
         for (int a = 0; a < 3; ++a) d[a] = dir[a] / n;
+    } else if (mode == 2) {
+        init_random_kernel<<<(ctx->P.Nc + 255) / 256, 256, 0, ctx->stream>>>(ctx->P);
+        ctx->launches += 1;
+        CU(cudaGetLastError());
+        ctx->ml_valid = false; ctx->aligned = false;
+        return MC_OK;
     } else if (mode != 0) return fail(ctx, MC_EINVAL, "mc_init_spins: unknown mode");
     float f[3] = { (float)d[0], (float)d[1], (float)d[2] };
     const double fn = sqrt((double)f[0] * f[0] + (double)f[1] * f[1] + (double)f[2] * f[2]);

@@ -20,7 +20,7 @@ __device__ __forceinline__ void grid_dependency_sync()
 }
 
 // Stream tags (counter word 1, low byte); colour goes to bits 8..
-constexpr uint32_t TAG_MOVE = 0u, TAG_PAIR = 1u, TAG_PAIRING = 2u;
+constexpr uint32_t TAG_MOVE = 0u, TAG_PAIR = 1u, TAG_PAIRING = 2u, TAG_INIT = 3u;
 
 // ---------------------------------------------------------------------------------------------------------------
 // Philox4x32-10 (Salmon et al., SC'11): 10 rounds of

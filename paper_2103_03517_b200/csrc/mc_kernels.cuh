@@ -696,6 +696,27 @@ __global__ void fill_kernel(const __grid_constant__ Params P, float vx, float vy
     }
 }
 
+// Random start (BASELINE.json configs[2]: "spins start uniformly random on the sphere (seeded)"): the site with lexicographic
+// index i takes (r0,r1,..) = Philox(ctr = (i, TAG_INIT, 0, 0), key = seed), z = 2 u(r0) - 1, phi = 2 pi u(r1).
+__global__ void init_random_kernel(const __grid_constant__ Params P)
+{
+    const uint32_t a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= P.Nc) return;
+    const uint32_t R = (uint32_t)P.R, row = a / R, xh = a - row * R, y = row % (uint32_t)P.ny, z = row / (uint32_t)P.ny;
+    for (uint32_t c = 0; c < 2; ++c) {
+        const uint32_t site = row * (uint32_t)P.nx + 2u * xh + ((y + z + c) & 1u);
+        uint32_t r0, r1, r2, r3;
+        philox4x32_10(P.key, site, TAG_INIT, 0u, 0u, r0, r1, r2, r3);
+        const float zz = fmaf(2.0f, uniform01(r0), -1.0f);
+        float sp, cp; sincospif(2.0f * uniform01(r1), &sp, &cp);
+        const float s = sqrtf(fmaxf(0.0f, fmaf(-zz, zz, 1.0f)));
+        float vx = s * cp, vy = s * sp, vz = zz;
+        const float n = rsqrtf(fmaf(vx, vx, fmaf(vy, vy, vz * vz)));
+        float* Sc = P.S + (long long)c * 3 * P.plane;
+        Sc[a] = vx * n; Sc[P.plane + a] = vy * n; Sc[2 * P.plane + a] = vz * n;
+    }
+}
+
 // rigid rotation S <- Rm S of every spin, renormalised (C-12)
 struct Mat3 { float m[9]; };
 __global__ void rotate_kernel(const __grid_constant__ Params P, const __grid_constant__ Mat3 Rm)

@@ -249,6 +249,15 @@ def test_set_get_roundtrip_and_init(mods):
     g.close()
 
 
+def test_random_start_matches_oracle(mods):
+    oracle, binding, inputs = mods
+    for shape in ((24, 20, 16), (6, 4, 4)):
+        g = binding.Lattice(*shape, seed=11); g.init_spins(2)
+        o = oracle.Oracle(*shape, seed=11); o.init_random()
+        assert np.abs(g.get_spins() - o.get_spins()).max() < 2e-6
+        g.close()
+
+
 def test_error_paths(mods):
     oracle, binding, inputs = mods
     g = binding.Lattice(8, 4, 4)

@@ -110,6 +110,23 @@ def test_p2_site_uniforms_pair_sharing_and_moments():
     assert np.abs(c - np.eye(3)).max() < 4 / np.sqrt(n)
 
 
+def test_random_start_is_uniform_on_the_sphere_and_seeded():
+    o = oracle.Oracle(24, 20, 16, seed=7); o.init_random(); S = o.get_spins()
+    n = len(S)
+    assert np.abs(np.linalg.norm(S, axis=1) - 1).max() < 1e-15
+    assert np.abs(S.mean(axis=0)).max() < 4 * np.sqrt(1 / 3 / n)                       # <S> = 0
+    assert np.abs((S ** 2).mean(axis=0) - 1 / 3).max() < 4 * np.sqrt(4 / 45 / n)      # <S_a^2> = 1/3, var = 4/45
+    hist, _ = np.histogram(S[:, 2], bins=10, range=(-1, 1))                           # z flat (Archimedes)
+    assert np.abs(hist - n / 10).max() < 5 * np.sqrt(n / 10)
+    phi = np.arctan2(S[:, 1], S[:, 0]); hist, _ = np.histogram(phi, bins=8, range=(-np.pi, np.pi))
+    assert np.abs(hist - n / 8).max() < 5 * np.sqrt(n / 8)
+    r = oracle.philox4x32_10([5, 3, 0, 0], [7, 0])                                      # the wiring: site 5, tag 3
+    z = 2 * oracle.uniform(int(r[0])) - 1; ph = 2 * np.pi * oracle.uniform(int(r[1]))
+    assert np.allclose(S[5], [np.sqrt(1 - z * z) * np.cos(ph), np.sqrt(1 - z * z) * np.sin(ph), z], atol=1e-15)
+    o2 = oracle.Oracle(24, 20, 16, seed=7); o2.init_random(); assert (o2.get_spins() == S).all()
+    o3 = oracle.Oracle(24, 20, 16, seed=8); o3.init_random(); assert not (o3.get_spins() == S).all()
+
+
 # ---------------------------------------------------------------------------------------- P-3 cone move
 def _spins():
     rng = np.random.default_rng(5)
