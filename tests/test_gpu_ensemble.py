@@ -222,6 +222,44 @@ def test_full_size_c3_half_sweep_parity(mods):
     _full_size_half_sweep(mods, (224, 224, 224), 1.2, 1.0, 42, dict(Kc=0.01), colour=1)
 
 
+def test_full_size_c3_timed_kernels_match_the_checked_ones(mods):
+    """The kernels bench.py times at c3 are the compile-time-row-length instantiation launched back to back with
+    programmatic dependent launch; the parity test above goes through the instantiation that also writes the decision
+    variable.  Same state, same sweep counter: (i) one colour pass of the timed instantiation against the oracle
+    (a spin may differ only where the oracle's decision was marginal), and bit for bit against the checked one;
+    (ii) mc_sweep(T, 2) = four dependent launches against the same four passes issued one by one with a
+    synchronisation after each: bitwise equal spins, sums and controller state."""
+    oracle, binding, inputs = mods
+    shape, T = (224, 224, 224), 1.2
+    N = 224 ** 3
+    s0 = inputs.random_unit_spins(N, seed=42)
+    ham = dict(Kc=0.01)
+    g = binding.Lattice(*shape, seed=42, cone0=1.0, adaptive=False, **ham)
+    o = oracle.Oracle(*shape, seed=42, cone0=1.0, adaptive=False, **ham)
+    g.set_spins(s0); g.set_sweep(77); o.set_sweep(77)
+    before = g.get_spins(); o.set_spins(before)
+    _, x_o, acc_o = o.half_sweep(T, 0, want_detail=True)
+    g.half_sweep(T, 0)                                                     # no detail: the timed instantiation
+    fast = g.get_spins()
+    g.set_spins(s0); g.set_sweep(77)
+    g.half_sweep(T, 0, want_detail=True)                                   # the checked instantiation
+    assert (g.get_spins() == fast).all()
+    after_o = o.get_spins()
+    bad = np.abs(fast.astype(np.float64) - after_o).max(axis=1) >= 1e-4
+    assert (np.abs(x_o[bad]) < 1e-5).all() and bad.sum() < 50
+    g.close()
+    a = binding.Lattice(*shape, seed=42, cone0=0.5, adaptive=True, **ham); a.set_spins(s0)
+    b = binding.Lattice(*shape, seed=42, cone0=0.5, adaptive=True, **ham); b.set_spins(s0)
+    a.sweep(T, 2)
+    for _ in range(2):
+        b.half_sweep(T, 0); b.observables(); b.half_sweep(T, 1); b.end_sweep(); b.observables()
+    oa, ob = a.observables(), b.observables()
+    assert (a.get_spins() == b.get_spins()).all()
+    assert oa.sweep == ob.sweep == 2 and oa.cone_rad == ob.cone_rad and oa.E_total == ob.E_total and list(oa.M) == list(ob.M)
+    assert (a.trace() == b.trace()).all()
+    a.close(); b.close()
+
+
 def test_full_size_c5_half_sweep_parity(mods):
     """config c5: 2048 x 2048 x 4 granular film (16.8 M spins), Voronoi grains, per-grain axes, open z."""
     oracle, binding, inputs = mods
