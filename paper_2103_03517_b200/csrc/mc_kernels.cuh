@@ -222,6 +222,15 @@ __device__ __forceinline__ void fx_flush(long long (&acc)[NQ], float (&f)[NQ], f
     for (int q = 0; q < NQ; ++q) { acc[q] += __float2ll_rn(f[q] * scale); f[q] = 0.0f; }
 }
 
+// The generic kernels keep the fixed-point sums of a thread in shared memory (column threadIdx.x of [NQ][BLOCK]: no bank
+// conflicts) instead of 18 registers: they are short of registers (spills), and the sums are touched once per
+// FLUSH_ITEMS items.
+__device__ __forceinline__ void fx_flush_shared(long long (*sacc)[BLOCK], float (&f)[NQ], float scale)
+{
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) { sacc[q][threadIdx.x] += __float2ll_rn(f[q] * scale); f[q] = 0.0f; }
+}
+
 __device__ __forceinline__ long long warp_sum_i64(long long v)
 {
 #pragma unroll
@@ -354,10 +363,10 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
     float* Sc = P.S + (long long)colour * 3 * P.plane;
     const Vec3 B = { P.B[0], P.B[1], P.B[2] };
 
-    long long acc[NQ];               // exact fixed-point sums of this thread (fx_flush)
+    __shared__ long long sacc[NQ][BLOCK];   // exact fixed-point sums of every thread of the block (fx_flush_shared)
     float fs[NQ];                    // fp32 running sums of at most FLUSH_ITEMS items
 #pragma unroll
-    for (int q = 0; q < NQ; ++q) { acc[q] = 0; fs[q] = 0.0f; }
+    for (int q = 0; q < NQ; ++q) { sacc[q][threadIdx.x] = 0; fs[q] = 0.0f; }
     int cnt = 0, pending = 0;
 
     const uint32_t stride = gridDim.x * BLOCK;
@@ -414,9 +423,12 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
         }
 #pragma unroll
         for (int k = 0; k < NQ; ++k) fs[k] += f[k];
-        if (++pending == FLUSH_ITEMS) { fx_flush(acc, fs, P.fx_scale); pending = 0; }
+        if (++pending == FLUSH_ITEMS) { fx_flush_shared(sacc, fs, P.fx_scale); pending = 0; }
     }
-    fx_flush(acc, fs, P.fx_scale);
+    fx_flush_shared(sacc, fs, P.fx_scale);
+    long long acc[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) acc[q] = sacc[q][threadIdx.x];
 
     block_reduce(acc, cnt, P, MODE == MODE_MEASURE ? 1 : 0);
     if (flags & F_FINALIZE) {
@@ -496,11 +508,10 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
     float* Sc = P.S + (long long)colour * 3 * P.plane;
     const Vec3 B = { P.B[0], P.B[1], P.B[2] };
 
-    long long acc[NQ];               // exact fixed-point sums of this thread (fx_flush)
-    float fs[NQ];                    // fp32 running sums of at most FLUSH_ITEMS items
+    __shared__ long long sacc[NQ][BLOCK];   // exact fixed-point sums of every thread of the block (fx_flush_shared)
 #pragma unroll
-    for (int q = 0; q < NQ; ++q) { acc[q] = 0; fs[q] = 0.0f; }
-    int cnt = 0, pending = 0;
+    for (int q = 0; q < NQ; ++q) sacc[q][threadIdx.x] = 0;
+    int cnt = 0;
 
     const uint32_t stride = gridDim.x * BLOCK;
     for (uint32_t t = blockIdx.x * BLOCK + threadIdx.x; t < G.n_threads; t += stride) {
@@ -615,11 +626,11 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
         }
         st_rw<VEC>(Sc + aL, nlx); st_rw<VEC>(Sc + P.plane + aL, nly); st_rw<VEC>(Sc + 2 * P.plane + aL, nlz);
         st_rw<VEC>(Sc + aF, nfx); st_rw<VEC>(Sc + P.plane + aF, nfy); st_rw<VEC>(Sc + 2 * P.plane + aF, nfz);
-#pragma unroll
-        for (int k = 0; k < NQ; ++k) fs[k] += f[k];
-        if (++pending == FLUSH_ITEMS) { fx_flush(acc, fs, P.fx_scale); pending = 0; }
+        fx_flush_shared(sacc, f, P.fx_scale);        // every item (8 updates): this kernel has no registers to spare for running sums
     }
-    fx_flush(acc, fs, P.fx_scale);
+    long long acc[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) acc[q] = sacc[q][threadIdx.x];
 
     block_reduce(acc, cnt, P, 0);
     if (flags & F_FINALIZE) {
