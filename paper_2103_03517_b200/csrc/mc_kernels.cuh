@@ -509,6 +509,10 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
     const Vec3 B = { P.B[0], P.B[1], P.B[2] };
 
     __shared__ long long sacc[NQ][BLOCK];   // exact fixed-point sums of every thread of the block (fx_flush_shared)
+    // VEC = 4: the follower group's spins (rows 0..11 = component * 4 + element) and exchange field (rows 12..23) of every
+    // thread live in shared memory: the leader's element k pairs with element (k + rot) & 3 of the follower group, which is
+    // then one indexed shared-memory access instead of a chain of register selects, and 24 registers less (the kernel spills)
+    __shared__ float sF[VEC == 4 ? 24 : 1][BLOCK];
 #pragma unroll
     for (int q = 0; q < NQ; ++q) sacc[q][threadIdx.x] = 0;
     int cnt = 0;
@@ -537,6 +541,13 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
         exchange_field<VEC, MASKED>(P, qF, colour, hF);
         if (ANISO & 1) { easy_axes<VEC>(P, qL, colour, eL); easy_axes<VEC>(P, qF, colour, eF); }
         Pack<VEC> nlx = lx, nly = ly, nlz = lz, nfx = fx, nfy = fy, nfz = fz;
+        if (VEC == 4) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                sF[e][threadIdx.x] = fx.v[e]; sF[4 + e][threadIdx.x] = fy.v[e]; sF[8 + e][threadIdx.x] = fz.v[e];
+                sF[12 + e][threadIdx.x] = hF[e].x; sF[16 + e][threadIdx.x] = hF[e].y; sF[20 + e][threadIdx.x] = hF[e].z;
+            }
+        }
         float f[NQ];
 #pragma unroll
         for (int k = 0; k < NQ; ++k) f[k] = 0.0f;
@@ -546,17 +557,18 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
             Vec3 Si = { lx.v[k], ly.v[k], lz.v[k] };
             Vec3 Sj, hj, ej; uint32_t site_j;
             if (VEC == 4) {
-                // register permutation: select without dynamic indexing
-                float jx = fx.v[0], jy = fy.v[0], jz = fz.v[0];
-                Vec3 hh = hF[0], ee = eF[0];
+                const uint32_t kf = (k + rot) & 3u;
+                Sj = { sF[kf][threadIdx.x], sF[4 + kf][threadIdx.x], sF[8 + kf][threadIdx.x] };
+                hj = { sF[12 + kf][threadIdx.x], sF[16 + kf][threadIdx.x], sF[20 + kf][threadIdx.x] };
+                Vec3 ee = eF[0];
+                if (ANISO & 1) {
 #pragma unroll
-                for (int s = 1; s < 4; ++s) {
-                    const bool pick = ((k + rot) & 3u) == (uint32_t)s;
-                    jx = pick ? fx.v[s] : jx; jy = pick ? fy.v[s] : jy; jz = pick ? fz.v[s] : jz;
-                    hh.x = pick ? hF[s].x : hh.x; hh.y = pick ? hF[s].y : hh.y; hh.z = pick ? hF[s].z : hh.z;
-                    if (ANISO & 1) { ee.x = pick ? eF[s].x : ee.x; ee.y = pick ? eF[s].y : ee.y; ee.z = pick ? eF[s].z : ee.z; }
+                    for (int s = 1; s < 4; ++s) {
+                        const bool pick = kf == (uint32_t)s;
+                        ee.x = pick ? eF[s].x : ee.x; ee.y = pick ? eF[s].y : ee.y; ee.z = pick ? eF[s].z : ee.z;
+                    }
                 }
-                Sj = { jx, jy, jz }; hj = hh; ej = ee;
+                ej = ee;
                 site_j = qF.site0 + 2u * ((k + rot) & 3u);
             } else {
                 Sj = { fx.v[0], fy.v[0], fz.v[0] }; hj = hF[0]; ej = eF[0]; site_j = qF.site0;
@@ -602,11 +614,8 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
             if (ok) {
                 Si = Sni; nlx.v[k] = Sni.x; nly.v[k] = Sni.y; nlz.v[k] = Sni.z;
                 if (VEC == 4) {
-#pragma unroll
-                    for (int s = 0; s < 4; ++s) {
-                        const bool pick = ((k + rot) & 3u) == (uint32_t)s;
-                        nfx.v[s] = pick ? Snj.x : nfx.v[s]; nfy.v[s] = pick ? Snj.y : nfy.v[s]; nfz.v[s] = pick ? Snj.z : nfz.v[s];
-                    }
+                    const uint32_t kf = (k + rot) & 3u;
+                    sF[kf][threadIdx.x] = Snj.x; sF[4 + kf][threadIdx.x] = Snj.y; sF[8 + kf][threadIdx.x] = Snj.z;
                 } else { nfx.v[0] = Snj.x; nfy.v[0] = Snj.y; nfz.v[0] = Snj.z; }
             } else {
                 Snj = Sj;
@@ -623,6 +632,10 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
             const Vec3 ti = onsite_torque<ANISO>(Si, P.Ku, eL[(ANISO & 1) ? k : 0], P.Kc, B);
             const Vec3 tj = onsite_torque<ANISO>(Snj, P.Ku, ej, P.Kc, B);
             f[6] += ti.x + tj.x; f[7] += ti.y + tj.y; f[8] += ti.z + tj.z;
+        }
+        if (VEC == 4) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) { nfx.v[e] = sF[e][threadIdx.x]; nfy.v[e] = sF[4 + e][threadIdx.x]; nfz.v[e] = sF[8 + e][threadIdx.x]; }
         }
         st_rw<VEC>(Sc + aL, nlx); st_rw<VEC>(Sc + P.plane + aL, nly); st_rw<VEC>(Sc + 2 * P.plane + aL, nlz);
         st_rw<VEC>(Sc + aF, nfx); st_rw<VEC>(Sc + P.plane + aF, nfy); st_rw<VEC>(Sc + 2 * P.plane + aF, nfz);
