@@ -166,6 +166,89 @@ __device__ __forceinline__ Vec3 onsite_torque(const Vec3& S, float Ku, const Vec
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// Two-wide fp32 (Blackwell FFMA2 / FADD2 / FMUL2: two independent fp32 operations in one issue slot) and the packed
+// twins of the functions above: lane x and lane y are two different sites / pairs, each lane performs exactly the
+// scalar function's arithmetic (fmaf <-> fma2 lane by lane).
+// ---------------------------------------------------------------------------------------------------------------
+typedef float2 f2;
+__device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ f2 splat(float v) { return make_float2(v, v); }
+__device__ __forceinline__ f2 neg2(f2 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ f2 sub2(f2 a, f2 b) { return add2(a, neg2(b)); }
+
+struct V3p { f2 x, y, z; };                                  // two 3-vectors, component-wise packed
+__device__ __forceinline__ V3p pack3(const Vec3& a, const Vec3& b) { return { make_float2(a.x, b.x), make_float2(a.y, b.y), make_float2(a.z, b.z) }; }
+__device__ __forceinline__ V3p splat3(const Vec3& a) { return { splat(a.x), splat(a.y), splat(a.z) }; }
+__device__ __forceinline__ Vec3 lane3(const V3p& a, int l) { return l ? Vec3{ a.x.y, a.y.y, a.z.y } : Vec3{ a.x.x, a.y.x, a.z.x }; }
+__device__ __forceinline__ f2 dot3p(const V3p& a, const V3p& b) { return fma2(a.x, b.x, fma2(a.y, b.y, mul2(a.z, b.z))); }
+
+__device__ __forceinline__ void cone_move2(const V3p& S, float one_minus_cos, f2 u0, f2 u1, V3p& d, V3p& Sn)
+{
+    const f2 w  = mul2(u0, splat(one_minus_cos));
+    const f2 t  = mul2(w, sub2(splat(2.0f), w));
+    const f2 sa = mul2(t, make_float2(rsqrtf(t.x), rsqrtf(t.y)));
+    const f2 ang = fma2(u1, splat(6.2831853071795865f), splat(-3.1415926535897932f));
+    const f2 cp = make_float2(-__cosf(ang.x), -__cosf(ang.y)), sp = make_float2(-__sinf(ang.x), -__sinf(ang.y));
+    const f2 sg = make_float2(S.z.x >= 0.0f ? 1.0f : -1.0f, S.z.y >= 0.0f ? 1.0f : -1.0f);
+    const f2 den = add2(sg, S.z);
+    const f2 a  = make_float2(__fdividef(-1.0f, den.x), __fdividef(-1.0f, den.y));
+    const f2 b  = mul2(mul2(S.x, S.y), a);
+    const V3p t1 = { fma2(mul2(mul2(sg, S.x), S.x), a, splat(1.0f)), mul2(sg, b), neg2(mul2(sg, S.x)) };
+    const V3p t2 = { b, fma2(mul2(S.y, S.y), a, sg), neg2(S.y) };
+    const f2 ca = mul2(sa, cp), cb = mul2(sa, sp), nw = neg2(w);
+    d.x = fma2(ca, t1.x, fma2(cb, t2.x, mul2(nw, S.x)));
+    d.y = fma2(ca, t1.y, fma2(cb, t2.y, mul2(nw, S.y)));
+    d.z = fma2(ca, t1.z, fma2(cb, t2.z, mul2(nw, S.z)));
+    const V3p v = { add2(S.x, d.x), add2(S.y, d.y), add2(S.z, d.z) };
+    const f2 inv = fma2(splat(-0.5f), dot3p(v, v), splat(1.5f));
+    Sn = { mul2(v.x, inv), mul2(v.y, inv), mul2(v.z, inv) };
+}
+
+template <int ANISO>
+__device__ __forceinline__ f2 delta_energy2(const V3p& S, const V3p& d, const V3p& hB, float Ku, const V3p& e, float Kc)
+{
+    f2 dE = neg2(dot3p(d, hB));
+    if (ANISO & 1) {
+        const V3p s2 = { fma2(splat(2.0f), S.x, d.x), fma2(splat(2.0f), S.y, d.y), fma2(splat(2.0f), S.z, d.z) };
+        dE = fma2(mul2(splat(-Ku), dot3p(d, e)), dot3p(s2, e), dE);
+    }
+    if (ANISO & 2) {
+        const f2 nx = add2(S.x, d.x), ny = add2(S.y, d.y), nz = add2(S.z, d.z);
+        const f2 qx = mul2(mul2(d.x, add2(S.x, nx)), fma2(S.x, S.x, mul2(nx, nx)));
+        const f2 qy = mul2(mul2(d.y, add2(S.y, ny)), fma2(S.y, S.y, mul2(ny, ny)));
+        const f2 qz = mul2(mul2(d.z, add2(S.z, nz)), fma2(S.z, S.z, mul2(nz, nz)));
+        dE = fma2(splat(-0.5f * Kc), add2(add2(qx, qy), qz), dE);
+    }
+    return dE;
+}
+
+template <int ANISO>
+__device__ __forceinline__ f2 aniso_energy2(const V3p& S, float Ku, const V3p& e, float Kc)
+{
+    f2 E = splat(0.0f);
+    if (ANISO & 1) { const f2 se = dot3p(S, e); E = mul2(mul2(splat(-Ku), se), se); }
+    if (ANISO & 2) {
+        const f2 x2 = mul2(S.x, S.x), y2 = mul2(S.y, S.y), z2 = mul2(S.z, S.z);
+        E = fma2(splat(Kc), fma2(x2, y2, fma2(x2, z2, mul2(y2, z2))), E);
+    }
+    return E;
+}
+
+template <int ANISO>
+__device__ __forceinline__ V3p onsite_torque2(const V3p& S, float Ku, const V3p& e, float Kc, const V3p& B)
+{
+    V3p H = B;
+    if (ANISO & 1) { const f2 f = mul2(splat(2.0f * Ku), dot3p(S, e)); H.x = fma2(f, e.x, H.x); H.y = fma2(f, e.y, H.y); H.z = fma2(f, e.z, H.z); }
+    if (ANISO & 2) {
+        const f2 x2 = mul2(S.x, S.x), y2 = mul2(S.y, S.y), z2 = mul2(S.z, S.z), g = splat(-2.0f * Kc);
+        H.x = fma2(mul2(g, S.x), add2(y2, z2), H.x); H.y = fma2(mul2(g, S.y), add2(x2, z2), H.y); H.z = fma2(mul2(g, S.z), add2(x2, y2), H.z);
+    }
+    return { sub2(mul2(S.y, H.z), mul2(S.z, H.y)), sub2(mul2(S.z, H.x), mul2(S.x, H.z)), sub2(mul2(S.x, H.y), mul2(S.y, H.x)) };
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // Division by a run-time constant with a precomputed magic number (host fills it): q = (n * mul) >> (32 + shift).
 // Exact for n < 2^31 (round-up method).
 // ---------------------------------------------------------------------------------------------------------------

@@ -551,8 +551,100 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
         float f[NQ];
 #pragma unroll
         for (int k = 0; k < NQ; ++k) f[k] = 0.0f;
+        if (VEC == 4) {
+            // ---- two pairs at a time in the two lanes of FFMA2 / FADD2 / FMUL2: lane x = pair kp, lane y = pair kp + 1.
+            // Lane by lane this is the arithmetic of the scalar loop below (VEC = 1), branches turned into selects.
+            const V3p eC2 = splat3(eC), B2 = splat3(B);
+            f2 f2s[NQ];
 #pragma unroll
-        for (int k = 0; k < VEC; ++k) {
+            for (int q = 0; q < NQ; ++q) f2s[q] = splat(0.0f);
+#pragma unroll
+            for (int kp = 0; kp < 4; kp += 2) {
+                const uint32_t kf0 = (kp + rot) & 3u, kf1 = (kp + 1 + rot) & 3u;
+                const uint32_t tx = threadIdx.x;
+                V3p Si = { make_float2(lx.v[kp], lx.v[kp + 1]), make_float2(ly.v[kp], ly.v[kp + 1]), make_float2(lz.v[kp], lz.v[kp + 1]) };
+                const V3p Sj = { make_float2(sF[kf0][tx], sF[kf1][tx]), make_float2(sF[4 + kf0][tx], sF[4 + kf1][tx]), make_float2(sF[8 + kf0][tx], sF[8 + kf1][tx]) };
+                const V3p hj = { make_float2(sF[12 + kf0][tx], sF[12 + kf1][tx]), make_float2(sF[16 + kf0][tx], sF[16 + kf1][tx]), make_float2(sF[20 + kf0][tx], sF[20 + kf1][tx]) };
+                const V3p hi = pack3(hL[kp], hL[kp + 1]);
+                V3p ei = eC2, ej = eC2;                      // placeholders when ANISO & 1 == 0
+                if (ANISO & 1) {
+                    ei = pack3(eL[kp], eL[kp + 1]);
+                    Vec3 e0 = eF[0], e1 = eF[0];
+#pragma unroll
+                    for (int s2 = 1; s2 < 4; ++s2) {
+                        const bool p0 = kf0 == (uint32_t)s2, p1 = kf1 == (uint32_t)s2;
+                        e0.x = p0 ? eF[s2].x : e0.x; e0.y = p0 ? eF[s2].y : e0.y; e0.z = p0 ? eF[s2].z : e0.z;
+                        e1.x = p1 ? eF[s2].x : e1.x; e1.y = p1 ? eF[s2].y : e1.y; e1.z = p1 ? eF[s2].z : e1.z;
+                    }
+                    ej = pack3(e0, e1);
+                }
+                const uint32_t site_i0 = qL.site0 + 2u * kp, site_i1 = site_i0 + 2u;
+                uint32_t a0, a1, a2, a3, b0, b1, b2, b3;
+                philox4x32_10(key, site_i0, c1, c2, c3, a0, a1, a2, a3);
+                philox4x32_10(key, site_i1, c1, c2, c3, b0, b1, b2, b3);
+                V3p di, Sni;
+                cone_move2(Si, omc, make_float2(uniform01(a0), uniform01(b0)), make_float2(uniform01(a1), uniform01(b1)), di, Sni);
+                const f2 pi_ = dot3p(Si, eC2), pj = dot3p(Sj, eC2), pni = dot3p(Sni, eC2);
+                const V3p dv = { sub2(Si.x, Sni.x), sub2(Si.y, Sni.y), sub2(Si.z, Sni.z) };
+                const f2 dpar = dot3p(dv, eC2), npj = neg2(pj), ndpar = neg2(dpar);
+                const V3p pj_perp = { fma2(npj, eC2.x, Sj.x), fma2(npj, eC2.y, Sj.y), fma2(npj, eC2.z, Sj.z) };
+                const V3p dl = { fma2(ndpar, eC2.x, dv.x), fma2(ndpar, eC2.y, dv.y), fma2(ndpar, eC2.z, dv.z) };
+                const V3p perp = { add2(pj_perp.x, dl.x), add2(pj_perp.y, dl.y), add2(pj_perp.z, dl.z) };
+                const V3p tw = { fma2(splat(2.0f), pj_perp.x, dl.x), fma2(splat(2.0f), pj_perp.y, dl.y), fma2(splat(2.0f), pj_perp.z, dl.z) };
+                const f2 rho = fma2(pj, pj, neg2(dot3p(dl, tw)));                                   // P:189 radicand, difference form
+                const bool v0 = rho.x > 0.0f, v1 = rho.y > 0.0f;                                    // C-13: radicand <= 0 rejects
+                const f2 rs = make_float2(v0 ? rho.x : 1.0f, v1 ? rho.y : 1.0f);
+                const f2 rt = mul2(rs, make_float2(rsqrtf(rs.x), rsqrtf(rs.y)));
+                const f2 pnj = make_float2(copysignf(rt.x, pj.x), copysignf(rt.y, pj.y));           // sign kept
+                const V3p v = { fma2(pnj, eC2.x, perp.x), fma2(pnj, eC2.y, perp.y), fma2(pnj, eC2.z, perp.z) };
+                const f2 inv = fma2(splat(-0.5f), dot3p(v, v), splat(1.5f));
+                const V3p Snj_new = { mul2(v.x, inv), mul2(v.y, inv), mul2(v.z, inv) };
+                const f2 yml = mul2(sub2(sub2(add2(pni, pnj), pi_), pj), splat(invML));              // (M_L^ - M_L)/M_L
+                const bool w0 = v0 && (1.0f + yml.x > 0.0f), w1 = v1 && (1.0f + yml.y > 0.0f);      // M_L^ > 0 (C-13)
+                const f2 poly = mul2(yml, fma2(neg2(yml), fma2(neg2(yml), fma2(splat(-0.25f), yml, splat(0.33333333f)), splat(0.5f)), splat(1.0f)));
+                const f2 lg = make_float2(__logf(w0 ? 1.0f + yml.x : 1.0f), __logf(w1 ? 1.0f + yml.y : 1.0f));
+                const f2 lr = make_float2(fabsf(yml.x) < 0.03f ? poly.x : lg.x, fabsf(yml.y) < 0.03f ? poly.y : lg.y);
+                const V3p dj = { sub2(Snj_new.x, Sj.x), sub2(Snj_new.y, Sj.y), sub2(Snj_new.z, Sj.z) };
+                const f2 J2 = splat(P.J);
+                const V3p hBi = { fma2(J2, hi.x, B2.x), fma2(J2, hi.y, B2.y), fma2(J2, hi.z, B2.z) };
+                const V3p hBj = { fma2(J2, hj.x, B2.x), fma2(J2, hj.y, B2.y), fma2(J2, hj.z, B2.z) };
+                const f2 dE = add2(delta_energy2<ANISO>(Si, di, hBi, P.Ku, ei, P.Kc), delta_energy2<ANISO>(Sj, dj, hBj, P.Ku, ej, P.Kc));   // P:193 (C-4)
+                const f2 lu = make_float2(__logf(uniform01(a2)), __logf(uniform01(b2)));
+                const f2 lq = make_float2(__logf(__fdividef(fabsf(pj.x), fabsf(pnj.x))), __logf(__fdividef(fabsf(pj.y), fabsf(pnj.y))));
+                const f2 xr = sub2(sub2(fma2(dE, splat(invT), lu), mul2(splat(2.0f), lr)), lq);     // P:193 in log form
+                const float INF = __int_as_float(0x7f800000);
+                const float x0 = w0 ? xr.x : INF, x1 = w1 ? xr.y : INF;
+                const bool ok0 = x0 < 0.0f, ok1 = x1 < 0.0f;
+                // P:194 keep or restore both members
+                Si.x = make_float2(ok0 ? Sni.x.x : Si.x.x, ok1 ? Sni.x.y : Si.x.y);
+                Si.y = make_float2(ok0 ? Sni.y.x : Si.y.x, ok1 ? Sni.y.y : Si.y.y);
+                Si.z = make_float2(ok0 ? Sni.z.x : Si.z.x, ok1 ? Sni.z.y : Si.z.y);
+                const V3p Snj = { make_float2(ok0 ? Snj_new.x.x : Sj.x.x, ok1 ? Snj_new.x.y : Sj.x.y),
+                                  make_float2(ok0 ? Snj_new.y.x : Sj.y.x, ok1 ? Snj_new.y.y : Sj.y.y),
+                                  make_float2(ok0 ? Snj_new.z.x : Sj.z.x, ok1 ? Snj_new.z.y : Sj.z.y) };
+                nlx.v[kp] = Si.x.x; nlx.v[kp + 1] = Si.x.y; nly.v[kp] = Si.y.x; nly.v[kp + 1] = Si.y.y; nlz.v[kp] = Si.z.x; nlz.v[kp + 1] = Si.z.y;
+                sF[kf0][tx] = Snj.x.x; sF[4 + kf0][tx] = Snj.y.x; sF[8 + kf0][tx] = Snj.z.x;
+                sF[kf1][tx] = Snj.x.y; sF[4 + kf1][tx] = Snj.y.y; sF[8 + kf1][tx] = Snj.z.y;
+                cnt += (ok0 ? 2 : 0) + (ok1 ? 2 : 0);                                               // P:195 (C-23)
+                const uint32_t site_j0 = qF.site0 + 2u * kf0, site_j1 = qF.site0 + 2u * kf1;
+                if (dbg_x)   { dbg_x[site_i0] = x0; dbg_x[site_i1] = x1; }
+                if (dbg_acc) { dbg_acc[site_i0] = (uint8_t)ok0; dbg_acc[site_j0] = (uint8_t)ok0; dbg_acc[site_i1] = (uint8_t)ok1; dbg_acc[site_j1] = (uint8_t)ok1; }
+                // fused sums of the final spins of both members
+                f2s[0] = add2(f2s[0], add2(Si.x, Snj.x)); f2s[1] = add2(f2s[1], add2(Si.y, Snj.y)); f2s[2] = add2(f2s[2], add2(Si.z, Snj.z));
+                if (colour == 1) {
+                    const V3p hJi = { mul2(J2, hi.x), mul2(J2, hi.y), mul2(J2, hi.z) }, hJj = { mul2(J2, hj.x), mul2(J2, hj.y), mul2(J2, hj.z) };
+                    f2s[3] = sub2(f2s[3], add2(dot3p(Si, hJi), dot3p(Snj, hJj)));
+                }
+                if (ANISO) f2s[4] = add2(f2s[4], add2(aniso_energy2<ANISO>(Si, P.Ku, ei, P.Kc), aniso_energy2<ANISO>(Snj, P.Ku, ej, P.Kc)));
+                f2s[5] = sub2(f2s[5], add2(dot3p(Si, B2), dot3p(Snj, B2)));
+                const V3p ti = onsite_torque2<ANISO>(Si, P.Ku, ei, P.Kc, B2), tj = onsite_torque2<ANISO>(Snj, P.Ku, ej, P.Kc, B2);
+                f2s[6] = add2(f2s[6], add2(ti.x, tj.x)); f2s[7] = add2(f2s[7], add2(ti.y, tj.y)); f2s[8] = add2(f2s[8], add2(ti.z, tj.z));
+            }
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) f[q] = f2s[q].x + f2s[q].y;
+        }
+#pragma unroll
+        for (int k = 0; k < (VEC == 4 ? 0 : VEC); ++k) {
             // leader element k pairs with follower element kf = (k + rot) mod Bl of the follower group (VEC = 4)
             Vec3 Si = { lx.v[k], ly.v[k], lz.v[k] };
             Vec3 Sj, hj, ej; uint32_t site_j;

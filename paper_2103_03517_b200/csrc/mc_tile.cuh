@@ -47,11 +47,7 @@ struct TileGeom {
 };
 
 // ---- packed two-wide fp32 helpers (FFMA2 / FADD2 / FMUL2 on sm_100a)
-typedef float2 f2;
-__device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
-__device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
-__device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
-__device__ __forceinline__ f2 splat(float v) { return make_float2(v, v); }
+// (f2, add2, mul2, fma2, splat: mc_device.cuh)
 
 // ---- mbarrier / TMA bulk-copy primitives (PTX; CTA-local shared addresses)
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
