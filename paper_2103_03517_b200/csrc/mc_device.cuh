@@ -175,8 +175,10 @@ __device__ __forceinline__ f2 add2(f2 a, f2 b) { return __fadd2_rn(a, b); }
 __device__ __forceinline__ f2 mul2(f2 a, f2 b) { return __fmul2_rn(a, b); }
 __device__ __forceinline__ f2 fma2(f2 a, f2 b, f2 c) { return __ffma2_rn(a, b, c); }
 __device__ __forceinline__ f2 splat(float v) { return make_float2(v, v); }
-__device__ __forceinline__ f2 neg2(f2 a) { return make_float2(-a.x, -a.y); }
-__device__ __forceinline__ f2 sub2(f2 a, f2 b) { return add2(a, neg2(b)); }
+// packed operands take no per-lane negation: a lane-wise minus would be two scalar instructions, so it is a multiply
+// by -1 (exact), and a - b is one FFMA2 (-1 * b + a, exact product: the same rounding as a subtraction)
+__device__ __forceinline__ f2 neg2(f2 a) { return mul2(a, splat(-1.0f)); }
+__device__ __forceinline__ f2 sub2(f2 a, f2 b) { return fma2(splat(-1.0f), b, a); }
 
 struct V3p { f2 x, y, z; };                                  // two 3-vectors, component-wise packed
 __device__ __forceinline__ V3p pack3(const Vec3& a, const Vec3& b) { return { make_float2(a.x, b.x), make_float2(a.y, b.y), make_float2(a.z, b.z) }; }

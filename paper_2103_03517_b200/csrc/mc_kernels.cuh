@@ -179,8 +179,20 @@ __device__ __forceinline__ void exchange_field(const Params& P, const ItemPos& q
                 s += (mb & 16u) ? zp.v[k] : 0.0f;
                 s += (mb & 32u) ? zm.v[k] : 0.0f;
                 hc[c][k] = s;
-            } else {
+            } else if (VEC != 4) {
                 hc[c][k] = ((o.v[k] + sh) + (yp.v[k] + ym.v[k])) + (zp.v[k] + zm.v[k]);
+            }
+        }
+        if (!MASKED && VEC == 4) {
+            // the same sums two lanes at a time (the float4 loads are already aligned register pairs)
+            const float s0 = q.par ? o.v[1] : ex, s1 = q.par ? o.v[2] : o.v[0], s2 = q.par ? o.v[3] : o.v[1], s3 = q.par ? ex : o.v[2];
+#pragma unroll
+            for (int h2 = 0; h2 < 2; ++h2) {
+                const int a = 2 * h2, b = 2 * h2 + 1;
+                const f2 sh2 = h2 ? make_float2(s2, s3) : make_float2(s0, s1);
+                const f2 r = add2(add2(add2(make_float2(o.v[a], o.v[b]), sh2), add2(make_float2(yp.v[a], yp.v[b]), make_float2(ym.v[a], ym.v[b]))),
+                                  add2(make_float2(zp.v[a], zp.v[b]), make_float2(zm.v[a], zm.v[b])));
+                hc[c][a] = r.x; hc[c][b] = r.y;
             }
         }
     }
