@@ -55,6 +55,7 @@ def lib():
     L.orc_uniform.argtypes = [C.c_uint32]; L.orc_uniform.restype = dbl
     L.orc_uniform_azimuth.argtypes = [C.c_uint32, C.c_uint32]; L.orc_uniform_azimuth.restype = dbl
     L.orc_site_uniforms.argtypes = [vp, i32, i32, i32, i32, u64, vp, vp, vp]; L.orc_site_uniforms.restype = None
+    L.orc_pair_uniforms.argtypes = [vp, i32, i32, i32, i32, u64, vp, vp, vp]; L.orc_pair_uniforms.restype = None
     L.orc_cone_move.argtypes = [vp, dbl, dbl, dbl, vp]; L.orc_cone_move.restype = None
     L.orc_create.argtypes = [i32, i32, i32, vp, dbl, dbl, vp, dbl, vp, vp, vp, vp, i32, dbl, i32, u64]
     L.orc_create.restype = vp
@@ -145,6 +146,12 @@ class Oracle:
     def profile_x(self):
         """[nx, 3] slice-averaged magnetisation along x (Fig. 2)."""
         out = np.zeros((self.shape[0], 3)); self.L.orc_profile_x(self.h, _p(out)); return out
+
+    def pair_uniforms(self, x, y, z, colour, sweep):
+        """(u0, u1, u2) of the constrained move of the pair led by site (x,y,z) (stream TAG_PAIR, reading C-26)."""
+        u = [C.c_double(), C.c_double(), C.c_double()]
+        self.L.orc_pair_uniforms(self.h, int(x), int(y), int(z), int(colour), int(sweep), C.byref(u[0]), C.byref(u[1]), C.byref(u[2]))
+        return tuple(v.value for v in u)
 
     # ---- state
     def set_spins(self, xyz):

@@ -259,16 +259,26 @@ void orc_set_sampling(orc_ctx* c, int on) { c->sampling = on; }
  *   u0 = ((w0 >> 9) + 0.5) 2^-23   (cone polar draw),     u2 = ((w1 >> 9) + 0.5) 2^-23   (acceptance draw),
  *   u1 = (((w0 & 511) << 9) | (w1 & 511)) 2^-18            (cone azimuth).
  * 64 random bits per update, every bit used once. */
-void orc_site_uniforms(const orc_ctx* c, int x, int y, int z, int colour, uint64_t sweep, double* u0, double* u1, double* u2)
+static void site_uniforms_tag(const orc_ctx* c, int x, int y, int z, uint32_t tag, int colour, uint64_t sweep, double* u0, double* u1, double* u2)
 {
     int64_t first = site_index(c, x & ~2, y, z);
     int half = (x >> 1) & 1;
     uint32_t r[4];
-    draw(c, (uint32_t)first, TAG_MOVE, colour, sweep, r);
+    draw(c, (uint32_t)first, tag, colour, sweep, r);
     uint32_t w0 = r[2 * half], w1 = r[2 * half + 1];
     *u0 = orc_uniform(w0);
     *u1 = orc_uniform_azimuth(w0, w1);
     *u2 = orc_uniform(w1);
+}
+
+void orc_site_uniforms(const orc_ctx* c, int x, int y, int z, int colour, uint64_t sweep, double* u0, double* u1, double* u2)
+{
+    site_uniforms_tag(c, x, y, z, TAG_MOVE, colour, sweep, u0, u1, u2);
+}
+/* the same 64 bits per move for the constrained pair move, keyed on the LEADER's site in its own stream (TAG_PAIR) */
+void orc_pair_uniforms(const orc_ctx* c, int x, int y, int z, int colour, uint64_t sweep, double* u0, double* u1, double* u2)
+{
+    site_uniforms_tag(c, x, y, z, TAG_PAIR, colour, sweep, u0, u1, u2);
 }
 
 /* ------------------------------------------------------------------ Table A1: one colour pass */
@@ -485,9 +495,8 @@ int orc_align_to(orc_ctx* c, const double eC[3])
 static int pair_update(orc_ctx* c, double T, const double e[3], int colour, int64_t si, int64_t sj,
                        double* ML, int ml_mode, double* xdec, int may_be_neighbours)
 {
-    uint32_t r[4];
-    draw(c, (uint32_t)si, TAG_PAIR, colour, c->sweep, r);
-    double u0 = orc_uniform(r[0]), u1 = orc_uniform(r[1]), u2 = orc_uniform(r[2]);
+    double u0, u1, u2;                                                    /* P:186, P:193 UniformRandom() x 3 (C-26) */
+    orc_pair_uniforms(c, (int)(si % c->nx), (int)((si / c->nx) % c->ny), (int)(si / ((int64_t)c->nx * c->ny)), colour, c->sweep, &u0, &u1, &u2);
     double *Si = &c->S[3 * si], *Sj = &c->S[3 * sj], Sni[3], Snj[3];
     orc_cone_move(Si, c->cone, u0, u1, Sni);                              /* P:186 */
     double Si_par = Si[0] * e[0] + Si[1] * e[1] + Si[2] * e[2];

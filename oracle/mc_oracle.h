@@ -45,6 +45,8 @@ double orc_uniform_azimuth(uint32_t w0, uint32_t w1);
 /* The three uniforms of the unconstrained update of site (x,y,z): one Philox block per pair of x-neighbours of one
  * colour (x, x^2), 64 bits per site (reading C-26 in DESIGN.md section 4). */
 void orc_site_uniforms(const orc_ctx* c, int x, int y, int z, int colour, uint64_t sweep, double* u0, double* u1, double* u2);
+/* The same for the constrained pair move of the pair whose LEADER is (x,y,z) (stream TAG_PAIR). */
+void orc_pair_uniforms(const orc_ctx* c, int x, int y, int z, int colour, uint64_t sweep, double* u0, double* u1, double* u2);
 /* Cone trial move: S unit, theta = cone half-angle, u0,u1 in (0,1). */
 void orc_cone_move(const double S[3], double theta, double u0, double u1, double Snew[3]);
 

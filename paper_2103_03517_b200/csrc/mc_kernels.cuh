@@ -481,6 +481,7 @@ __device__ __forceinline__ ItemPos locate_linear(const Params& P, const PairGeom
     ItemPos q;
     const uint32_t R = (uint32_t)P.R, ny = (uint32_t)P.ny, nz = (uint32_t)P.nz;
     q.par = (y + z + (uint32_t)colour) & 1u;
+    q.xh0 = xh0;
     q.a0 = a0;
     q.site0 = row * (uint32_t)P.nx + 2u * xh0 + q.par;
     const uint32_t yp = (y + 1 == ny) ? 0u : y + 1, ym = (y == 0) ? ny - 1 : y - 1;
@@ -591,11 +592,11 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
                     ej = pack3(e0, e1);
                 }
                 const uint32_t site_i0 = qL.site0 + 2u * kp, site_i1 = site_i0 + 2u;
-                uint32_t a0, a1, a2, a3, b0, b1, b2, b3;
-                philox4x32_10(key, site_i0, c1, c2, c3, a0, a1, a2, a3);
-                philox4x32_10(key, site_i1, c1, c2, c3, b0, b1, b2, b3);
+                // one Philox block per two pairs: the leaders site_i0 (bit 1 of x clear) and site_i0 + 2 take words (0,1) and (2,3) (C-26)
+                uint32_t a0, a1, b0, b1;
+                philox4x32_10(key, site_i0, c1, c2, c3, a0, a1, b0, b1);
                 V3p di, Sni;
-                cone_move2(Si, omc, make_float2(uniform01(a0), uniform01(b0)), make_float2(uniform01(a1), uniform01(b1)), di, Sni);
+                cone_move2(Si, omc, make_float2(uniform01(a0), uniform01(b0)), make_float2(uniform_azimuth(a0, a1), uniform_azimuth(b0, b1)), di, Sni);
                 const f2 pi_ = dot3p(Si, eC2), pj = dot3p(Sj, eC2), pni = dot3p(Sni, eC2);
                 const V3p dv = { sub2(Si.x, Sni.x), sub2(Si.y, Sni.y), sub2(Si.z, Sni.z) };
                 const f2 dpar = dot3p(dv, eC2), npj = neg2(pj), ndpar = neg2(dpar);
@@ -621,7 +622,7 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
                 const V3p hBi = { fma2(J2, hi.x, B2.x), fma2(J2, hi.y, B2.y), fma2(J2, hi.z, B2.z) };
                 const V3p hBj = { fma2(J2, hj.x, B2.x), fma2(J2, hj.y, B2.y), fma2(J2, hj.z, B2.z) };
                 const f2 dE = add2(delta_energy2<ANISO>(Si, di, hBi, P.Ku, ei, P.Kc), delta_energy2<ANISO>(Sj, dj, hBj, P.Ku, ej, P.Kc));   // P:193 (C-4)
-                const f2 lu = make_float2(__logf(uniform01(a2)), __logf(uniform01(b2)));
+                const f2 lu = make_float2(__logf(uniform01(a1)), __logf(uniform01(b1)));
                 const f2 lq = make_float2(__logf(__fdividef(fabsf(pj.x), fabsf(pnj.x))), __logf(__fdividef(fabsf(pj.y), fabsf(pnj.y))));
                 const f2 xr = sub2(sub2(fma2(dE, splat(invT), lu), mul2(splat(2.0f), lr)), lq);     // P:193 in log form
                 const float INF = __int_as_float(0x7f800000);
@@ -678,10 +679,15 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
                 Sj = { fx.v[0], fy.v[0], fz.v[0] }; hj = hF[0]; ej = eF[0]; site_j = qF.site0;
             }
             const uint32_t site_i = qL.site0 + 2u * k;
-            uint32_t r0, r1, r2, r3;
-            philox4x32_10(key, site_i, c1, c2, c3, r0, r1, r2, r3);
+            uint32_t w0, w1;                                                           // the leader's 64 bits (C-26)
+            {
+                const uint32_t half = (qL.xh0 + (uint32_t)k) & 1u;
+                uint32_t r0, r1, r2, r3;
+                philox4x32_10(key, site_i - 2u * half, c1, c2, c3, r0, r1, r2, r3);
+                w0 = half ? r2 : r0; w1 = half ? r3 : r1;
+            }
             Vec3 di, Sni;
-            cone_move(Si, omc, uniform01(r0), uniform01(r1), di, Sni);
+            cone_move(Si, omc, uniform01(w0), uniform_azimuth(w0, w1), di, Sni);
             const float pi_ = dot3(Si, eC), pj = dot3(Sj, eC), pni = dot3(Sni, eC);
             const Vec3 dv = { Si.x - Sni.x, Si.y - Sni.y, Si.z - Sni.z };             // stored displacement, exact in fp32
             // transverse parts: S_j,perp and the compensation delta = S_i,perp - S'_i,perp
@@ -711,7 +717,7 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
                     const float dE = delta_energy<ANISO>(Si, di, hBi, P.Ku, eL[(ANISO & 1) ? k : 0], P.Kc)
                                    + delta_energy<ANISO>(Sj, dj, hBj, P.Ku, ej, P.Kc);  // P:193 (C-4)
                     // P:193 in log form: dE/T - 2 ln(M_L^/M_L) - ln|S_j,par / S'_j,par| + ln u2 < 0
-                    x = fmaf(dE, invT, __logf(uniform01(r2))) - 2.0f * lr - __logf(__fdividef(fabsf(pj), fabsf(pnj)));
+                    x = fmaf(dE, invT, __logf(uniform01(w1))) - 2.0f * lr - __logf(__fdividef(fabsf(pj), fabsf(pnj)));
                     ok = x < 0.0f;
                 }
             }

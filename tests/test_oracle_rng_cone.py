@@ -110,6 +110,19 @@ def test_p2_site_uniforms_pair_sharing_and_moments():
     assert np.abs(c - np.eye(3)).max() < 4 / np.sqrt(n)
 
 
+def test_pair_move_uniforms_share_blocks_like_the_site_uniforms_in_their_own_stream():
+    """Constrained pair move (stream tag 1, keyed on the leader): same 64-bit split as C-26, different stream."""
+    o = oracle.Oracle(16, 8, 8, seed=99)
+    for (x, y, z) in ((0, 0, 0), (2, 0, 0), (5, 3, 2), (7, 3, 2), (14, 7, 7)):
+        c = (x + y + z) & 1
+        first = (x & ~2) + 16 * (y + 8 * z)
+        r = [int(v) for v in oracle.philox4x32_10([first, 1 | (c << 8), 12, 0], [99, 0])]
+        w0, w1 = (r[2], r[3]) if x & 2 else (r[0], r[1])
+        want = (((w0 >> 9) + 0.5) / 2**23, (((w0 & 511) << 9) | (w1 & 511)) / 2**18, ((w1 >> 9) + 0.5) / 2**23)
+        assert o.pair_uniforms(x, y, z, c, 12) == want
+        assert o.pair_uniforms(x, y, z, c, 12) != o.site_uniforms(x, y, z, c, 12)
+
+
 def test_random_start_is_uniform_on_the_sphere_and_seeded():
     o = oracle.Oracle(24, 20, 16, seed=7); o.init_random(); S = o.get_spins()
     n = len(S)
