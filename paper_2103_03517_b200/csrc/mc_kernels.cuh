@@ -405,8 +405,43 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
                 for (int k = 0; k + 1 < VEC; k += 2) philox4x32_10(key, q.site0 + 2u * k, c1, c2, c3, w0[k], w1[k], w0[k + 1], w1[k + 1]);
             }
         }
+        if (VEC == 4 && MODE == MODE_SWEEP) {
+            // ---- two sites at a time in the lanes of FFMA2 / FADD2 / FMUL2 (lane by lane the arithmetic of the scalar loop below)
+            const V3p B2 = splat3(B);
+            f2 f2s[6];
 #pragma unroll
-        for (int k = 0; k < VEC; ++k) {
+            for (int qq = 0; qq < 6; ++qq) f2s[qq] = splat(0.0f);
+#pragma unroll
+            for (int kp = 0; kp < 4; kp += 2) {
+                V3p S = { make_float2(sx.v[kp], sx.v[kp + 1]), make_float2(sy.v[kp], sy.v[kp + 1]), make_float2(sz.v[kp], sz.v[kp + 1]) };
+                const V3p hp = pack3(h[kp], h[kp + 1]);
+                const f2 J2 = splat(P.J);
+                const V3p hJ = { mul2(J2, hp.x), mul2(J2, hp.y), mul2(J2, hp.z) };
+                const V3p ep = (ANISO & 1) ? pack3(e[kp], e[kp + 1]) : B2;
+                V3p d, Sn;
+                cone_move2(S, omc, make_float2(uniform01(w0[kp]), uniform01(w0[kp + 1])),
+                           make_float2(uniform_azimuth(w0[kp], w1[kp]), uniform_azimuth(w0[kp + 1], w1[kp + 1])), d, Sn);
+                const V3p hB = { add2(hJ.x, B2.x), add2(hJ.y, B2.y), add2(hJ.z, B2.z) };
+                const f2 dE = delta_energy2<ANISO>(S, d, hB, P.Ku, ep, P.Kc);
+                const f2 xx = fma2(dE, splat(invT), make_float2(__logf(uniform01(w1[kp])), __logf(uniform01(w1[kp + 1]))));   // P:157-158 in log form (C-8)
+                const bool ok0 = xx.x < 0.0f, ok1 = xx.y < 0.0f;
+                S.x = make_float2(ok0 ? Sn.x.x : S.x.x, ok1 ? Sn.x.y : S.x.y);
+                S.y = make_float2(ok0 ? Sn.y.x : S.y.x, ok1 ? Sn.y.y : S.y.y);
+                S.z = make_float2(ok0 ? Sn.z.x : S.z.x, ok1 ? Sn.z.y : S.z.y);
+                nxv.v[kp] = S.x.x; nxv.v[kp + 1] = S.x.y; nyv.v[kp] = S.y.x; nyv.v[kp + 1] = S.y.y; nzv.v[kp] = S.z.x; nzv.v[kp + 1] = S.z.y;
+                cnt += (int)ok0 + (int)ok1;
+                if (dbg_x)   { dbg_x[q.site0 + 2u * kp] = xx.x; dbg_x[q.site0 + 2u * kp + 2u] = xx.y; }
+                if (dbg_acc) { dbg_acc[q.site0 + 2u * kp] = (uint8_t)ok0; dbg_acc[q.site0 + 2u * kp + 2u] = (uint8_t)ok1; }
+                f2s[0] = add2(f2s[0], S.x); f2s[1] = add2(f2s[1], S.y); f2s[2] = add2(f2s[2], S.z);
+                if (colour == 1) f2s[3] = sub2(f2s[3], dot3p(S, hJ));
+                if (ANISO) f2s[4] = add2(f2s[4], aniso_energy2<ANISO>(S, P.Ku, ep, P.Kc));
+                f2s[5] = sub2(f2s[5], dot3p(S, B2));
+            }
+#pragma unroll
+            for (int qq = 0; qq < 6; ++qq) f[qq] += f2s[qq].x + f2s[qq].y;
+        }
+#pragma unroll
+        for (int k = 0; k < ((VEC == 4 && MODE == MODE_SWEEP) ? 0 : VEC); ++k) {
             Vec3 S = { sx.v[k], sy.v[k], sz.v[k] };
             const Vec3 hJ = { P.J * h[k].x, P.J * h[k].y, P.J * h[k].z };
             if (MODE == MODE_SWEEP) {
