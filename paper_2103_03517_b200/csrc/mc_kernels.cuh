@@ -167,7 +167,7 @@ __device__ __forceinline__ void exchange_field(const Params& P, const ItemPos& q
         for (int k = 0; k < VEC; ++k) {
             // the second x-neighbour: next column if par = 1, previous column if par = 0
             const float sh = q.par ? ((k + 1 < VEC) ? o.v[(k + 1) % VEC] : ex) : ((k > 0) ? o.v[(k + VEC - 1) % VEC] : ex);
-            if (MASKED) {
+            if (MASKED && VEC != 4) {
                 const uint32_t mb = mbits[k];
                 // o.v[k] is the +x neighbour when par = 0 and the -x neighbour when par = 1
                 const uint32_t bit_o = q.par ? 2u : 1u, bit_s = q.par ? 1u : 2u;
@@ -183,15 +183,28 @@ __device__ __forceinline__ void exchange_field(const Params& P, const ItemPos& q
                 hc[c][k] = ((o.v[k] + sh) + (yp.v[k] + ym.v[k])) + (zp.v[k] + zm.v[k]);
             }
         }
-        if (!MASKED && VEC == 4) {
-            // the same sums two lanes at a time (the float4 loads are already aligned register pairs)
+        if (VEC == 4) {
+            // the same sums two lanes at a time (the float4 loads are already aligned register pairs); a masked bond is a
+            // factor 0 or 1 in an FFMA2 (same value and rounding as adding the neighbour or adding 0)
             const float s0 = q.par ? o.v[1] : ex, s1 = q.par ? o.v[2] : o.v[0], s2 = q.par ? o.v[3] : o.v[1], s3 = q.par ? ex : o.v[2];
 #pragma unroll
             for (int h2 = 0; h2 < 2; ++h2) {
                 const int a = 2 * h2, b = 2 * h2 + 1;
                 const f2 sh2 = h2 ? make_float2(s2, s3) : make_float2(s0, s1);
-                const f2 r = add2(add2(add2(make_float2(o.v[a], o.v[b]), sh2), add2(make_float2(yp.v[a], yp.v[b]), make_float2(ym.v[a], ym.v[b]))),
-                                  add2(make_float2(zp.v[a], zp.v[b]), make_float2(zm.v[a], zm.v[b])));
+                f2 r;
+                if (MASKED) {
+                    const uint32_t bo = q.par ? 1u : 0u, bs = q.par ? 0u : 1u;      // bit index of o's bond / sh's bond
+                    auto mf = [&](uint32_t bit) { return make_float2((mbits[a] & (1u << bit)) ? 1.0f : 0.0f, (mbits[b] & (1u << bit)) ? 1.0f : 0.0f); };
+                    r = mul2(mf(bo), make_float2(o.v[a], o.v[b]));
+                    r = fma2(mf(bs), sh2, r);
+                    r = fma2(mf(2u), make_float2(yp.v[a], yp.v[b]), r);
+                    r = fma2(mf(3u), make_float2(ym.v[a], ym.v[b]), r);
+                    r = fma2(mf(4u), make_float2(zp.v[a], zp.v[b]), r);
+                    r = fma2(mf(5u), make_float2(zm.v[a], zm.v[b]), r);
+                } else {
+                    r = add2(add2(add2(make_float2(o.v[a], o.v[b]), sh2), add2(make_float2(yp.v[a], yp.v[b]), make_float2(ym.v[a], ym.v[b]))),
+                             add2(make_float2(zp.v[a], zp.v[b]), make_float2(zm.v[a], zm.v[b])));
+                }
                 hc[c][a] = r.x; hc[c][b] = r.y;
             }
         }
