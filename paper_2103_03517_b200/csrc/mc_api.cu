@@ -222,10 +222,11 @@ bool plan_tile(mc_ctx* c)
     return c->tile_ok;
 }
 
-int grid_for(const mc_ctx* c, uint32_t n_threads_needed)
+// grid of a grid-stride kernel: one resident wave (the CTAs per SM its launch bounds allow) unless the environment overrides
+int grid_for(const mc_ctx* c, uint32_t n_threads_needed, int resident_per_sm)
 {
     const long long need = ((long long)n_threads_needed + BLOCK - 1) / BLOCK;
-    long long cap = (long long)c->sm_count * c->blocks_per_sm;
+    long long cap = (long long)c->sm_count * (c->blocks_per_sm > 0 ? c->blocks_per_sm : resident_per_sm);
     if (cap > c->P.max_blocks) cap = c->P.max_blocks;
     long long g = need < cap ? need : cap;
     return (int)(g < 1 ? 1 : g);
@@ -259,7 +260,7 @@ int launch_pass(mc_ctx* ctx, int mode, int colour, float invT, int flags, float*
     }
     PassFn fn = (ctx->vec == 4) ? (mode == MODE_SWEEP ? pick_pass<4, MODE_SWEEP>(ctx->aniso, ctx->masked) : pick_pass<4, MODE_MEASURE>(ctx->aniso, ctx->masked))
                                 : (mode == MODE_SWEEP ? pick_pass<1, MODE_SWEEP>(ctx->aniso, ctx->masked) : pick_pass<1, MODE_MEASURE>(ctx->aniso, ctx->masked));
-    const int grid = grid_for(ctx, ctx->geom.n_items);
+    const int grid = grid_for(ctx, ctx->geom.n_items, MC_PASS_MIN_BLOCKS);
     // measurement uses partial slots 2,3 so that it never disturbs a sweep assembled from the half-sweep hooks
     CU(launch_dependent(fn, grid, BLOCK, 0, ctx->stream, ctx->P, ctx->geom, colour, invT, flags, dx, da));
     ctx->launches += 1;
@@ -269,7 +270,7 @@ int launch_pass(mc_ctx* ctx, int mode, int colour, float invT, int flags, float*
 int launch_pair(mc_ctx* ctx, int colour, float invT, int flags, float* dx, uint8_t* da)
 {
     PairFn fn = (ctx->vec == 4) ? pick_pair<4>(ctx->aniso, ctx->masked) : pick_pair<1>(ctx->aniso, ctx->masked);
-    const int grid = grid_for(ctx, ctx->pgeom.n_threads);
+    const int grid = grid_for(ctx, ctx->pgeom.n_threads, MC_PAIR_MIN_BLOCKS);
     CU(launch_dependent(fn, grid, BLOCK, 0, ctx->stream, ctx->P, ctx->pgeom, colour, invT, flags, dx, da));
     ctx->launches += 1;
     return MC_OK;
@@ -337,7 +338,7 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     double n = sqrt(ham->eu[0] * ham->eu[0] + ham->eu[1] * ham->eu[1] + ham->eu[2] * ham->eu[2]);
     for (int a = 0; a < 3; ++a) { ctx->eu[a] = n > 0 ? ham->eu[a] / n : (a == 2 ? 1.0 : 0.0); ctx->B[a] = ham->B[a]; }
     ctx->stream = (cudaStream_t)cuda_stream;
-    ctx->blocks_per_sm = 4;
+    ctx->blocks_per_sm = 0;                                    // 0: one resident wave per kernel (grid_for)
     if (const char* env = getenv("MC_B200_BLOCKS_PER_SM")) { int v = atoi(env); if (v >= 1 && v <= 32) ctx->blocks_per_sm = v; }
 
     auto bail = [&](int code, const char* msg) { fprintf(stderr, "mc_create: %s\n", msg); delete ctx; return code; };

@@ -372,7 +372,7 @@ __device__ __forceinline__ bool last_block_done(DevState* st)
 // E_exch = -sum_{i black} S_i.h_i with h already in registers (0 extra bytes).
 // --------------------------------------------------------------------------------------------------------------
 #ifndef MC_PASS_MIN_BLOCKS
-#define MC_PASS_MIN_BLOCKS 2      // <= 128 registers: two CTAs per SM (c5 film: 354 -> 224 us per sweep)
+#define MC_PASS_MIN_BLOCKS 3      // <= 80 registers: three CTAs per SM (c5 film: one 354, two 185, three 166 us per sweep)
 #endif
 template <int VEC, int ANISO, bool MASKED, int MODE>
 __global__ void __launch_bounds__(BLOCK, MC_PASS_MIN_BLOCKS)
