@@ -243,7 +243,7 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
                 const f2 nt1x = fma2(q, uu, splat(-1.0f));
                 const f2 nt1y = mul2(q, vv);
                 const f2 nt2x = mul2(Sy, uu);
-                const f2 nt2y = fma2(Sy, vv, make_float2(-sg.x, -sg.y));
+                const f2 nt2y = fma2(Sy, vv, make_float2(xor_sign(-1.0f, Sz.x), xor_sign(-1.0f, Sz.y)));   // - sg, on the integer pipe
                 const f2 dx = fma2(Cc, nt1x, fma2(Ss, nt2x, mul2(nw, Sx)));
                 const f2 dy = fma2(Cc, nt1y, fma2(Ss, nt2y, mul2(nw, Sy)));
                 const f2 dz = fma2(Cc, q,    fma2(Ss, Sy,   mul2(nw, Sz)));
@@ -270,7 +270,7 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
                     const f2 S2x = mul2(Sx, Sx), S2y = mul2(Sy, Sy), S2z = mul2(Sz, Sz);
                     s4S = fma2(S2x, S2x, fma2(S2y, S2y, mul2(S2z, S2z)));
                     s4v = fma2(V2x, V2x, fma2(V2y, V2y, mul2(V2z, V2z)));
-                    dE = fma2(nhKc2, add2(s4v, make_float2(-s4S.x, -s4S.y)), dE);
+                    dE = fma2(nhKc2, sub2(s4v, s4S), dE);
                 }
 
                 const f2 u2 = add2(f2u, nCU2);
