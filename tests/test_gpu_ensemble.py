@@ -268,11 +268,13 @@ def test_full_size_c5_half_sweep_parity(mods):
     _full_size_half_sweep(mods, shape, 0.5, 0.8, 43, dict(periodic=(1, 1, 0), Ku=0.02, bond_mask=mask, region=region, region_axis=axes))
 
 
-def test_full_size_c4_constrained_half_sweep_parity(mods):
-    """config c4: 128^3, K_u = 0.05, constrained pass at theta = 45 deg."""
+@pytest.mark.parametrize("L", [128, 224])
+def test_full_size_c4_constrained_half_sweep_parity(mods, L):
+    """config c4: 128^3, K_u = 0.05, constrained pass at theta = 45 deg; and the same pass on the 224^3 lattice on which
+    bench.py times the constrained sweeps (other_paths)."""
     oracle, binding, inputs = mods
-    shape, T, theta = (128, 128, 128), 0.8, np.pi / 4
-    N = 128 ** 3
+    shape, T, theta = (L, L, L), 0.8, np.pi / 4
+    N = L ** 3
     e = np.array([np.sin(theta), 0.0, np.cos(theta)])
     g = binding.Lattice(*shape, Ku=0.05, cone0=0.6, adaptive=False, seed=42)
     o = oracle.Oracle(*shape, Ku=0.05, cone0=0.6, adaptive=False, seed=42)
@@ -287,9 +289,9 @@ def test_full_size_c4_constrained_half_sweep_parity(mods):
     assert (lead == ~np.isnan(x_g)).all()                                  # identical pairing roles at full size
     differ = lead & (acc_g != acc_o)
     assert (np.abs(x_o[differ]) < 1e-5).all()
-    s = np.arange(N); col = ((s % 128) + (s // 128) % 128 + s // (128 * 128)) & 1
+    s = np.arange(N); col = ((s % L) + (s // L) % L + s // (L * L)) & 1
     same = (acc_g == acc_o) & (col == 0)
     assert np.abs(after_g[same] - after_o[same]).max() < 1e-4
     fin = lead & np.isfinite(x_o) & np.isfinite(x_g)
-    print(f"\nfull size c4 constrained: pairs {lead.sum()}, accepted {acc_g[lead].mean():.3f}, flips {differ.sum()}, max |dx| {np.abs(x_g[fin]-x_o[fin]).max():.2e}")
+    print(f"\nfull size {L}^3 constrained: pairs {lead.sum()}, accepted {acc_g[lead].mean():.3f}, flips {differ.sum()}, max |dx| {np.abs(x_g[fin]-x_o[fin]).max():.2e}")
     g.close()
