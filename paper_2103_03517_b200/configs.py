@@ -1,0 +1,119 @@
+"""The five workloads of BASELINE.json, run in full through the library (python -m paper_2103_03517_b200.configs).
+
+Every schedule is the one BASELINE.json / SURVEY.md 8(d) states (no shortening: on a B200 all five together take well
+under a minute of device time); inputs are seeded and synthetic (paper_2103_03517_b200/inputs.py).  Prints one JSON
+object per config with the outputs the config names (per-sweep acceptance and m; m(T), susceptibilities and T_C from the
+susceptibility peak; throughput; torque versus theta and K(T); film m(T)) next to what the paper prints for the same
+physics where it prints something (P:44 T_C and beta, P:52 anisotropy exponent).  Host analysis: analysis.py.
+"""
+from __future__ import annotations
+
+import json
+import sys
+import time
+
+import numpy as np
+
+from . import analysis, binding, inputs
+
+
+def _sync():
+    import torch
+    torch.cuda.synchronize()
+
+
+def c1(device="cuda:0"):
+    g = binding.Lattice(16, 16, 16, Ku=0.01, cone0=0.5, adaptive=True, seed=42, device=device)
+    g.sweep(1.0, 1000)
+    tr = g.trace()
+    out = {"config": "c1 16^3, Ku=0.01, T=1.0, 1000 sweeps, +z start, adaptive cone from 0.5 rad",
+           "acceptance_first_10": [round(v, 4) for v in tr[:10, 0]], "acceptance_last_500_mean": float(tr[-500:, 0].mean()),
+           "cone_rad_final": float(g.observables().cone_rad),
+           "m_last_500_mean": float(np.linalg.norm(tr[-500:, 2:5], axis=1).mean())}
+    g.close()
+    return out
+
+
+def c2(device="cuda:0", L=64, equil=5000, sample=5000):
+    Ts = [0.1 * k for k in range(1, 17)]
+    m, chi_l, chi_t = [], [], []
+    for k, T in enumerate(Ts, start=1):
+        g = binding.Lattice(L, L, L, Ku=0.01, cone0=0.5, adaptive=True, seed=42 + k, device=device)   # +z start at every T
+        g.sweep(T, equil); g.reset_accumulators(); g.sweep(T, sample)
+        ob = g.observables()
+        chi = analysis.susceptibilities(ob, T)
+        m.append(ob.sum_m[0] / ob.n_samples); chi_l.append(float(chi[0])); chi_t.append(float(0.5 * (chi[1] + chi[2])))
+        g.close()
+    tc_peak = Ts[int(np.argmax(chi_l))]
+    below = [i for i, T in enumerate(Ts) if T < tc_peak and m[i] > 0.3]
+    tc_fit, beta, _ = analysis.fit_bloch([Ts[i] for i in below], [m[i] for i in below])
+    return {"config": f"c2 {L}^3, Ku=0.01, T=0.1..1.6, {equil}+{sample} sweeps per point", "T": Ts, "m": m, "chi_longitudinal": chi_l,
+            "chi_transverse": chi_t, "Tc_from_chi_peak": tc_peak, "bloch_fit": {"Tc": tc_fit, "beta": beta},
+            "paper": {"kB_Tc_over_J": 1.4451, "beta": 0.340, "where": "P:44 (50 nm^3 mesh, 8 M spins)"}}
+
+
+def c3(device="cuda:0", L=224, sweeps=2000):
+    import torch
+    N = L ** 3
+    out = {"config": f"c3 {L}^3, Kc=0.01, T in (0.5, 1.2, 1.44), {sweeps} sweeps each from a seeded random-sphere start", "points": []}
+    for T in (0.5, 1.2, 1.44):
+        g = binding.Lattice(L, L, L, Kc=0.01, cone0=0.5, adaptive=True, seed=42, device=device)
+        g.init_spins(2)
+        g.sweep(T, sweeps // 2); _sync()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(); g.sweep(T, sweeps - sweeps // 2); e1.record(); _sync()
+        ob = g.observables()
+        out["points"].append({"T": T, "m": ob.m, "E_per_site": ob.E_total, "acceptance": ob.last_acceptance, "cone_rad": ob.cone_rad,
+                              "updates_per_s_last_half": N * (sweeps - sweeps // 2) / (e0.elapsed_time(e1) * 1e-3)})
+        g.close()
+    return out
+
+
+def c4(device="cuda:0", L=128, sweeps=5000, discard=1000):
+    thetas = np.deg2rad(np.arange(0, 91, 9))                  # 0..90 deg in 10 steps (C-20)
+    out = {"config": f"c4 {L}^3, Ku=0.05, constrained, theta=0..90 deg (11 points), T in (0.3, 0.8, 1.2), {sweeps} sweeps per point", "points": []}
+    Ks, ms = [], []
+    for T in (0.3, 0.8, 1.2):
+        tau, mm = [], []
+        for th in thetas:
+            g = binding.Lattice(L, L, L, Ku=0.05, cone0=0.5, adaptive=True, seed=42, device=device)   # +z, rotated onto e_C (C-12)
+            g.constrained_sweep(T, th, 0.0, discard); g.reset_accumulators(); g.constrained_sweep(T, th, 0.0, sweeps - discard)
+            ob = g.observables()
+            tau.append(ob.sum_torque[1] / ob.n_samples); mm.append(ob.sum_m[0] / ob.n_samples)
+            g.close()
+        fit = thetas <= np.deg2rad(45.5)                     # towards the hard plane the uniform state of so large a lattice is not
+        K = analysis.anisotropy_from_torque(thetas[fit], np.array(tau)[fit])   # stable over 5000 sweeps (|M| drops, domains): fit the stable branch
+        Ks.append(K); ms.append(float(np.mean(np.array(mm)[fit])))
+        out["points"].append({"T": T, "torque_y": tau, "m_of_theta": mm, "m": ms[-1], "K_fit_theta_le_45deg": K})
+    k, K0 = analysis.power_law_exponent(np.array(ms), np.array(Ks))
+    out["K_over_m_exponent"] = k; out["K0_extrapolated"] = K0
+    out["paper"] = {"uniaxial_exponent": 2.95, "where": "P:52 (Callen-Callen: 3)"}
+    return out
+
+
+def c5(device="cuda:0", nx=2048, ny=2048, nz=4, sweeps=3000):
+    mask, region, axes = inputs.voronoi_film(nx, ny, nz, 40, seed=42)
+    g = binding.Lattice(nx, ny, nz, periodic=(1, 1, 0), Ku=0.02, bond_mask=mask, region=region, region_axis=axes,
+                        cone0=0.5, adaptive=True, seed=42, device=device)
+    Ts, m = [0.1 * k for k in range(1, 16)], []
+    for T in Ts:                                              # increasing sweep, state and cone carried over
+        g.sweep(T, sweeps - 1000); g.reset_accumulators(); g.sweep(T, 1000)
+        ob = g.observables(); m.append(ob.sum_m[0] / ob.n_samples)
+    g.close()
+    return {"config": f"c5 {nx}x{ny}x{nz} granular film, {axes.shape[0]} grains, Ku=0.02 per-grain axes, T=0.1..1.5, {sweeps} sweeps each", "T": Ts, "m": m}
+
+
+def main(argv=None):
+    names = (argv or sys.argv[1:]) or ["c1", "c2", "c3", "c4", "c5"]
+    table = {"c1": c1, "c2": c2, "c3": c3, "c4": c4, "c5": c5}
+    for n in names:
+        t0 = time.perf_counter()
+        res = table[n]()
+        _sync()
+        res["wall_s"] = round(time.perf_counter() - t0, 2)
+        print(json.dumps(res), flush=True)
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
