@@ -228,11 +228,6 @@ __device__ __forceinline__ void easy_axes(const Params& P, const ItemPos& q, int
 }
 
 // --------------------------------------------------------------------------------------------------------------
-// Block reduction of the per-thread fused sums in a FIXED order (deterministic two-pass fp64 reduction, pass 1):
-// lanes by xor-shuffle, warps sequentially; thread 0 writes the block partial.
-// --------------------------------------------------------------------------------------------------------------
-
-// --------------------------------------------------------------------------------------------------------------
 // Fused sums (a-9), pass 1.  A thread carries fp32 partial sums over a small bounded set of sites, converts them ONCE to
 // 64-bit fixed point (unit 2^-k) and from there on every addition is an integer addition: exact, hence independent of
 // the order (warp shuffles, warps of a block, one 64-bit atomic per block and quantity) and bitwise reproducible.

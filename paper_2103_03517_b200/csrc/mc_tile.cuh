@@ -13,7 +13,7 @@
 //     (one issue slot for two sites); Philox, MUFU and the selects stay scalar.
 //   * Own colour: LDG.64 / STG.64 straight from/to the colour-split planes (read once, written once).
 //   * Fused sums (a-9) are carried per thread in fp32 over its <= 2*NPASS*Lz sites (a bounded, fixed set), converted to
-//     fp64 once, then reduced in a fixed order (deterministic two-pass reduction, pass 1).
+//     64-bit fixed point once, then summed exactly (block_reduce: order-independent, reproducible); fp64 in final_reduce.
 // Arithmetic contract: identical to pass_kernel / DESIGN.md section 3 (same Philox stream, same cone construction).
 #pragma once
 
