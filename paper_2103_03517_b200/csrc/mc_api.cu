@@ -213,9 +213,13 @@ bool plan_tile(mc_ctx* c)
     if (want_segs > 0 && want_segs <= lat.nz) n_segs = want_segs;
     G.n_segs = n_segs; G.Lz = lat.nz / n_segs; G.Lz_rem = lat.nz % n_segs;
     if ((long long)G.n_slabs * G.n_segs > c->P.max_blocks) return false;
-    c->tile_ok = true;
-    if (const char* env = getenv("MC_B200_PATH")) { if (!strcmp(env, "generic")) c->tile_ok = false; }
-    else if (c->P.Nc < 65536u) c->tile_ok = false;              // small lattices are launch-bound: the generic kernel has less prologue
+    // Default: the tiled pass runs where it has a compile-time-row-length instantiation (R = 32, 64, 112 in the specialised slab
+    // shape: 64^3, 128^3, 224^3 of BASELINE.json); everywhere else the generic pass is faster since it went packed and to three
+    // CTAs per SM (measured: 96^3 16.3 vs 18.5 us per sweep, 160^3 40 vs 49, 256^3 148 vs 164, 512^3 1222 vs 1285).
+    // MC_B200_PATH=tile forces the tiled pass wherever the geometry allows it (tests), =generic forces the generic one.
+    const bool specialised = (R == 32 || R == 64 || R == 112) && G.Ty == TILE_TY_RT && G.NPASS == TILE_NPASS_RT && !c->P.anti_x;
+    c->tile_ok = specialised && c->P.Nc >= 65536u;             // small lattices are launch-bound: the generic kernel has less prologue
+    if (const char* env = getenv("MC_B200_PATH")) { c->tile_ok = !strcmp(env, "tile"); }
     if (getenv("MC_B200_VERBOSE"))
         fprintf(stderr, "mc tile plan: ok=%d R=%d PR=%d RP=%d NPASS=%d Ty=%d slabs=%d segs=%d Lz=%d(+%d) threads=%d smem=%zu ctas/SM=%d\n",
                 (int)c->tile_ok, R, PR, RP, NP, G.Ty, G.n_slabs, G.n_segs, G.Lz, G.Lz_rem, c->tile_threads, c->tile_smem, per_sm);

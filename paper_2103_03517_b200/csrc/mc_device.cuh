@@ -226,6 +226,42 @@ __device__ __forceinline__ f2 delta_energy2(const V3p& S, const V3p& d, const V3
     return dE;
 }
 
+// delta_energy2 that also hands back what the on-site energy of whichever spin is kept needs, so that it is not evaluated
+// again: cubic through s4 = sum_a S_a^4 of the old spin (s4S) and of the trial spin S + d (s4v) -- on the unit sphere
+// Sx^2Sy^2 + Sx^2Sz^2 + Sy^2Sz^2 = (1 - s4)/2, so dE_c = -Kc/2 (s4v - s4S) and E_c = Kc/2 (1 - s4); uniaxial through
+// (S.e)^2 (euS) and ((S+d).e)^2 (euv) with the difference in difference form.  E_onsite(kept) = onsite_from(...).
+template <int ANISO>
+__device__ __forceinline__ f2 delta_energy2_keep(const V3p& S, const V3p& d, const V3p& hB, float Ku, const V3p& e, float Kc,
+                                                 f2& s4S, f2& s4v, f2& euS, f2& euv)
+{
+    f2 dE = neg2(dot3p(d, hB));
+    s4S = s4v = euS = euv = splat(0.0f);
+    if (ANISO & 1) {
+        const f2 de = dot3p(d, e), se = dot3p(S, e);
+        const f2 du = mul2(de, fma2(splat(2.0f), se, de));           // ((S+d).e)^2 - (S.e)^2
+        dE = fma2(splat(-Ku), du, dE);
+        euS = mul2(se, se); euv = add2(euS, du);
+    }
+    if (ANISO & 2) {
+        const f2 vx = add2(S.x, d.x), vy = add2(S.y, d.y), vz = add2(S.z, d.z);
+        const f2 S2x = mul2(S.x, S.x), S2y = mul2(S.y, S.y), S2z = mul2(S.z, S.z);
+        const f2 V2x = mul2(vx, vx), V2y = mul2(vy, vy), V2z = mul2(vz, vz);
+        s4S = fma2(S2x, S2x, fma2(S2y, S2y, mul2(S2z, S2z)));
+        s4v = fma2(V2x, V2x, fma2(V2y, V2y, mul2(V2z, V2z)));
+        dE = fma2(splat(-0.5f * Kc), sub2(s4v, s4S), dE);
+    }
+    return dE;
+}
+// on-site energy of the kept spins from the pieces above: lane l keeps the trial spin iff ok_l
+template <int ANISO>
+__device__ __forceinline__ f2 onsite_from(bool ok0, bool ok1, f2 s4S, f2 s4v, f2 euS, f2 euv, float Ku, float Kc)
+{
+    f2 E = splat(0.0f);
+    if (ANISO & 1) E = mul2(splat(-Ku), make_float2(ok0 ? euv.x : euS.x, ok1 ? euv.y : euS.y));
+    if (ANISO & 2) E = fma2(splat(-0.5f * Kc), make_float2(ok0 ? s4v.x : s4S.x, ok1 ? s4v.y : s4S.y), add2(E, splat(0.5f * Kc)));
+    return E;
+}
+
 template <int ANISO>
 __device__ __forceinline__ f2 aniso_energy2(const V3p& S, float Ku, const V3p& e, float Kc)
 {

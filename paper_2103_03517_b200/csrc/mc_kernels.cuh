@@ -430,7 +430,8 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
                 cone_move2(S, omc, make_float2(uniform01(w0[kp]), uniform01(w0[kp + 1])),
                            make_float2(uniform_azimuth(w0[kp], w1[kp]), uniform_azimuth(w0[kp + 1], w1[kp + 1])), d, Sn);
                 const V3p hB = { add2(hJ.x, B2.x), add2(hJ.y, B2.y), add2(hJ.z, B2.z) };
-                const f2 dE = delta_energy2<ANISO>(S, d, hB, P.Ku, ep, P.Kc);
+                f2 s4S, s4v, euS, euv;
+                const f2 dE = delta_energy2_keep<ANISO>(S, d, hB, P.Ku, ep, P.Kc, s4S, s4v, euS, euv);
                 const f2 xx = fma2(dE, splat(invT), make_float2(__logf(uniform01(w1[kp])), __logf(uniform01(w1[kp + 1]))));   // P:157-158 in log form (C-8)
                 const bool ok0 = xx.x < 0.0f, ok1 = xx.y < 0.0f;
                 S.x = make_float2(ok0 ? Sn.x.x : S.x.x, ok1 ? Sn.x.y : S.x.y);
@@ -442,7 +443,7 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
                 if (dbg_acc) { dbg_acc[q.site0 + 2u * kp] = (uint8_t)ok0; dbg_acc[q.site0 + 2u * kp + 2u] = (uint8_t)ok1; }
                 f2s[0] = add2(f2s[0], S.x); f2s[1] = add2(f2s[1], S.y); f2s[2] = add2(f2s[2], S.z);
                 if (colour == 1) f2s[3] = sub2(f2s[3], dot3p(S, hJ));
-                if (ANISO) f2s[4] = add2(f2s[4], aniso_energy2<ANISO>(S, P.Ku, ep, P.Kc));
+                if (ANISO) f2s[4] = add2(f2s[4], onsite_from<ANISO>(ok0, ok1, s4S, s4v, euS, euv, P.Ku, P.Kc));
                 f2s[5] = sub2(f2s[5], dot3p(S, B2));
             }
 #pragma unroll
@@ -691,7 +692,7 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
                     const V3p hJi = { mul2(J2, hi.x), mul2(J2, hi.y), mul2(J2, hi.z) }, hJj = { mul2(J2, hj.x), mul2(J2, hj.y), mul2(J2, hj.z) };
                     f2s[3] = sub2(f2s[3], add2(dot3p(Si, hJi), dot3p(Snj, hJj)));
                 }
-                if (ANISO) f2s[4] = add2(f2s[4], add2(aniso_energy2<ANISO>(Si, P.Ku, ei, P.Kc), aniso_energy2<ANISO>(Snj, P.Ku, ej, P.Kc)));
+                if (ANISO) f2s[4] = add2(f2s[4], add2(aniso_energy2<ANISO>(Si, P.Ku, ei, P.Kc), aniso_energy2<ANISO>(Snj, P.Ku, ej, P.Kc)));   // (the pair pass has no registers for the kept-pieces variant)
                 f2s[5] = sub2(f2s[5], add2(dot3p(Si, B2), dot3p(Snj, B2)));
                 const V3p ti = onsite_torque2<ANISO>(Si, P.Ku, ei, P.Kc, B2), tj = onsite_torque2<ANISO>(Snj, P.Ku, ej, P.Kc, B2);
                 f2s[6] = add2(f2s[6], add2(ti.x, tj.x)); f2s[7] = add2(f2s[7], add2(ti.y, tj.y)); f2s[8] = add2(f2s[8], add2(ti.z, tj.z));

@@ -87,6 +87,16 @@ CASES = [
 ]
 
 
+# lattices on which the tiled pass is not the default (no compile-time row length, or anti-periodic) but must stay correct
+TILED_CASES = [c for c in CASES if c[0] in ((96, 40, 36), (80, 30, 58))]
+
+
+@pytest.mark.parametrize("shape,T,cone,ham", TILED_CASES)
+def test_half_sweep_parity_forced_tiled_pass(mods, shape, T, cone, ham, monkeypatch):
+    monkeypatch.setenv("MC_B200_PATH", "tile")                 # read by mc_create
+    test_half_sweep_parity_random_state(mods, shape, T, cone, ham)
+
+
 @pytest.mark.parametrize("shape,T,cone,ham", CASES)
 def test_half_sweep_parity_random_state(mods, shape, T, cone, ham):
     oracle, binding, inputs = mods
