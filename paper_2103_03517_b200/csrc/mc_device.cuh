@@ -186,25 +186,31 @@ __device__ __forceinline__ V3p splat3(const Vec3& a) { return { splat(a.x), spla
 __device__ __forceinline__ Vec3 lane3(const V3p& a, int l) { return l ? Vec3{ a.x.y, a.y.y, a.z.y } : Vec3{ a.x.x, a.y.x, a.z.x }; }
 __device__ __forceinline__ f2 dot3p(const V3p& a, const V3p& b) { return fma2(a.x, b.x, fma2(a.y, b.y, mul2(a.z, b.z))); }
 
+__device__ __forceinline__ float xor_sign(float a, float s) { return __uint_as_float(__float_as_uint(a) ^ (__float_as_uint(s) & 0x80000000u)); }   // a * copysign(1, s)
+
+// cone_move for two sites.  Same construction as the scalar function, written with the signs folded in (as the tiled pass
+// does): with phi - pi = ang, cos(phi) = -cos(ang), sin(phi) = -sin(ang), so d = sa (cos(ang) (-t1) + sin(ang) (-t2)) - w S,
+//   -t1 = (q uu - 1, q vv, q),  -t2 = (Sy uu, Sy vv - sg, Sy),  q = sg Sx,  uu = Sx / (sg + Sz),  vv = Sy / (sg + Sz).
 __device__ __forceinline__ void cone_move2(const V3p& S, float one_minus_cos, f2 u0, f2 u1, V3p& d, V3p& Sn)
 {
-    const f2 w  = mul2(u0, splat(one_minus_cos));
-    const f2 t  = mul2(w, sub2(splat(2.0f), w));
+    const f2 nw = mul2(u0, splat(-one_minus_cos));
+    const f2 t  = mul2(nw, fma2(nw, splat(-1.0f), splat(-2.0f)));                 // w (2 - w)
     const f2 sa = mul2(t, make_float2(rsqrtf(t.x), rsqrtf(t.y)));
     const f2 ang = fma2(u1, splat(6.2831853071795865f), splat(-3.1415926535897932f));
-    const f2 cp = make_float2(-__cosf(ang.x), -__cosf(ang.y)), sp = make_float2(-__sinf(ang.x), -__sinf(ang.y));
-    const f2 sg = make_float2(S.z.x >= 0.0f ? 1.0f : -1.0f, S.z.y >= 0.0f ? 1.0f : -1.0f);
+    const f2 Cc = mul2(sa, make_float2(__cosf(ang.x), __cosf(ang.y)));
+    const f2 Ss = mul2(sa, make_float2(__sinf(ang.x), __sinf(ang.y)));
+    const f2 sg = make_float2(copysignf(1.0f, S.z.x), copysignf(1.0f, S.z.y));
     const f2 den = add2(sg, S.z);
-    const f2 a  = make_float2(__fdividef(-1.0f, den.x), __fdividef(-1.0f, den.y));
-    const f2 b  = mul2(mul2(S.x, S.y), a);
-    const V3p t1 = { fma2(mul2(mul2(sg, S.x), S.x), a, splat(1.0f)), mul2(sg, b), neg2(mul2(sg, S.x)) };
-    const V3p t2 = { b, fma2(mul2(S.y, S.y), a, sg), neg2(S.y) };
-    const f2 ca = mul2(sa, cp), cb = mul2(sa, sp), nw = neg2(w);
-    d.x = fma2(ca, t1.x, fma2(cb, t2.x, mul2(nw, S.x)));
-    d.y = fma2(ca, t1.y, fma2(cb, t2.y, mul2(nw, S.y)));
-    d.z = fma2(ca, t1.z, fma2(cb, t2.z, mul2(nw, S.z)));
+    const f2 ia = make_float2(__fdividef(1.0f, den.x), __fdividef(1.0f, den.y));
+    const f2 uu = mul2(S.x, ia), vv = mul2(S.y, ia);
+    const f2 q  = make_float2(xor_sign(S.x.x, S.z.x), xor_sign(S.x.y, S.z.y));    // sg Sx, on the integer pipe
+    const f2 nt1x = fma2(q, uu, splat(-1.0f)), nt1y = mul2(q, vv);
+    const f2 nt2x = mul2(S.y, uu), nt2y = fma2(S.y, vv, make_float2(xor_sign(-1.0f, S.z.x), xor_sign(-1.0f, S.z.y)));
+    d.x = fma2(Cc, nt1x, fma2(Ss, nt2x, mul2(nw, S.x)));
+    d.y = fma2(Cc, nt1y, fma2(Ss, nt2y, mul2(nw, S.y)));
+    d.z = fma2(Cc, q,    fma2(Ss, S.y,  mul2(nw, S.z)));
     const V3p v = { add2(S.x, d.x), add2(S.y, d.y), add2(S.z, d.z) };
-    const f2 inv = fma2(splat(-0.5f), dot3p(v, v), splat(1.5f));
+    const f2 inv = fma2(dot3p(v, v), splat(-0.5f), splat(1.5f));
     Sn = { mul2(v.x, inv), mul2(v.y, inv), mul2(v.z, inv) };
 }
 

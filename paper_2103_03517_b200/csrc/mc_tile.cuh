@@ -102,8 +102,7 @@ __device__ __forceinline__ void tile_issue_plane(const TileGeom& G, int R, const
 
 // u = f - (1 - 2^-24) with f = 1 + (w >> 9) 2^-23 in [1,2): one funnel shift builds f (C-8)
 __device__ __forceinline__ float mantissa_1p(uint32_t w) { return __uint_as_float(__funnelshift_r(w, 0x7Fu, 9)); }
-// a with the sign of s folded in: a * copysign(1, s), on the integer pipe
-__device__ __forceinline__ float xor_sign(float a, float s) { return __uint_as_float(__float_as_uint(a) ^ (__float_as_uint(s) & 0x80000000u)); }
+// (xor_sign: mc_device.cuh)
 
 // ANISO: bit 0 uniaxial (uniform axis), bit 1 cubic.  FIELD: Zeeman term.  RT: colour-sites per row as a compile-time
 // constant (0 = run-time value; the specialisations turn every shared-memory offset into an immediate).
