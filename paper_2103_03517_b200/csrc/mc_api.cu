@@ -146,7 +146,7 @@ template <int RT, bool DEBUG, bool ANTI = false> TileFn pick_tile_rt(int aniso, 
     }
 }
 // Row lengths with a specialised instantiation (every shared-memory offset an immediate): R = nx/2 of BASELINE's
-// periodic configs c2 (64^3), c4 (128^3) and c3 (224^3).  Any other R runs the run-time-R instantiation.
+// periodic configs c2 (64^3), c4 (128^3) and c3 (224^3), plus 192^3 (R = 96: 58 against 65 us per sweep for the generic pass).  Any other R runs the run-time-R instantiation.
 // The decision-variable debug outputs of the test hooks exist only in the run-time-R instantiation (same arithmetic).
 TileFn pick_tile(int R, int Ty, int npass, bool debug, int aniso, bool field, bool anti)
 {
@@ -155,6 +155,7 @@ TileFn pick_tile(int R, int Ty, int npass, bool debug, int aniso, bool field, bo
     if (getenv("MC_B200_NO_RT") || Ty != TILE_TY_RT || npass != TILE_NPASS_RT) return pick_tile_rt<0, false>(aniso, field);
     switch (R) {
         case 32:  return pick_tile_rt<32, false>(aniso, field);
+        case 96:  return pick_tile_rt<96, false>(aniso, field);
         case 64:  return pick_tile_rt<64, false>(aniso, field);
         case 112: return pick_tile_rt<112, false>(aniso, field);
         default:  return pick_tile_rt<0, false>(aniso, field);
@@ -185,8 +186,8 @@ bool plan_tile(mc_ctx* c)
     const size_t smem_cap = (size_t)(220 * 1024) / TILE_MIN_BLOCKS - 3 * 1024;   // TILE_MIN_BLOCKS CTAs per SM
     auto slot_bytes = [&](int ty) { return (size_t)3 * (ty + 2) * R * sizeof(float); };
     if (lat.ny % (2 * RP) == 0 && TILE_NSLOT * slot_bytes(2 * RP) <= smem_cap) NP = 2;
-    // row lengths with a compile-time specialisation (R = 32, 64, 112) take its slab shape when it fits: 64^3 13.3 -> 11.3 us per sweep
-    if ((R == 32 || R == 64 || R == 112) && lat.ny % TILE_TY_RT == 0 && PR * (TILE_TY_RT / TILE_NPASS_RT) <= max_threads) {
+    // row lengths with a compile-time specialisation (R = 32, 64, 96, 112) take its slab shape when it fits: 64^3 13.3 -> 11.3 us per sweep
+    if ((R == 32 || R == 64 || R == 96 || R == 112) && lat.ny % TILE_TY_RT == 0 && PR * (TILE_TY_RT / TILE_NPASS_RT) <= max_threads) {
         RP = TILE_TY_RT / TILE_NPASS_RT; NP = TILE_NPASS_RT;
     }
     if (want_rp > 0 && lat.ny % want_rp == 0 && PR * want_rp <= TILE_MAX_THREADS) { RP = want_rp; NP = 1; if (lat.ny % (2 * RP) == 0 && TILE_NSLOT * slot_bytes(2 * RP) <= smem_cap) NP = 2; }
@@ -213,11 +214,11 @@ bool plan_tile(mc_ctx* c)
     if (want_segs > 0 && want_segs <= lat.nz) n_segs = want_segs;
     G.n_segs = n_segs; G.Lz = lat.nz / n_segs; G.Lz_rem = lat.nz % n_segs;
     if ((long long)G.n_slabs * G.n_segs > c->P.max_blocks) return false;
-    // Default: the tiled pass runs where it has a compile-time-row-length instantiation (R = 32, 64, 112 in the specialised slab
-    // shape: 64^3, 128^3, 224^3 of BASELINE.json); everywhere else the generic pass is faster since it went packed and to three
+    // Default: the tiled pass runs where it has a compile-time-row-length instantiation (R = 32, 64, 96, 112 in the specialised slab
+    // shape: 64^3, 128^3, 224^3 of BASELINE.json, and 192^3); everywhere else the generic pass is faster since it went packed and to three
     // CTAs per SM (measured: 96^3 16.3 vs 18.5 us per sweep, 160^3 40 vs 49, 256^3 148 vs 164, 512^3 1222 vs 1285).
     // MC_B200_PATH=tile forces the tiled pass wherever the geometry allows it (tests), =generic forces the generic one.
-    const bool specialised = (R == 32 || R == 64 || R == 112) && G.Ty == TILE_TY_RT && G.NPASS == TILE_NPASS_RT && !c->P.anti_x;
+    const bool specialised = (R == 32 || R == 64 || R == 96 || R == 112) && G.Ty == TILE_TY_RT && G.NPASS == TILE_NPASS_RT && !c->P.anti_x;
     c->tile_ok = specialised && c->P.Nc >= 65536u;             // small lattices are launch-bound: the generic kernel has less prologue
     if (const char* env = getenv("MC_B200_PATH")) { c->tile_ok = !strcmp(env, "tile"); }
     if (getenv("MC_B200_VERBOSE"))

@@ -196,6 +196,29 @@ def test_observables_match_oracle(mods):
     g.close()
 
 
+@pytest.mark.parametrize("shape", [(64, 64, 64), (128, 32, 32), (192, 32, 24)])
+def test_compile_time_row_length_instantiations_match_the_checked_one(mods, shape):
+    """R = 32, 64, 96 (R = 112: the 224^3 test): the instantiation mc_sweep launches writes no decision variable, so it is
+    compared bit for bit with the run-time-row-length instantiation that does and that the oracle parity cases go through."""
+    oracle, binding, inputs = mods
+    s0 = inputs.random_unit_spins(shape[0] * shape[1] * shape[2], seed=21)
+    g = binding.Lattice(*shape, Ku=0.02, Kc=0.1, B=(0.05, 0.0, -0.1), cone0=0.8, adaptive=False, seed=3)
+    out = []
+    for detail in (False, True):
+        g.set_spins(s0); g.set_sweep(41)
+        for colour in (0, 1):
+            g.half_sweep(0.9, colour, want_detail=detail)
+        out.append(g.get_spins())
+    assert (out[0] == out[1]).all() and not (out[0] == s0).all()
+    o = oracle.Oracle(*shape, Ku=0.02, Kc=0.1, B=(0.05, 0.0, -0.1), cone0=0.8, adaptive=False, seed=3)
+    g.set_spins(s0); g.set_sweep(41); o.set_sweep(41); o.set_spins(g.get_spins())
+    _, x_o, _ = o.half_sweep(0.9, 0, want_detail=True)
+    g.half_sweep(0.9, 0)
+    bad = np.abs(g.get_spins().astype(np.float64) - o.get_spins()).max(axis=1) >= SPIN_TOL
+    assert (np.abs(x_o[bad]) < X_BAND).all()
+    g.close()
+
+
 def test_tiled_pass_fused_sums_match_a_fresh_measurement(mods):
     """The tiled pass forms the on-site energies of the final spin from the dE terms (s4 identity, (S.e)^2 difference form)
     and sums in 64-bit fixed point: its per-sweep M and E must equal a standalone measurement of the same state, and the
