@@ -249,7 +249,7 @@ def run_ours(args, rank, local_rank, world):
     t_launch = ms * 1e-3 / launches                       # average duration of one colour-pass launch over the timed region
     alg_bytes_per_launch = BYTES_PER_UPDATE * (N // 2)    # one launch updates one colour
     achieved = alg_bytes_per_launch / t_launch / 1e9
-    roofline = {"bound": "hbm", "kernel": "pass_kernel (one colour pass)", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    roofline = {"bound": "hbm", "kernel": "tile_pass_kernel<ANISO=2, FIELD=0, RT=112> (one colour pass = one launch)", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": recorded_traffic(), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes_per_launch, "avg_launch_us": t_launch * 1e6,
                 "frac_of_nominal_8TBs": achieved / 8000.0}
