@@ -43,6 +43,7 @@ struct orc_ctx {
     /* constrained state */
     int aligned; double eC[3];
     int sampling;           /* 1 = measure + trace + accumulate after every sweep (default) */
+    int torque_sampling;    /* 1 only inside orc_constrained_sweep: the torque is the constrained method's observable */
 };
 
 /* ------------------------------------------------------------------ Philox4x32-10 (pin P-1) */
@@ -86,8 +87,10 @@ void orc_cone_move(const double S[3], double theta, double u0, double u1, double
     double w = u0 * (1.0 - cos(theta));
     double sa = sqrt(w * (2.0 - w));
     double phi = 2.0 * PI * u1;
-    /* orthonormal frame (t1,t2) perpendicular to S (Duff et al. 2017 construction) */
-    double sg = (S[2] >= 0.0) ? 1.0 : -1.0;
+    /* orthonormal frame (t1,t2) perpendicular to S (Duff et al. 2017 construction).  sigma = sign of S_z taken from the
+     * SIGN BIT (reading C-29): S_z = -0.0 gives sigma = -1; either frame is a valid frame (sigma + S_z = -1, no
+     * singularity), the reading only fixes which one so that every implementation proposes the same trial spin. */
+    double sg = signbit(S[2]) ? -1.0 : 1.0;
     double a = -1.0 / (sg + S[2]);
     double b = S[0] * S[1] * a;
     double t1[3] = { 1.0 + sg * S[0] * S[0] * a, sg * b, -sg * S[0] };
@@ -300,6 +303,7 @@ static int metropolis_update(orc_ctx* c, int x, int y, int z, int colour, double
 int64_t orc_half_sweep(orc_ctx* c, double T, int colour, double* xdec, uint8_t* acc)
 {
     int64_t count = 0;
+    c->aligned = 0;   /* an unconstrained pass moves M off e_C: the next constrained sweep re-aligns (reading C-12) */
     for (int z = 0; z < c->nz; ++z) for (int y = 0; y < c->ny; ++y) for (int x = 0; x < c->nx; ++x) {
         if (((x + y + z) & 1) != colour) continue;            /* red = even (C-10) */
         int a = metropolis_update(c, x, y, z, colour, T, xdec);
@@ -372,7 +376,7 @@ void orc_end_sweep(orc_ctx* c, int64_t count)
     double mv[4] = { o.m, o.M[0], o.M[1], o.M[2] };
     for (int a = 0; a < 4; ++a) { c->sum_m[a] += mv[a]; c->sum_m2[a] += mv[a] * mv[a]; }
     c->sum_E += o.E_total; c->sum_E2 += o.E_total * o.E_total;
-    for (int a = 0; a < 3; ++a) c->sum_torque[a] += o.torque[a];
+    if (c->torque_sampling) for (int a = 0; a < 3; ++a) c->sum_torque[a] += o.torque[a];   /* constrained sweeps only */
     c->n_samples += 1;
     if (c->trace_len == c->trace_cap) {
         c->trace_cap = c->trace_cap ? 2 * c->trace_cap : 1024;
@@ -395,6 +399,7 @@ void orc_sweep(orc_ctx* c, double T, int64_t n)
 void orc_sweep_random_order(orc_ctx* c, double T, int64_t n)
 {
     int64_t* order = (int64_t*)malloc(sizeof(int64_t) * c->N);
+    c->aligned = 0;   /* reading C-12, as in orc_half_sweep */
     for (int64_t it = 0; it < n; ++it) {
         for (int64_t i = 0; i < c->N; ++i) order[i] = i;
         for (int64_t i = c->N - 1; i > 0; --i) {
@@ -609,16 +614,18 @@ int orc_constrained_sweep(orc_ctx* c, double T, double theta, double phi, int64_
     double e[3] = { sin(theta) * cos(phi), sin(theta) * sin(phi), cos(theta) };
     if (!c->aligned || e[0] != c->eC[0] || e[1] != c->eC[1] || e[2] != c->eC[2])
         if (orc_align_to(c, e)) return -1;                                /* C-12 */
+    c->torque_sampling = 1;
     for (int64_t it = 0; it < n; ++it) {
         double ML = 0.0;
         for (int64_t i = 0; i < c->N; ++i) ML += c->S[3 * i] * e[0] + c->S[3 * i + 1] * e[1] + c->S[3 * i + 2] * e[2];
-        if (!(ML > 0.0)) return -1;
+        if (!(ML > 0.0)) { c->torque_sampling = 0; return -1; }
         if (pairing_mode == 2) { orc_end_sweep(c, serial_any_pair_sweep(c, T, e, &ML)); continue; }
         int64_t count = orc_constrained_half_sweep(c, T, e, 0, &ML, ml_mode, pairing_mode, NULL, NULL);
         int64_t cb    = orc_constrained_half_sweep(c, T, e, 1, &ML, ml_mode, pairing_mode, NULL, NULL);   /* P:204 (C-5) */
-        if (count < 0 || cb < 0) return -1;
+        if (count < 0 || cb < 0) { c->torque_sampling = 0; return -1; }
         orc_end_sweep(c, count + cb);
     }
+    c->torque_sampling = 0;
     return 0;
 }
 

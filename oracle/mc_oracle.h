@@ -9,8 +9,9 @@
  * Citations "P:NN" are line numbers of /root/reference/PAPER.md (Lepadatu et al., arXiv 2103.03517).
  *
  * Parity status: the paper prints no numeric worked example of a single update or sweep, so the
- * bit-level update sequence is "parity unpinned"; every arithmetic piece is pinned by closed forms,
- * invariants and brute force in tests/test_oracle_*.py.
+ * bit-level update sequence is "parity unpinned"; every function is pinned by closed forms,
+ * invariants and brute force in tests/test_oracle_*.py (orc_align_to:
+ * tests/test_oracle_align.py).
  */
 #ifndef MC_ORACLE_H
 #define MC_ORACLE_H
