@@ -10,9 +10,13 @@
  *   - extern "C", plain pointers and sizes, no exceptions, no globals, no callbacks.  Every pointer argument is a
  *     HOST pointer unless its name starts with dev_.  The caller owns every buffer it passes; the library copies
  *     what it needs during the call and keeps no host pointer afterwards.
- *   - The library allocates NO device memory: the caller hands mc_create() one device workspace of at least
- *     mc_workspace_bytes() bytes (e.g. a torch.empty(..., dtype=uint8, device="cuda")) and a CUDA stream.  All
- *     kernels of a handle run on that stream.  Handles are independent (replicas); one stream per handle.
+ *   - The library allocates NO device memory and changes no device-wide setting: the caller hands mc_create() one
+ *     device workspace of at least mc_workspace_bytes() bytes (e.g. a torch.empty(..., dtype=uint8, device="cuda"))
+ *     and a CUDA stream.  The workspace holds the spin state (12 B per site), the side data, the controller state, the
+ *     trace ring and a staging area of 12 B per site that mc_set_spins / mc_get_spins / the half-sweep hooks /
+ *     mc_profile_x use for their host <-> device copies.  All kernels of a handle run on that stream, on the device the
+ *     workspace lives on (entry points switch to it and restore the caller's current device).  Handles are
+ *     independent (replicas); one stream per handle.  The library reads no environment variable.
  *   - Return value: MC_OK (0) or a negative error code; mc_last_error() gives the message of the last failure.
  *     CUDA errors are sticky per handle (MC_ECUDA).
  *   - Reduced units: k_B = 1, energies in units of J (C-17).  Spins are fp32 on the device.
@@ -106,13 +110,15 @@ int mc_sweep(mc_ctx* ctx, double T, int64_t n);
 
 /* n iterations of the constrained algorithm, Table A2, holding M/|M| along
  * e_C = (sin theta cos phi, sin theta sin phi, cos theta).  On the first call, after mc_set_spins/mc_init_spins,
- * or when (theta, phi) changes, all spins are first rotated rigidly so that M/|M| = e_C (C-12; this step
- * synchronises once; MC_ESTATE if |M|/N < 1e-6).  Pairs are same-colour, formed by the analytic pairing of C-11;
+ * after any unconstrained pass (mc_sweep, mc_half_sweep: they move M off e_C), or when (theta, phi) changes, all spins
+ * are first rotated rigidly so that M/|M| = e_C (C-12; this step synchronises once; MC_ESTATE if |M|/N < 1e-6).  Pairs are same-colour, formed by the analytic pairing of C-11;
  * M_L is taken once per iteration.  Needs an even number of sites per colour (C-15). */
 int mc_constrained_sweep(mc_ctx* ctx, double T, double theta, double phi, int64_t n);
 
-/* Test hooks for per-colour parity (C-14): ONE colour pass of Table A1 / A2 with the current sweep counter and cone;
- * no controller step, no accumulation.  host_x / host_acc are optional [N] outputs in lexicographic site order:
+/* Test hooks for per-colour parity (C-14): ONE colour pass of Table A1 / A2 with the current sweep counter and cone.
+ * No controller step: the accepted count and the fused sums of the pass stay pending on the device until
+ * mc_end_sweep() closes the sweep; if mc_sweep / mc_constrained_sweep is called instead, the pending contribution is
+ * discarded (the spins the hook wrote stay).  host_x / host_acc are optional [N] outputs in lexicographic site order:
  * the fp32 decision variable x = dE/T + ln u2 (constrained: the log form of P:193, stored at the leader's site,
  * +inf for the hard rejections of C-13) and the accept flag; entries of the other colour are left untouched.
  * mc_constrained_half_sweep does not rotate: the caller passes an aligned state and M_L explicitly.  Synchronous. */
@@ -137,8 +143,17 @@ int mc_trace(mc_ctx* ctx, int64_t max_rows, double* host_rows, int64_t* n_rows);
 /* Domain-wall profile (Fig. 2: "the normalized magnetization z component is obtained for each profile point by
  * averaging over the respective cross-section slice"): host_profile[3*x + a] = mean over (y,z) of component a of the spins
  * at that x, x = 0..nx-1 (HOST pointer to 3*nx doubles, caller-owned).  Exact fixed-point sums on the device, so the
- * result is reproducible.  Borrows 24*nx bytes of stream-ordered scratch; synchronous. */
+ * result is reproducible.  Uses 24*nx bytes of the workspace's staging area; synchronous. */
 int mc_profile_x(mc_ctx* ctx, double* host_profile);
+
+/* Test hook: which kernel mc_sweep / mc_half_sweep launch for the colour pass.  MC_PATH_AUTO (default): the planner's
+ * choice for this lattice; MC_PATH_GENERIC: the grid-stride gather pass (covers every lattice); MC_PATH_STAGED: the
+ * TMA-fed shared-memory pass wherever its geometry covers the lattice (MC_EINVAL otherwise).  The arithmetic contract is
+ * the same on every path (same Philox stream, same decisions); parity tests use this to check each one. */
+#define MC_PATH_AUTO     0
+#define MC_PATH_GENERIC  1
+#define MC_PATH_STAGED   2
+int mc_debug_set_path(mc_ctx* ctx, int path);
 
 /* Number of kernel launches this handle has enqueued since creation (bench.py's gpu_launches). */
 int64_t mc_launch_count(const mc_ctx* ctx);

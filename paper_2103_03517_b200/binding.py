@@ -16,12 +16,13 @@ LIB_PATH = os.path.join(_HERE, "libmc_b200.so")
 
 MC_OK, MC_EINVAL, MC_ECUDA, MC_ESTATE = 0, -1, -2, -3
 MC_TRACE_CAPACITY = 16384
+MC_PATH_AUTO, MC_PATH_GENERIC, MC_PATH_STAGED = 0, 1, 2
 
 # every symbol include/mc.h declares (tests/test_abi.py checks the header against this list and the .so)
 SYMBOLS = [
     "mc_workspace_bytes", "mc_create", "mc_destroy", "mc_init_spins", "mc_set_spins", "mc_get_spins", "mc_set_cone",
     "mc_set_sweep", "mc_sweep", "mc_constrained_sweep", "mc_half_sweep", "mc_constrained_half_sweep", "mc_end_sweep",
-    "mc_align_to", "mc_observables", "mc_reset_accumulators", "mc_trace", "mc_profile_x", "mc_launch_count", "mc_last_error", "mc_version",
+    "mc_align_to", "mc_observables", "mc_reset_accumulators", "mc_trace", "mc_profile_x", "mc_debug_set_path", "mc_launch_count", "mc_last_error", "mc_version",
 ]
 
 
@@ -85,6 +86,7 @@ def load():
     L.mc_reset_accumulators.argtypes = [vp]; L.mc_reset_accumulators.restype = i32
     L.mc_trace.argtypes = [vp, i64, vp, vp]; L.mc_trace.restype = i32
     L.mc_profile_x.argtypes = [vp, vp]; L.mc_profile_x.restype = i32
+    L.mc_debug_set_path.argtypes = [vp, i32]; L.mc_debug_set_path.restype = i32
     L.mc_launch_count.argtypes = [vp]; L.mc_launch_count.restype = i64
     L.mc_last_error.argtypes = [vp]; L.mc_last_error.restype = C.c_char_p
     L.mc_version.argtypes = []; L.mc_version.restype = C.c_char_p
@@ -211,4 +213,5 @@ class Lattice:
         self._chk(self.L.mc_trace(self.h, int(max_rows), _p(rows), C.byref(k)))
         return rows[: k.value].copy()
 
+    def debug_set_path(self, path): self._chk(self.L.mc_debug_set_path(self.h, int(path)))
     def launch_count(self): return int(self.L.mc_launch_count(self.h))

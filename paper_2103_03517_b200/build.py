@@ -1,22 +1,32 @@
-"""Builds libmc_b200.so in-tree with nvcc for sm_100a (cross-compiles without a GPU)."""
+"""Builds libmc_b200.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
+
+One object per translation unit (compiled in parallel), then one link: the kernels of the generic pass, the pair pass and
+the staged passes each live in their own .cu so that a change to one does not rebuild the others.
+"""
 from __future__ import annotations
 
+import glob
+import hashlib
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
+OBJDIR = os.path.join(_HERE, "build")
 LIB = os.path.join(_HERE, "libmc_b200.so")
-SOURCES = [os.path.join(CSRC, "mc_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "mc_kernels.cuh"), os.path.join(CSRC, "mc_device.cuh"), os.path.join(CSRC, "mc_tile.cuh"),
-                  os.path.join(os.path.dirname(_HERE), "include", "mc.h")]
+HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h"))) + [os.path.join(os.path.dirname(_HERE), "include", "mc.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-ftz=true", "-prec-div=false", "-prec-sqrt=false",
-    "-shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-O2",
+    "-Xcompiler", "-fPIC", "-Xcompiler", "-O2",
 ]
+
+
+def sources():
+    return sorted(glob.glob(os.path.join(CSRC, "*.cu")))
 
 
 def nvcc() -> str:
@@ -26,16 +36,26 @@ def nvcc() -> str:
     return "nvcc"
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    newest = max(os.path.getmtime(p) for p in DEPS)
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
-        return LIB
-    tmp = f"{LIB}.{os.getpid()}.tmp"
-    extra = os.environ.get("MC_B200_NVCC_EXTRA", "").split()      # experiments only (e.g. -DMC_TILE_MIN_BLOCKS=3)
-    cmd = [nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
-    subprocess.check_call(cmd)
-    os.replace(tmp, LIB)
-    return LIB
+def build(force: bool = False, verbose: bool = False, extra=(), lib: str = LIB, objdir: str = OBJDIR) -> str:
+    """Compiles what is out of date and links ``lib``.  ``extra`` (additional nvcc flags, e.g. ``-DMC_X=1``) and a different
+    ``lib`` / ``objdir`` are for experiment builds next to the product library; the product build passes none."""
+    os.makedirs(objdir, exist_ok=True)
+    tag = hashlib.sha1(" ".join(list(NVCC_FLAGS) + list(extra)).encode()).hexdigest()[:10]
+    newest_hdr = max(os.path.getmtime(p) for p in HEADERS)
+    jobs, objs = [], []
+    for src in sources():
+        obj = os.path.join(objdir, f"{os.path.splitext(os.path.basename(src))[0]}.{tag}.o")
+        objs.append(obj)
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(newest_hdr, os.path.getmtime(src)):
+            jobs.append([nvcc()] + NVCC_FLAGS + list(extra) + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, src])
+    if jobs:
+        with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
+            list(ex.map(subprocess.check_call, jobs))
+    if jobs or not os.path.exists(lib) or os.path.getmtime(lib) < max(os.path.getmtime(o) for o in objs):
+        tmp = f"{lib}.{os.getpid()}.tmp"
+        subprocess.check_call([nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp] + objs)
+        os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":

@@ -1,13 +1,11 @@
 // mc_api.cu -- host side of libmc_b200.so: the C ABI declared in include/mc.h.
 // Argument marshalling, workspace carving, launch configuration.  Every step of the hot path runs in the kernels
 // of mc_kernels.cuh; there is no CPU fallback (without a device every entry point returns MC_ECUDA).
-#include "../../include/mc.h"
-#include "mc_kernels.cuh"
-#include "mc_tile.cuh"
+#include "mc_host.h"
+#include "mc_util.cuh"
 
 #include <cmath>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <vector>
 
@@ -19,7 +17,7 @@ constexpr size_t ALIGN = 256;
 inline size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {            // byte offsets into the caller's workspace
-    size_t spins, mask, region, axis, state, trace, total;
+    size_t spins, mask, region, axis, state, trace, staging, staging_bytes, total;
     long long plane, mask_plane, region_plane;
     int max_blocks;
 };
@@ -60,6 +58,11 @@ Layout make_layout(const mc_lattice* lat, const mc_hamiltonian* ham)
     L.axis = off;     if (ham->region) off += round_up((size_t)ham->n_regions * sizeof(float4), ALIGN);
     L.state = off;    off += round_up(sizeof(DevState), ALIGN);
     L.trace = off;    off += round_up((size_t)TRACE_CAP * 6 * sizeof(double), ALIGN);
+    // staging: the [N][3] fp32 lexicographic image of the state during mc_set_spins / mc_get_spins, or the [N] fp32 + [N] u8
+    // outputs of a half-sweep hook, or the 3 nx int64 sums of mc_profile_x -- the library allocates nothing itself
+    const size_t N = (size_t)lat->nx * lat->ny * lat->nz;
+    L.staging_bytes = round_up(N * 3 * sizeof(float), ALIGN) + round_up((size_t)lat->nx * 3 * sizeof(long long), ALIGN);
+    L.staging = off;  off += L.staging_bytes;
     L.total = off;
     return L;
 }
@@ -78,207 +81,27 @@ FastDiv make_div(uint32_t d)
 
 }  // namespace
 
-struct mc_ctx {
-    mc_lattice lat;
-    double J, Ku, Kc, eu[3], B[3];
-    int adaptive;
-    uint64_t seed;
-    Params P;
-    Geom geom;
-    PairGeom pgeom;
-    bool pair_ok;
-    bool tile_ok; TileGeom tgeom; int tile_threads; size_t tile_smem;   // fast path of the colour pass (mc_tile.cuh)
-    bool field;
-    int vec, aniso;
-    bool masked;
-    cudaStream_t stream;
-    int sm_count, blocks_per_sm;
-    bool ml_valid, aligned;
-    double theta, phi, eC[3];
-    int64_t launches;
-    int sticky;
-    char err[512];
-};
-
 namespace {
 
-int fail(mc_ctx* c, int code, const char* fmt, const char* detail = "")
-{
-    if (c) { snprintf(c->err, sizeof c->err, fmt, detail); if (code == MC_ECUDA) c->sticky = MC_ECUDA; }
-    return code;
-}
-
-#define CU(call)                                                                                   \
-    do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail(ctx, MC_ECUDA, "CUDA error: %s", cudaGetErrorString(e_)); } while (0)
+#define CU(call) MC_CU(call)
+// every entry point runs on the handle's device, whatever the caller's current device is, and restores it on return
+struct DeviceGuard {
+    int prev = -1; bool switched = false;
+    explicit DeviceGuard(int dev) { if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess; }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
 #define CHECK_CTX()                                                                                \
-    do { if (!ctx) return MC_EINVAL; if (ctx->sticky) return ctx->sticky; ctx->err[0] = 0; } while (0)
-
-typedef void (*PassFn)(const Params, const Geom, int, float, int, float*, uint8_t*);
-typedef void (*PairFn)(const Params, const PairGeom, int, float, int, float*, uint8_t*);
-
-template <int VEC, int MODE> PassFn pick_pass(int aniso, bool masked)
-{
-    switch (aniso * 2 + (masked ? 1 : 0)) {
-        case 0: return pass_kernel<VEC, 0, false, MODE>;  case 1: return pass_kernel<VEC, 0, true, MODE>;
-        case 2: return pass_kernel<VEC, 1, false, MODE>;  case 3: return pass_kernel<VEC, 1, true, MODE>;
-        case 4: return pass_kernel<VEC, 2, false, MODE>;  case 5: return pass_kernel<VEC, 2, true, MODE>;
-        case 6: return pass_kernel<VEC, 3, false, MODE>;  default: return pass_kernel<VEC, 3, true, MODE>;
-    }
-}
-template <int VEC> PairFn pick_pair(int aniso, bool masked)
-{
-    switch (aniso * 2 + (masked ? 1 : 0)) {
-        case 0: return pair_kernel<VEC, 0, false>;  case 1: return pair_kernel<VEC, 0, true>;
-        case 2: return pair_kernel<VEC, 1, false>;  case 3: return pair_kernel<VEC, 1, true>;
-        case 4: return pair_kernel<VEC, 2, false>;  case 5: return pair_kernel<VEC, 2, true>;
-        case 6: return pair_kernel<VEC, 3, false>;  default: return pair_kernel<VEC, 3, true>;
-    }
-}
-
-typedef void (*TileFn)(const Params, const TileGeom, int, float, int, float*, uint8_t*);
-template <int RT, bool DEBUG, bool ANTI = false> TileFn pick_tile_rt(int aniso, bool field)
-{
-    switch (aniso * 2 + (field ? 1 : 0)) {
-        case 0: return tile_pass_kernel<0, false, RT, DEBUG, ANTI>;  case 1: return tile_pass_kernel<0, true, RT, DEBUG, ANTI>;
-        case 2: return tile_pass_kernel<1, false, RT, DEBUG, ANTI>;  case 3: return tile_pass_kernel<1, true, RT, DEBUG, ANTI>;
-        case 4: return tile_pass_kernel<2, false, RT, DEBUG, ANTI>;  case 5: return tile_pass_kernel<2, true, RT, DEBUG, ANTI>;
-        case 6: return tile_pass_kernel<3, false, RT, DEBUG, ANTI>;  default: return tile_pass_kernel<3, true, RT, DEBUG, ANTI>;
-    }
-}
-// Row lengths with a specialised instantiation (every shared-memory offset an immediate): R = nx/2 of BASELINE's
-// periodic configs c2 (64^3), c4 (128^3) and c3 (224^3), plus 192^3 (R = 96: 58 against 65 us per sweep for the generic pass).  Any other R runs the run-time-R instantiation.
-// The decision-variable debug outputs of the test hooks exist only in the run-time-R instantiation (same arithmetic).
-TileFn pick_tile(int R, int Ty, int npass, bool debug, int aniso, bool field, bool anti)
-{
-    if (anti) return debug ? pick_tile_rt<0, true, true>(aniso, field) : pick_tile_rt<0, false, true>(aniso, field);
-    if (debug) return pick_tile_rt<0, true>(aniso, field);
-    if (getenv("MC_B200_NO_RT") || Ty != TILE_TY_RT || npass != TILE_NPASS_RT) return pick_tile_rt<0, false>(aniso, field);
-    switch (R) {
-        case 32:  return pick_tile_rt<32, false>(aniso, field);
-        case 96:  return pick_tile_rt<96, false>(aniso, field);
-        case 64:  return pick_tile_rt<64, false>(aniso, field);
-        case 112: return pick_tile_rt<112, false>(aniso, field);
-        default:  return pick_tile_rt<0, false>(aniso, field);
-    }
-}
-
-// Chooses the slab / segment decomposition of the tiled colour pass.  Returns false when the
-// lattice is not eligible (then the generic pass_kernel runs).
-bool plan_tile(mc_ctx* c)
-{
-    c->tile_ok = false;
-    const mc_lattice& lat = c->lat;
-    if (c->masked || c->P.region) return false;
-    if (!(lat.periodic[0] >= 1 && lat.periodic[1] == 1 && lat.periodic[2] == 1)) return false;   // x may be anti-periodic (ANTI instantiation)
-    const int R = lat.nx / 2;
-    if (R % 4) return false;                                    // TMA bulk copies move whole rows: 16-byte multiples
-    const int PR = R / 2;
-    int max_threads = TILE_MAX_THREADS, want_rp = 0, want_np = 0, want_segs = 0;
-    if (const char* env = getenv("MC_B200_TILE")) sscanf(env, "%d,%d,%d,%d", &want_rp, &want_np, &want_segs, &max_threads);
-    if (max_threads > TILE_MAX_THREADS) max_threads = TILE_MAX_THREADS;
-    if (PR > max_threads) return false;
-    TileGeom& G = c->tgeom;
-    G.R = R; G.PR = PR; G.nx = lat.nx; G.ny = lat.ny; G.nz = lat.nz;
-    int RP = 1;
-    for (int d = 1; d <= lat.ny; ++d) if (lat.ny % d == 0 && PR * d <= max_threads) RP = d;
-    if (want_rp > 0 && lat.ny % want_rp == 0 && PR * want_rp <= TILE_MAX_THREADS) RP = want_rp;
-    int NP = 1;
-    const size_t smem_cap = (size_t)(220 * 1024) / TILE_MIN_BLOCKS - 3 * 1024;   // TILE_MIN_BLOCKS CTAs per SM
-    auto slot_bytes = [&](int ty) { return (size_t)3 * (ty + 2) * R * sizeof(float); };
-    if (lat.ny % (2 * RP) == 0 && TILE_NSLOT * slot_bytes(2 * RP) <= smem_cap) NP = 2;
-    // row lengths with a compile-time specialisation (R = 32, 64, 96, 112) take its slab shape when it fits: 64^3 13.3 -> 11.3 us per sweep
-    if ((R == 32 || R == 64 || R == 96 || R == 112) && lat.ny % TILE_TY_RT == 0 && PR * (TILE_TY_RT / TILE_NPASS_RT) <= max_threads) {
-        RP = TILE_TY_RT / TILE_NPASS_RT; NP = TILE_NPASS_RT;
-    }
-    if (want_rp > 0 && lat.ny % want_rp == 0 && PR * want_rp <= TILE_MAX_THREADS) { RP = want_rp; NP = 1; if (lat.ny % (2 * RP) == 0 && TILE_NSLOT * slot_bytes(2 * RP) <= smem_cap) NP = 2; }
-    if (want_np > 0 && lat.ny % (want_np * RP) == 0) NP = want_np;
-    G.RP = RP; G.NPASS = NP; G.Ty = RP * NP;
-    G.n_slabs = lat.ny / G.Ty;
-    G.slot_floats = 3 * (G.Ty + 2) * R;
-    G.n_active = PR * RP;
-    c->tile_threads = (G.n_active + 31) / 32 * 32;
-    c->tile_smem = TILE_NSLOT * slot_bytes(G.Ty);
-    if (c->tile_smem > 200 * 1024) return false;
-    // every instantiation this handle can launch must be allowed its dynamic shared memory
-    TileFn fns[2] = { pick_tile(R, G.Ty, G.NPASS, false, c->aniso, c->field, c->P.anti_x != 0), pick_tile(R, G.Ty, G.NPASS, true, c->aniso, c->field, c->P.anti_x != 0) };
-    int per_sm = 1;
-    for (TileFn f : fns) {
-        if (cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tile_smem) != cudaSuccess) { cudaGetLastError(); return false; }
-    }
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)fns[0], c->tile_threads, c->tile_smem) != cudaSuccess || per_sm < 1) { cudaGetLastError(); return false; }
-    // one wave of CTAs: n_segs z-segments per slab so that n_slabs * n_segs fills sm_count * per_sm slots
-    long long slots = (long long)c->sm_count * per_sm;
-    int n_segs = (int)(slots / G.n_slabs);
-    if (n_segs < 1) n_segs = 1;
-    if (n_segs > lat.nz) n_segs = lat.nz;
-    if (want_segs > 0 && want_segs <= lat.nz) n_segs = want_segs;
-    G.n_segs = n_segs; G.Lz = lat.nz / n_segs; G.Lz_rem = lat.nz % n_segs;
-    if ((long long)G.n_slabs * G.n_segs > c->P.max_blocks) return false;
-    // Default: the tiled pass runs where it has a compile-time-row-length instantiation (R = 32, 64, 96, 112 in the specialised slab
-    // shape: 64^3, 128^3, 224^3 of BASELINE.json, and 192^3); everywhere else the generic pass is faster since it went packed and to three
-    // CTAs per SM (measured: 96^3 16.3 vs 18.5 us per sweep, 160^3 40 vs 49, 256^3 148 vs 164, 512^3 1222 vs 1285).
-    // MC_B200_PATH=tile forces the tiled pass wherever the geometry allows it (tests), =generic forces the generic one.
-    const bool specialised = (R == 32 || R == 64 || R == 96 || R == 112) && G.Ty == TILE_TY_RT && G.NPASS == TILE_NPASS_RT && !c->P.anti_x;
-    c->tile_ok = specialised && c->P.Nc >= 65536u;             // small lattices are launch-bound: the generic kernel has less prologue
-    if (const char* env = getenv("MC_B200_PATH")) { c->tile_ok = !strcmp(env, "tile"); }
-    if (getenv("MC_B200_VERBOSE"))
-        fprintf(stderr, "mc tile plan: ok=%d R=%d PR=%d RP=%d NPASS=%d Ty=%d slabs=%d segs=%d Lz=%d(+%d) threads=%d smem=%zu ctas/SM=%d\n",
-                (int)c->tile_ok, R, PR, RP, NP, G.Ty, G.n_slabs, G.n_segs, G.Lz, G.Lz_rem, c->tile_threads, c->tile_smem, per_sm);
-    return c->tile_ok;
-}
-
-// grid of a grid-stride kernel: one resident wave (the CTAs per SM its launch bounds allow) unless the environment overrides
-int grid_for(const mc_ctx* c, uint32_t n_threads_needed, int resident_per_sm)
-{
-    const long long need = ((long long)n_threads_needed + BLOCK - 1) / BLOCK;
-    long long cap = (long long)c->sm_count * (c->blocks_per_sm > 0 ? c->blocks_per_sm : resident_per_sm);
-    if (cap > c->P.max_blocks) cap = c->P.max_blocks;
-    long long g = need < cap ? need : cap;
-    return (int)(g < 1 ? 1 : g);
-}
-
-// Launch of a pass kernel with programmatic dependent launch: the grid may be scheduled while the previous kernel of the
-// stream drains (every pass kernel starts with grid_dependency_sync(), so it reads nothing early).  Hides the launch
-// gap between the 2n back-to-back colour passes of mc_sweep(T, n).
-template <class Fn, class Geo>
-cudaError_t launch_dependent(Fn fn, int grid, int block, size_t smem, cudaStream_t stream, const Params& P, const Geo& G,
-                             int colour, float invT, int flags, float* dx, uint8_t* da)
-{
-    static const bool no_pdl = getenv("MC_B200_NO_PDL") != nullptr;
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr; cfg.numAttrs = no_pdl ? 0 : 1;
-    return cudaLaunchKernelEx(&cfg, fn, P, G, colour, invT, flags, dx, da);
-}
+    if (!ctx) return MC_EINVAL; if (ctx->sticky) return ctx->sticky; ctx->err[0] = 0; DeviceGuard guard_(ctx->device)
 
 int launch_pass(mc_ctx* ctx, int mode, int colour, float invT, int flags, float* dx, uint8_t* da)
 {
-    if (mode == MODE_SWEEP && ctx->tile_ok) {
-        TileFn fn = pick_tile(ctx->tgeom.R, ctx->tgeom.Ty, ctx->tgeom.NPASS, dx || da, ctx->aniso, ctx->field, ctx->P.anti_x != 0);
-        const int grid = ctx->tgeom.n_slabs * ctx->tgeom.n_segs;
-        CU(launch_dependent(fn, grid, ctx->tile_threads, ctx->tile_smem, ctx->stream, ctx->P, ctx->tgeom, colour, invT, flags, dx, da));
-        ctx->launches += 1;
-        return MC_OK;
-    }
-    PassFn fn = (ctx->vec == 4) ? (mode == MODE_SWEEP ? pick_pass<4, MODE_SWEEP>(ctx->aniso, ctx->masked) : pick_pass<4, MODE_MEASURE>(ctx->aniso, ctx->masked))
-                                : (mode == MODE_SWEEP ? pick_pass<1, MODE_SWEEP>(ctx->aniso, ctx->masked) : pick_pass<1, MODE_MEASURE>(ctx->aniso, ctx->masked));
-    const int grid = grid_for(ctx, ctx->geom.n_items, MC_PASS_MIN_BLOCKS);
-    // measurement uses partial slots 2,3 so that it never disturbs a sweep assembled from the half-sweep hooks
-    CU(launch_dependent(fn, grid, BLOCK, 0, ctx->stream, ctx->P, ctx->geom, colour, invT, flags, dx, da));
-    ctx->launches += 1;
-    return MC_OK;
+    if (mode == MODE_SWEEP && ctx->tile_ok) return launch_pass_tile(ctx, colour, invT, flags, dx, da);
+    return launch_pass_generic(ctx, mode, colour, invT, flags, dx, da);
 }
 
 int launch_pair(mc_ctx* ctx, int colour, float invT, int flags, float* dx, uint8_t* da)
 {
-    PairFn fn = (ctx->vec == 4) ? pick_pair<4>(ctx->aniso, ctx->masked) : pick_pair<1>(ctx->aniso, ctx->masked);
-    const int grid = grid_for(ctx, ctx->pgeom.n_threads, MC_PAIR_MIN_BLOCKS);
-    CU(launch_dependent(fn, grid, BLOCK, 0, ctx->stream, ctx->P, ctx->pgeom, colour, invT, flags, dx, da));
-    ctx->launches += 1;
-    return MC_OK;
+    return launch_pair_generic(ctx, colour, invT, flags, dx, da);
 }
 
 int launch_state(mc_ctx* ctx, int what, double a = 0, double b = 0, double c = 0, unsigned long long u = 0)
@@ -304,6 +127,15 @@ int read_state(mc_ctx* ctx, DevState* host)
     CU(cudaMemcpyAsync(host, ctx->P.st, sizeof(DevState), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     return MC_OK;
+}
+
+// A half-sweep hook that was not closed by mc_end_sweep() left its accepted count and fused sums in DevState: a following
+// mc_sweep / mc_constrained_sweep starts from a clean sweep (the hook's contribution is discarded, the spins it wrote stay).
+int discard_pending_hook(mc_ctx* ctx)
+{
+    if (!ctx->hook_pending) return MC_OK;
+    ctx->hook_pending = false;
+    return launch_state(ctx, ST_RESET_SWEEP);
 }
 
 void direction(double theta, double phi, double e[3])
@@ -343,23 +175,18 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     double n = sqrt(ham->eu[0] * ham->eu[0] + ham->eu[1] * ham->eu[1] + ham->eu[2] * ham->eu[2]);
     for (int a = 0; a < 3; ++a) { ctx->eu[a] = n > 0 ? ham->eu[a] / n : (a == 2 ? 1.0 : 0.0); ctx->B[a] = ham->B[a]; }
     ctx->stream = (cudaStream_t)cuda_stream;
-    ctx->blocks_per_sm = 0;                                    // 0: one resident wave per kernel (grid_for)
-    if (const char* env = getenv("MC_B200_BLOCKS_PER_SM")) { int v = atoi(env); if (v >= 1 && v <= 32) ctx->blocks_per_sm = v; }
 
     auto bail = [&](int code, const char* msg) { fprintf(stderr, "mc_create: %s\n", msg); delete ctx; return code; };
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return bail(MC_ECUDA, "no CUDA device");
-    if (cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return bail(MC_ECUDA, "cannot query the device");
-    {   // mc_set_spins / mc_get_spins borrow stream-ordered scratch (cudaMallocAsync) and return it before they end; keep
-        // what they return cached in the device's default pool instead of handing it back to the driver at every
-        // synchronisation (the default threshold of 0 makes every upload pay a fresh 135 MB allocation at c3)
-        cudaMemPool_t pool;
-        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-            unsigned long long keep = ~0ull;
-            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-        }
-        cudaGetLastError();
+    {   // the workspace pointer decides the device of the handle (a process may hold handles on several devices)
+        cudaPointerAttributes pa;
+        if (cudaPointerGetAttributes(&pa, dev_workspace) == cudaSuccess && pa.type == cudaMemoryTypeDevice) dev = pa.device;
+        else cudaGetLastError();
     }
+    ctx->device = dev;
+    DeviceGuard guard_(dev);
+    if (cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return bail(MC_ECUDA, "cannot query the device");
 
     const int nx = lat->nx, ny = lat->ny, nz = lat->nz;
     const uint32_t N = (uint32_t)nx * ny * nz, R = nx / 2, Nc = N / 2;
@@ -382,12 +209,12 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
         P.fx_scale = (float)ldexp(1.0, k); P.fx_inv = ldexp(1.0, -k);
     }
     P.trace = (double*)(ws + L.trace);
+    ctx->staging = ws + L.staging; ctx->staging_bytes = L.staging_bytes;
 
     ctx->aniso = (ham->Ku != 0.0 ? 1 : 0) | (ham->Kc != 0.0 ? 2 : 0);
     ctx->field = ham->B[0] != 0.0 || ham->B[1] != 0.0 || ham->B[2] != 0.0;
     ctx->masked = needs_mask(lat, ham);
     ctx->vec = (nx % 8 == 0) ? 4 : 1;
-    if (const char* env = getenv("MC_B200_VEC")) { if (atoi(env) == 1) ctx->vec = 1; }     // experiments
     ctx->geom.RV = R / ctx->vec; ctx->geom.n_items = Nc / ctx->vec;
     ctx->geom.div_rv = make_div(ctx->geom.RV); ctx->geom.div_nz = make_div((uint32_t)nz);
     { uint32_t sh = 0; while (sh < 5 && ny % (2 << sh) == 0) ++sh; ctx->geom.yb_shift = sh; }      // up to 32 rows per block
@@ -488,6 +315,19 @@ int mc_destroy(mc_ctx* ctx) { if (!ctx) return MC_EINVAL; delete ctx; return MC_
 const char* mc_last_error(const mc_ctx* ctx) { return ctx ? ctx->err : "null handle"; }
 int64_t mc_launch_count(const mc_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+int mc_debug_set_path(mc_ctx* ctx, int path)
+{
+    CHECK_CTX();
+    if (path == MC_PATH_AUTO) { const bool keep = ctx->tile_possible; plan_tile(ctx); ctx->tile_possible = keep || ctx->tile_possible; }
+    else if (path == MC_PATH_GENERIC) ctx->tile_ok = false;
+    else if (path == MC_PATH_STAGED) {
+        if (!ctx->tile_possible) return fail(ctx, MC_EINVAL, "mc_debug_set_path: the staged pass does not cover this lattice / Hamiltonian");
+        ctx->tile_ok = true;
+    } else return fail(ctx, MC_EINVAL, "mc_debug_set_path: unknown path");
+    ctx->path = path;
+    return MC_OK;
+}
+
 int mc_init_spins(mc_ctx* ctx, int mode, const double dir[3])
 {
     CHECK_CTX();
@@ -519,13 +359,11 @@ int mc_set_spins(mc_ctx* ctx, const float* host_xyz)
     CHECK_CTX();
     if (!host_xyz) return fail(ctx, MC_EINVAL, "mc_set_spins: null pointer");
     const size_t bytes = (size_t)ctx->P.N * 3 * sizeof(float);
-    float* tmp = nullptr;
-    CU(cudaMallocAsync((void**)&tmp, bytes, ctx->stream));       // stream-ordered scratch, returned before the call ends
+    float* tmp = (float*)ctx->staging;                           // staging area of the caller's workspace
     CU(cudaMemcpyAsync(tmp, host_xyz, bytes, cudaMemcpyHostToDevice, ctx->stream));
     lex_to_split_kernel<<<(ctx->P.N + 255) / 256, 256, 0, ctx->stream>>>(ctx->P, tmp);
     ctx->launches += 1;
     CU(cudaGetLastError());
-    CU(cudaFreeAsync(tmp, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     ctx->ml_valid = false; ctx->aligned = false;
     return MC_OK;
@@ -536,13 +374,11 @@ int mc_get_spins(mc_ctx* ctx, float* host_xyz)
     CHECK_CTX();
     if (!host_xyz) return fail(ctx, MC_EINVAL, "mc_get_spins: null pointer");
     const size_t bytes = (size_t)ctx->P.N * 3 * sizeof(float);
-    float* tmp = nullptr;
-    CU(cudaMallocAsync((void**)&tmp, bytes, ctx->stream));
+    float* tmp = (float*)ctx->staging;
     split_to_lex_kernel<<<(ctx->P.N + 255) / 256, 256, 0, ctx->stream>>>(ctx->P, tmp);
     ctx->launches += 1;
     CU(cudaGetLastError());
     CU(cudaMemcpyAsync(host_xyz, tmp, bytes, cudaMemcpyDeviceToHost, ctx->stream));
-    CU(cudaFreeAsync(tmp, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     return MC_OK;
 }
@@ -572,6 +408,11 @@ int mc_sweep(mc_ctx* ctx, double T, int64_t n)
     CHECK_CTX();
     if (!(T > 0.0) || n < 0) return fail(ctx, MC_EINVAL, "mc_sweep: need T > 0 and n >= 0");      // C-16
     const float invT = (float)(1.0 / T);
+    if (n > 0) {
+        int rc;
+        if ((rc = discard_pending_hook(ctx))) return rc;
+        ctx->aligned = false;             // an unconstrained pass moves M off e_C: the next constrained sweep re-aligns (C-12)
+    }
     for (int64_t i = 0; i < n; ++i) {
         int rc;
         if ((rc = launch_pass(ctx, MODE_SWEEP, 0, invT, 0, nullptr, nullptr))) return rc;
@@ -638,6 +479,7 @@ int mc_constrained_sweep(mc_ctx* ctx, double T, double theta, double phi, int64_
         if ((rc = read_state(ctx, &st))) return rc;
         if (!(st.ML > 0.0)) return fail(ctx, MC_ESTATE, "mc_constrained_sweep: M.e_C <= 0");
     }
+    if ((rc = discard_pending_hook(ctx))) return rc;
     const float invT = (float)(1.0 / T);
     const int fl = F_TORQUE | F_SAMPLE_TORQUE;
     for (int64_t i = 0; i < n; ++i) {
@@ -652,14 +494,17 @@ int mc_constrained_sweep(mc_ctx* ctx, double T, double theta, double phi, int64_
 static int hook_common(mc_ctx* ctx, int colour, float* host_x, uint8_t* host_acc, bool pair, float invT)
 {
     const uint32_t N = ctx->P.N;
-    float* dx = nullptr; uint8_t* da = nullptr;
-    if (host_x)   { CU(cudaMallocAsync((void**)&dx, (size_t)N * sizeof(float), ctx->stream)); CU(cudaMemsetAsync(dx, 0xFF, (size_t)N * sizeof(float), ctx->stream)); }
-    if (host_acc) { CU(cudaMallocAsync((void**)&da, (size_t)N, ctx->stream)); CU(cudaMemsetAsync(da, 0, (size_t)N, ctx->stream)); }
+    // outputs in the staging area of the workspace: [N] fp32 decision variables, then [N] accept flags
+    float* dx = host_x ? (float*)ctx->staging : nullptr;
+    uint8_t* da = host_acc ? (uint8_t*)ctx->staging + round_up((size_t)N * sizeof(float), ALIGN) : nullptr;
+    if (dx) CU(cudaMemsetAsync(dx, 0xFF, (size_t)N * sizeof(float), ctx->stream));
+    if (da) CU(cudaMemsetAsync(da, 0, (size_t)N, ctx->stream));
+    ctx->hook_pending = true;             // the pass leaves its count and fused sums in DevState until mc_end_sweep()
     int rc = pair ? launch_pair(ctx, colour, invT, F_TORQUE, dx, da) : launch_pass(ctx, MODE_SWEEP, colour, invT, 0, dx, da);
     if (rc) return rc;
     std::vector<float> hx; std::vector<uint8_t> ha;
-    if (host_x)   { hx.resize(N); CU(cudaMemcpyAsync(hx.data(), dx, (size_t)N * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream)); CU(cudaFreeAsync(dx, ctx->stream)); }
-    if (host_acc) { ha.resize(N); CU(cudaMemcpyAsync(ha.data(), da, (size_t)N, cudaMemcpyDeviceToHost, ctx->stream)); CU(cudaFreeAsync(da, ctx->stream)); }
+    if (host_x)   { hx.resize(N); CU(cudaMemcpyAsync(hx.data(), dx, (size_t)N * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream)); }
+    if (host_acc) { ha.resize(N); CU(cudaMemcpyAsync(ha.data(), da, (size_t)N, cudaMemcpyDeviceToHost, ctx->stream)); }
     CU(cudaStreamSynchronize(ctx->stream));
     const int nx = ctx->P.nx, ny = ctx->P.ny;
     for (uint32_t s = 0; s < N; ++s) {
@@ -669,6 +514,7 @@ static int hook_common(mc_ctx* ctx, int colour, float* host_x, uint8_t* host_acc
         if (host_acc) host_acc[s] = ha[s];
     }
     ctx->ml_valid = false;
+    if (!pair) ctx->aligned = false;
     return MC_OK;
 }
 
@@ -700,6 +546,7 @@ int mc_end_sweep(mc_ctx* ctx)
     finalize_kernel<<<1, BLOCK, 0, ctx->stream>>>(ctx->P, 0, 0);
     ctx->launches += 1;
     CU(cudaGetLastError());
+    ctx->hook_pending = false;
     return MC_OK;
 }
 
@@ -734,8 +581,7 @@ int mc_profile_x(mc_ctx* ctx, double* host_profile)
     if (!host_profile) return fail(ctx, MC_EINVAL, "mc_profile_x: null pointer");
     const int nx = ctx->P.nx;
     const size_t bytes = (size_t)nx * 3 * sizeof(long long);
-    long long* tmp = nullptr;
-    CU(cudaMallocAsync((void**)&tmp, bytes, ctx->stream));        // stream-ordered scratch, returned before the call ends
+    long long* tmp = (long long*)((char*)ctx->staging + ctx->staging_bytes - round_up(bytes, ALIGN));   // tail of the staging area
     CU(cudaMemsetAsync(tmp, 0, bytes, ctx->stream));
     const uint32_t rows = (uint32_t)ctx->P.ny * (uint32_t)ctx->P.nz;
     const uint32_t n_threads = (uint32_t)ctx->P.R * ((rows + PROFILE_ROWS - 1) / PROFILE_ROWS);
@@ -744,7 +590,6 @@ int mc_profile_x(mc_ctx* ctx, double* host_profile)
     CU(cudaGetLastError());
     std::vector<long long> sums((size_t)nx * 3);
     CU(cudaMemcpyAsync(sums.data(), tmp, bytes, cudaMemcpyDeviceToHost, ctx->stream));
-    CU(cudaFreeAsync(tmp, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     const double scale = ctx->P.fx_inv / ((double)ctx->P.ny * (double)ctx->P.nz);
     for (size_t i = 0; i < sums.size(); ++i) host_profile[i] = (double)sums[i] * scale;

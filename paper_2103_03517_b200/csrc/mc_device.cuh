@@ -99,7 +99,7 @@ __device__ __forceinline__ void cone_move(const Vec3& S, float one_minus_cos, fl
     const float sa = t * rsqrtf(t);                          // sqrt(t), t > 0 always (u0 >= 2^-24, theta >= 1 deg)
     const float ang = fmaf(u1, 6.2831853071795865f, -3.1415926535897932f);
     const float cp = -__cosf(ang), sp = -__sinf(ang);
-    const float sg = (S.z >= 0.0f) ? 1.0f : -1.0f;
+    const float sg = copysignf(1.0f, S.z);                   // sign BIT of S_z (C-29): -0.0 gives -1, as in the packed paths
     const float a  = __fdividef(-1.0f, sg + S.z);
     const float b  = S.x * S.y * a;
     const Vec3 t1 = { fmaf(sg * S.x * S.x, a, 1.0f), sg * b, -sg * S.x };

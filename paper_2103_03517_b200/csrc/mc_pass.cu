@@ -1,0 +1,32 @@
+// mc_pass.cu -- instantiations and launcher of the generic colour pass (mc_pass.cuh).
+#include "mc_host.h"
+#include "mc_pass.cuh"
+
+namespace mc {
+namespace {
+
+typedef void (*PassFn)(const Params, const Geom, int, float, int, float*, uint8_t*);
+
+template <int VEC, int MODE> PassFn pick_pass(int aniso, bool masked)
+{
+    switch (aniso * 2 + (masked ? 1 : 0)) {
+        case 0: return pass_kernel<VEC, 0, false, MODE>;  case 1: return pass_kernel<VEC, 0, true, MODE>;
+        case 2: return pass_kernel<VEC, 1, false, MODE>;  case 3: return pass_kernel<VEC, 1, true, MODE>;
+        case 4: return pass_kernel<VEC, 2, false, MODE>;  case 5: return pass_kernel<VEC, 2, true, MODE>;
+        case 6: return pass_kernel<VEC, 3, false, MODE>;  default: return pass_kernel<VEC, 3, true, MODE>;
+    }
+}
+
+}  // namespace
+
+int launch_pass_generic(mc_ctx* ctx, int mode, int colour, float invT, int flags, float* dx, uint8_t* da)
+{
+    PassFn fn = (ctx->vec == 4) ? (mode == MODE_SWEEP ? pick_pass<4, MODE_SWEEP>(ctx->aniso, ctx->masked) : pick_pass<4, MODE_MEASURE>(ctx->aniso, ctx->masked))
+                                : (mode == MODE_SWEEP ? pick_pass<1, MODE_SWEEP>(ctx->aniso, ctx->masked) : pick_pass<1, MODE_MEASURE>(ctx->aniso, ctx->masked));
+    const int grid = grid_for(ctx, ctx->geom.n_items, MC_PASS_MIN_BLOCKS);
+    MC_CU(launch_dependent(fn, grid, BLOCK, 0, ctx->stream, ctx->P, ctx->geom, colour, invT, flags, dx, da));
+    ctx->launches += 1;
+    return MC_OK;
+}
+
+}  // namespace mc

@@ -17,7 +17,7 @@
 // Arithmetic contract: identical to pass_kernel / DESIGN.md section 3 (same Philox stream, same cone construction).
 #pragma once
 
-#include "mc_kernels.cuh"
+#include "mc_common.cuh"
 
 namespace mc {
 

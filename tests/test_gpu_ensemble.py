@@ -260,16 +260,51 @@ def test_full_size_c3_timed_kernels_match_the_checked_ones(mods):
     a.close(); b.close()
 
 
-def test_full_size_c5_half_sweep_parity(mods):
+@pytest.mark.parametrize("T", [0.5, 1.44])
+def test_full_size_c3_parity_at_the_points_bench_times(mods, T):
+    """bench.py cycles T through {0.5, 1.2, 1.44} with the adaptive cone from a random-sphere start.  Here the library
+    itself runs 60 such sweeps at T (the controller settles near 0.67 rad at T = 0.5 and near 1.6 rad at T = 1.44), then
+    BOTH colour passes from that state, with that cone and sweep counter, are compared with the oracle site by site."""
+    oracle, binding, inputs = mods
+    shape = (224, 224, 224); N = 224 ** 3
+    ham = dict(Kc=0.01)
+    g = binding.Lattice(*shape, seed=42, cone0=0.5, adaptive=True, **ham)
+    g.set_spins(inputs.random_unit_spins(N, seed=42))
+    g.sweep(T, 60)
+    ob = g.observables()
+    o = oracle.Oracle(*shape, seed=42, cone0=ob.cone_rad, adaptive=False, **ham)
+    o.set_sweep(ob.sweep)
+    s = np.arange(N); col = ((s % 224) + (s // 224) % 224 + s // (224 * 224)) & 1
+    for colour in (0, 1):
+        before = g.get_spins(); o.set_spins(before)
+        _, x_o, acc_o = o.half_sweep(T, colour, want_detail=True)
+        x_g, acc_g = g.half_sweep(T, colour, want_detail=True)
+        after_g = g.get_spins(); after_o = o.get_spins()
+        mine = col == colour
+        differ = mine & (acc_g != acc_o)
+        assert (np.abs(x_o[differ]) < 1e-5).all()
+        agree = mine & ~differ
+        assert np.abs(after_g[agree].astype(np.float64) - after_o[agree]).max() < 1e-4
+        assert (after_g[~mine] == before[~mine]).all()
+        near = mine & (np.abs(x_o) < 2.0)
+        print(f"\n224^3 T={T} cone={ob.cone_rad:.3f} colour {colour}: accepted {acc_g[mine].mean():.3f}, marginal flips {differ.sum()}, "
+              f"max |dx| near the boundary {np.abs(x_g[near] - x_o[near]).max():.2e}")
+        assert np.abs(x_g[near] - x_o[near]).max() < 1e-5
+    g.close()
+
+
+@pytest.mark.parametrize("colour", [0, 1])
+def test_full_size_c5_half_sweep_parity(mods, colour):
     """config c5: 2048 x 2048 x 4 granular film (16.8 M spins), Voronoi grains, per-grain axes, open z."""
     oracle, binding, inputs = mods
     shape = (2048, 2048, 4)
     mask, region, axes = inputs.voronoi_film(*shape, mean_diameter=40, seed=42)
-    _full_size_half_sweep(mods, shape, 0.5, 0.8, 43, dict(periodic=(1, 1, 0), Ku=0.02, bond_mask=mask, region=region, region_axis=axes))
+    _full_size_half_sweep(mods, shape, 0.5, 0.8, 43, dict(periodic=(1, 1, 0), Ku=0.02, bond_mask=mask, region=region, region_axis=axes), colour=colour)
 
 
+@pytest.mark.parametrize("colour", [0, 1])
 @pytest.mark.parametrize("L", [128, 224])
-def test_full_size_c4_constrained_half_sweep_parity(mods, L):
+def test_full_size_c4_constrained_half_sweep_parity(mods, L, colour):
     """config c4: 128^3, K_u = 0.05, constrained pass at theta = 45 deg; and the same pass on the 224^3 lattice on which
     bench.py times the constrained sweeps (other_paths)."""
     oracle, binding, inputs = mods
@@ -282,15 +317,15 @@ def test_full_size_c4_constrained_half_sweep_parity(mods, L):
     g.set_sweep(9); o.set_sweep(9)
     before = g.get_spins(); o.set_spins(before)
     ML = float((before.astype(np.float64) @ e).sum())
-    _, _, x_o, acc_o = o.constrained_half_sweep(T, e, 0, ML, want_detail=True)
-    x_g, acc_g = g.constrained_half_sweep(T, theta, 0.0, 0, ML, want_detail=True)
+    _, _, x_o, acc_o = o.constrained_half_sweep(T, e, colour, ML, want_detail=True)
+    x_g, acc_g = g.constrained_half_sweep(T, theta, 0.0, colour, ML, want_detail=True)
     after_g = g.get_spins().astype(np.float64); after_o = o.get_spins()
     lead = ~np.isnan(x_o)
     assert (lead == ~np.isnan(x_g)).all()                                  # identical pairing roles at full size
     differ = lead & (acc_g != acc_o)
     assert (np.abs(x_o[differ]) < 1e-5).all()
     s = np.arange(N); col = ((s % L) + (s // L) % L + s // (L * L)) & 1
-    same = (acc_g == acc_o) & (col == 0)
+    same = (acc_g == acc_o) & (col == colour)
     assert np.abs(after_g[same] - after_o[same]).max() < 1e-4
     fin = lead & np.isfinite(x_o) & np.isfinite(x_g)
     print(f"\nfull size {L}^3 constrained: pairs {lead.sum()}, accepted {acc_g[lead].mean():.3f}, flips {differ.sum()}, max |dx| {np.abs(x_g[fin]-x_o[fin]).max():.2e}")

@@ -31,10 +31,12 @@ def _colour(shape):
     return ((s % nx) + (s // nx) % ny + s // (nx * ny)) & 1
 
 
-def _pair(mods, shape, seed=42, cone=0.5, sweep=0, **ham):
+def _pair(mods, shape, seed=42, cone=0.5, sweep=0, path=None, **ham):
     oracle, binding, inputs = mods
     o = oracle.Oracle(*shape, seed=seed, cone0=cone, adaptive=False, **ham)
     g = binding.Lattice(*shape, seed=seed, cone0=cone, adaptive=False, **ham)
+    if path is not None:
+        g.debug_set_path(path)                              # documented test hook of include/mc.h (no environment variables)
     o.set_sweep(sweep); g.set_sweep(sweep)
     return o, g
 
@@ -92,15 +94,19 @@ TILED_CASES = [c for c in CASES if c[0] in ((96, 40, 36), (80, 30, 58))]
 
 
 @pytest.mark.parametrize("shape,T,cone,ham", TILED_CASES)
-def test_half_sweep_parity_forced_tiled_pass(mods, shape, T, cone, ham, monkeypatch):
-    monkeypatch.setenv("MC_B200_PATH", "tile")                 # read by mc_create
-    test_half_sweep_parity_random_state(mods, shape, T, cone, ham)
+def test_half_sweep_parity_forced_staged_pass(mods, shape, T, cone, ham):
+    test_half_sweep_parity_random_state(mods, shape, T, cone, ham, path=2)      # MC_PATH_STAGED
+
+
+@pytest.mark.parametrize("shape,T,cone,ham", [c for c in CASES if c[0] == (64, 64, 64)] + TILED_CASES)
+def test_half_sweep_parity_forced_generic_pass(mods, shape, T, cone, ham):
+    test_half_sweep_parity_random_state(mods, shape, T, cone, ham, path=1)      # MC_PATH_GENERIC
 
 
 @pytest.mark.parametrize("shape,T,cone,ham", CASES)
-def test_half_sweep_parity_random_state(mods, shape, T, cone, ham):
+def test_half_sweep_parity_random_state(mods, shape, T, cone, ham, path=None):
     oracle, binding, inputs = mods
-    o, g = _pair(mods, shape, cone=cone, sweep=(3 << 32) | 12345, **ham)
+    o, g = _pair(mods, shape, cone=cone, sweep=(3 << 32) | 12345, path=path, **ham)
     g.set_spins(inputs.random_unit_spins(g.N, seed=7))
     worst = 0.0; flips = 0
     for colour in (0, 1, 0, 1):
@@ -372,3 +378,102 @@ def test_align_rotation_matches_oracle(mods):
     ob = g.observables()
     assert np.allclose(np.array(ob.M) / ob.m, e, atol=1e-6)
     g.close()
+
+
+# ------------------------------------------------------------------------------------------ whole constrained sweeps (a-10)
+def test_constrained_sweep_equals_hooks_and_fused_ML_is_exact(mods):
+    """Constrained twin of test_sweep_equals_hooks_and_is_deterministic.  mc_constrained_sweep(T, theta, phi, 3) takes M_L of
+    every sweep from the fused fixed-point sums of the previous one (SURVEY a-10); the hook-assembled twin is handed
+    M_L = the fp64 sum of S_i.e_C of the same state (computed here with NumPy from mc_get_spins).
+      * the fused M (hence M_L = N M.e_C) of every sweep, read from the trace, equals the fp64 value of the post-sweep state
+        to 2e-7 per site -- an O(1/N) slip (one spin dropped or counted twice: 2.4e-4 per site here) fails;
+      * the two runs end in bit-identical spins (16^3: a decision inside the ~1e-7 band that the last-bit difference of the
+        two M_L values opens has probability ~1e-3 over the 6144 pair decisions; the seeds are fixed, so the outcome is too);
+      * acceptance and cone trace agree exactly."""
+    oracle, binding, inputs = mods
+    shape, T, theta, phi = (16, 16, 16), 0.8, 0.7, 0.4
+    N = 16 ** 3
+    e = np.array([np.sin(theta) * np.cos(phi), np.sin(theta) * np.sin(phi), np.cos(theta)])
+    s0 = inputs.thermal_like_spins(N, seed=2, spread=0.5, direction=e)
+    a = binding.Lattice(*shape, Ku=0.05, cone0=0.6, adaptive=True, seed=42); a.set_spins(s0)
+    b = binding.Lattice(*shape, Ku=0.05, cone0=0.6, adaptive=True, seed=42); b.set_spins(s0)
+    a.align_to(theta, phi); b.align_to(theta, phi)
+    assert (a.get_spins() == b.get_spins()).all()
+    states = []
+    for k in range(3):
+        a.constrained_sweep(T, theta, phi, 1)
+        states.append(a.get_spins())
+    tr = a.trace()
+    assert len(tr) == 3
+    for k in range(3):
+        M64 = states[k].astype(np.float64).sum(axis=0) / N
+        assert np.abs(tr[k, 2:5] - M64).max() < 2e-7, (k, tr[k, 2:5], M64)
+    for k in range(3):
+        cur = b.get_spins().astype(np.float64)
+        ML = float((cur @ e).sum())
+        b.constrained_half_sweep(T, theta, phi, 0, ML)
+        b.constrained_half_sweep(T, theta, phi, 1, ML)                    # stale M_L: the same value for both colours (P:38)
+        b.end_sweep()
+        assert (b.get_spins() == states[k]).all(), k
+    tb = b.trace()
+    assert (tb[:, :2] == tr[:, :2]).all() and np.abs(tb[:, 2:] - tr[:, 2:]).max() < 1e-9
+    # one call of 3 sweeps = three calls of 1 sweep, bitwise (P-20 for the constrained path)
+    c = binding.Lattice(*shape, Ku=0.05, cone0=0.6, adaptive=True, seed=42); c.set_spins(s0)
+    c.constrained_sweep(T, theta, phi, 3)
+    assert (c.get_spins() == states[2]).all() and (c.trace() == tr).all()
+    a.close(); b.close(); c.close()
+
+
+def test_unconstrained_sweeps_invalidate_the_alignment_on_the_gpu(mods):
+    """constrained -> mc_sweep -> constrained with the same (theta, phi): the library re-aligns (C-12), as the oracle does
+    (tests/test_oracle_align.py).  Without the re-alignment M stays tilted: the pair move conserves its transverse part."""
+    oracle, binding, inputs = mods
+    shape, T, theta, phi = (16, 16, 16), 1.0, 0.6, 0.3
+    e = np.array([np.sin(theta) * np.cos(phi), np.sin(theta) * np.sin(phi), np.cos(theta)])
+    g = binding.Lattice(*shape, Ku=0.05, cone0=0.6, adaptive=True, seed=5)
+    g.constrained_sweep(T, theta, phi, 20)
+    ob = g.observables(); assert np.abs(np.array(ob.M) / ob.m - e).max() < 2e-6
+    g.sweep(T, 40)
+    ob = g.observables(); assert np.abs(np.array(ob.M) / ob.m - e).max() > 1e-3
+    g.constrained_sweep(T, theta, phi, 5)
+    ob = g.observables(); assert np.abs(np.array(ob.M) / ob.m - e).max() < 2e-6
+    g.half_sweep(T, 0); g.half_sweep(T, 1); g.end_sweep()                 # the hooks invalidate it as well
+    g.constrained_sweep(T, theta, phi, 1)
+    ob = g.observables(); assert np.abs(np.array(ob.M) / ob.m - e).max() < 2e-6
+    g.close()
+
+
+def test_a_hook_without_end_sweep_does_not_leak_into_the_next_sweep(mods):
+    """include/mc.h: a half-sweep hook leaves its count and fused sums pending; mc_sweep discards them."""
+    oracle, binding, inputs = mods
+    shape = (16, 16, 16)
+    s0 = inputs.random_unit_spins(16 ** 3, seed=3)
+    a = binding.Lattice(*shape, Ku=0.01, cone0=2.5, adaptive=True, seed=7); a.set_spins(s0)
+    a.half_sweep(3.0, 0)                                                  # never closed: ~4096 * 0.5 * 0.9 accepted moves pending
+    b = binding.Lattice(*shape, Ku=0.01, cone0=2.5, adaptive=True, seed=7); b.set_spins(a.get_spins())   # a clean handle, same spins
+    a.sweep(3.0, 2); b.sweep(3.0, 2)
+    ta, tb = a.trace(), b.trace()
+    assert (a.get_spins() == b.get_spins()).all()
+    assert (ta == tb).all() and (ta[:, 0] <= 1.0).all()                   # acceptance, cone, M, E: nothing of the hook's pass is left
+    ob = a.observables()
+    assert np.abs(ta[-1, 2:5] - np.array(ob.M)).max() < 1e-6              # the fused M of the last sweep holds one sweep only
+    a.close(); b.close()
+
+
+def test_negative_zero_sz_takes_the_sign_bit_frame_on_every_path(mods):
+    """Reading C-29: sigma of the Duff frame is the sign bit of S_z.  Spins with S_z = -0.0 (and +0.0) on the scalar path
+    (VEC = 1), the packed generic path (VEC = 4) and the staged pass propose the oracle's trial spins."""
+    oracle, binding, inputs = mods
+    for shape, path in (((6, 4, 4), None), ((16, 16, 16), None), ((96, 40, 36), 2)):
+        N = shape[0] * shape[1] * shape[2]
+        s = inputs.random_unit_spins(N, seed=12)
+        s[0::3, 2] = -0.0; s[1::3, 2] = 0.0
+        s /= np.linalg.norm(s.astype(np.float64), axis=1, keepdims=True).astype(np.float32)
+        assert np.signbit(s[0::3, 2]).all() and not np.signbit(s[1::3, 2]).any()
+        o, g = _pair(mods, shape, cone=1.0, sweep=5, path=path, Ku=0.05)
+        g.set_spins(s)
+        got = g.get_spins()
+        assert np.signbit(got[0::3, 2]).all()                            # the upload keeps the sign bit
+        for colour in (0, 1):
+            _check_half_sweep(o, g, 1.0, colour, shape)
+        g.close()
