@@ -450,7 +450,9 @@ def test_a_hook_without_end_sweep_does_not_leak_into_the_next_sweep(mods):
     s0 = inputs.random_unit_spins(16 ** 3, seed=3)
     a = binding.Lattice(*shape, Ku=0.01, cone0=2.5, adaptive=True, seed=7); a.set_spins(s0)
     a.half_sweep(3.0, 0)                                                  # never closed: ~4096 * 0.5 * 0.9 accepted moves pending
-    b = binding.Lattice(*shape, Ku=0.01, cone0=2.5, adaptive=True, seed=7); b.set_spins(a.get_spins())   # a clean handle, same spins
+    snap = a.get_spins()
+    a.set_spins(snap)                                                     # the upload renormalises: both handles take the same one
+    b = binding.Lattice(*shape, Ku=0.01, cone0=2.5, adaptive=True, seed=7); b.set_spins(snap)            # a clean handle, same spins
     a.sweep(3.0, 2); b.sweep(3.0, 2)
     ta, tb = a.trace(), b.trace()
     assert (a.get_spins() == b.get_spins()).all()
