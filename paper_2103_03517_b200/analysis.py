@@ -59,3 +59,83 @@ def power_law_exponent(m, K, m_min: float = 0.0):
     sel = (m > m_min) & (K > 0) & (m < 1.0)
     k, lnK0 = np.polyfit(np.log(m[sel]), np.log(K[sel]), 1)
     return float(k), float(np.exp(lnK0))
+
+
+def anisotropy_scaling_easy_axis(E_aniso_per_site: float, Ku: float = 0.0, Kc: float = 0.0) -> float:
+    """Eq. (4): the anisotropy scaling k(T) = K(T)/K(0) from a STANDARD (unconstrained) run whose magnetisation
+    stays along an easy axis, through the average easy-axis anisotropy energy alone:
+        k_u = 1 - 3 K_easy / (2 K_0,hard),   k_c = 1 - 5 K_easy / (3 K_0,hard).
+    The paper measures the anisotropy energy from its minimum: K_easy = <E_aniso> - E_aniso(easy axis, T = 0) and
+    K_0,hard = E_aniso(hard axis, T = 0) - E_aniso(easy axis, T = 0).  With this library's Eq. (2) conventions
+    (uniaxial -Ku (S.e)^2: easy -Ku, hard 0; cubic +Kc (Sx^2 Sy^2 + Sy^2 Sz^2 + Sz^2 Sx^2): easy 0, hard <111> Kc/3)
+    that is K_easy = Ku + <E_aniso>, K_0,hard = Ku and K_easy = <E_aniso>, K_0,hard = Kc/3.  Both are the thermal averages
+    of the l = 2 / l = 4 harmonics, (3 <cos^2> - 1)/2 and 1 - 5 <Sx^2 Sy^2 + ...> (Callen-Callen).
+    `E_aniso_per_site` is mc_obs.E_aniso averaged over sampling sweeps; exactly one of Ku, Kc must be non-zero."""
+    if (Ku != 0.0) == (Kc != 0.0):
+        raise ValueError("exactly one of Ku, Kc")
+    if Ku != 0.0:
+        return 1.0 - 3.0 * (Ku + E_aniso_per_site) / (2.0 * Ku)
+    return 1.0 - 5.0 * E_aniso_per_site / (3.0 * (Kc / 3.0))
+
+
+def chi_perp_uniaxial(m: float, K_T: float) -> float:
+    """Eq. (7): transverse susceptibility of a uniaxial magnet below T_C, chi_perp = M_S(0) m^2 / (2 K_u(T)).
+    In the reduced units of `susceptibilities` (mu_S = k_B = 1, energies per spin, C-18) M_S(0) -> 1 per site and
+    K_u(T) -> K(T) = K k_u(T) per site, so chi_perp = m^2 / (2 K(T)); compare with the mean of the two hard-axis chi_alpha."""
+    if not K_T > 0.0:
+        raise ValueError("Eq. (7) holds for T < T_C where K(T) > 0")
+    return m * m / (2.0 * K_T)
+
+
+def multi_bloch(T, w, tc, beta):
+    """Right-hand side of Eq. (8): sum_i w_i (1 - T/T_C,i)^beta_i, a term vanishing above its own T_C,i."""
+    T = np.asarray(T, float)[:, None]
+    w = np.asarray(w, float)[None, :]; tc = np.asarray(tc, float)[None, :]; beta = np.asarray(beta, float)[None, :]
+    return (w * np.clip(1.0 - T / tc, 0.0, None) ** beta).sum(axis=1)
+
+
+def fit_multi_bloch(T, m, n_terms: int, tc_range=None, beta0: float = 0.34, seed: int = 0):
+    """Fit Eq. (8) with N_B = n_terms Bloch terms to a film's m(T): weights w_i >= 0 with sum 1, one
+    (T_C,i, beta_i) per term.  Returns (w, T_C, beta, Tbar_C, rms) with Tbar_C = sum_i w_i T_C,i (second line of Eq. 8).
+    Variable projection: for given (T_C,i, beta_i) the weights solve a non-negative least-squares problem with the
+    sum-to-one condition as a heavily weighted extra row; the outer least squares moves (T_C,i, beta_i) inside tc_range
+    (default: from the lowest T with m < 0.98 to 1.5 x the highest T) and [0.1, 1].  The paper increases N_B until
+    Tbar_C converges (N_B > 10 for its films)."""
+    from scipy.optimize import least_squares, nnls
+    T = np.asarray(T, float); m = np.asarray(m, float)
+    if tc_range is None:
+        lo = float(T[m < 0.98].min()) if (m < 0.98).any() else float(T.min())
+        tc_range = (max(lo, 1e-6), 1.5 * float(T.max()))
+    n = int(n_terms)
+    lam = 1e3
+
+    def weights(tc, beta):
+        A = np.clip(1.0 - T[:, None] / tc[None, :], 0.0, None) ** beta[None, :]
+        w, _ = nnls(np.vstack([A, lam * np.ones((1, n))]), np.concatenate([m, [lam]]))
+        s = w.sum()
+        return w / s if s > 0 else np.full(n, 1.0 / n)
+
+    def resid(p):
+        tc, beta = p[:n], p[n:]
+        return multi_bloch(T, weights(tc, beta), tc, beta) - m
+
+    lb = np.concatenate([np.full(n, tc_range[0]), np.full(n, 0.1)])
+    ub = np.concatenate([np.full(n, tc_range[1]), np.full(n, 1.0)])
+    span = tc_range[1] - tc_range[0]
+    # starting T_C,i: spread over the temperatures where m(T) falls (a term switches off at its own T_C,i)
+    falling = T[m > 1e-3]
+    t_hi = float(falling.max()) if falling.size else tc_range[1]
+    tc0 = np.clip(np.linspace(tc_range[0] + 0.5 * (t_hi - tc_range[0]), min(tc_range[1], t_hi * 1.1), n + 2)[1:-1], lb[:n], ub[:n])
+    p0 = np.concatenate([tc0, np.full(n, beta0)])
+    best = None
+    rng = np.random.default_rng(seed)
+    for trial in range(6):
+        start = p0 if trial == 0 else np.clip(p0 + np.concatenate([rng.normal(0, 0.08 * span, n), rng.normal(0, 0.05, n)]), lb, ub)
+        r = least_squares(resid, start, bounds=(lb, ub), x_scale=np.concatenate([np.full(n, 0.1 * span), np.full(n, 0.1)]))
+        if best is None or r.cost < best.cost:
+            best = r
+    tc, beta = best.x[:n], best.x[n:]
+    w = weights(tc, beta)
+    order = np.argsort(tc)
+    w, tc, beta = w[order], tc[order], beta[order]
+    return w, tc, beta, float((w * tc).sum()), float(np.sqrt(np.mean(best.fun ** 2)))

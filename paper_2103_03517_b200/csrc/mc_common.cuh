@@ -1,6 +1,6 @@
 // mc_common.cuh -- what every kernel of the checkerboard Metropolis path shares: the data layout, the controller /
 // reduction state, the colour indexing (a-1), the exchange-field gather (a-3) and the fused per-sweep reductions with the
-// cone controller (a-7, a-8, a-9).  The kernels: mc_pass.cuh (Table A1, generic), mc_tile.cuh / mc_ring.cuh (Table A1,
+// cone controller (a-7, a-8, a-9).  The kernels: mc_pass.cuh (Table A1, generic), mc_tile.cuh (Table A1,
 // staged), mc_pair.cuh (Table A2), mc_util.cuh (layout conversion, state edits, slice profile).
 //
 // Data layout in HBM: colour-split SoA fp32 planes.  For colour c and component k the plane
