@@ -51,13 +51,14 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-def recorded_traffic():
-    """dram bytes per colour-pass launch from the committed ncu --set full capture, if any (profiles/traffic.txt)."""
+def recorded_traffic(key="pass_kernel_dram_bytes_per_launch_warm"):
+    """dram bytes per colour-pass launch from the committed ncu captures, if any (profiles/traffic.txt): `warm` = back to back
+    as the timed region runs it (ncu --cache-control none), `cold` = ncu's default flushed-cache replay."""
     path = os.path.join(ROOT, "profiles", "traffic.txt")
     try:
         for line in open(path):
             t = line.split()
-            if t and t[0] == "pass_kernel_dram_bytes_per_launch":
+            if t and t[0] == key:
                 return float(t[1])
     except Exception:
         pass
@@ -187,11 +188,8 @@ def run_ours(args, rank, local_rank, world):
     from paper_2103_03517_b200 import binding, build, inputs
     build.build()
     torch.cuda.set_device(local_rank)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist_
-        dist = dist_
-        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
+    from paper_2103_03517_b200 import replicas
+    dist = replicas.init_distributed("nccl") if world > 1 else None      # plumbing only: barrier + max over ranks
 
     N = SHAPE[0] * SHAPE[1] * SHAPE[2]
     spp = args.sweeps_per_step
@@ -220,8 +218,7 @@ def run_ours(args, rank, local_rank, world):
     ms = ev0.elapsed_time(ev1)
     launches = g.launch_count() - l0
     clocks = sampler.stop() if rank == 0 else None
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); ms = float(t.item())
+    ms = replicas.max_over_ranks(ms, dist)
     value = world * N * spp * args.steps / (ms * 1e-3)
 
     # ---- end to end through the C ABI with host buffers: H2D of the state + sweeps + D2H of the observables, every step
@@ -238,8 +235,7 @@ def run_ours(args, rank, local_rank, world):
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
         e2e_s = dt if e2e_s is None else min(e2e_s, dt)
-    if dist is not None:
-        t = torch.tensor([e2e_s], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); e2e_s = float(t.item())
+    e2e_s = replicas.max_over_ranks(e2e_s, dist)
     e2e_value = world * N * spp * e2e_steps / e2e_s
 
     if rank != 0:
@@ -250,7 +246,7 @@ def run_ours(args, rank, local_rank, world):
     alg_bytes_per_launch = BYTES_PER_UPDATE * (N // 2)    # one launch updates one colour
     achieved = alg_bytes_per_launch / t_launch / 1e9
     roofline = {"bound": "hbm", "kernel": "tile_pass_kernel<ANISO=2, FIELD=0, RT=112> (one colour pass = one launch)", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": recorded_traffic(), "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": recorded_traffic(), "traffic_cold_cache": recorded_traffic("pass_kernel_dram_bytes_per_launch_cold"), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes_per_launch, "avg_launch_us": t_launch * 1e6,
                 "frac_of_nominal_8TBs": achieved / 8000.0}
 
@@ -272,7 +268,8 @@ def run_ours(args, rank, local_rank, world):
                        "sweeps_per_step": spp, "spins": N, "state_bytes": N * 12, "l2_policy": "inputs larger than L2 (134.9 MB state vs 126 MB L2)",
                        "parallelism": f"replicas x{world} (no collective)", "final_m": ob.m, "final_acceptance": ob.last_acceptance},
             "clocks": clocks,
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": N * 12, "d2h_bytes_per_step": DEV_STATE_BYTES, "steps": e2e_steps, "regions": "best of 2"},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": N * 12, "d2h_bytes_per_step": DEV_STATE_BYTES, "steps": e2e_steps, "regions": "best of 2",
+                    "sweeps_per_step": spp, "note": "one state upload (mc_set_spins, pinned host) and one mc_observables read-back per STEP of sweeps_per_step sweeps; a per-sweep upload would be PCIe-bound (134.9 MB at ~50 GB/s = 2.7 ms against ~90 us of compute)"},
             "gpu_launches": launches,
             "roofline": roofline,
             "cpu_baseline": cpu,
@@ -297,6 +294,13 @@ def main():
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                   # timing rule: W >= 3
     rank = int(os.environ.get("RANK", "0")); local_rank = int(os.environ.get("LOCAL_RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # not under a launcher: spawn one rank per GPU ourselves (what the driver's torchrun line does) and relay their output
+        import socket
+        sock = socket.socket(); sock.bind(("127.0.0.1", 0)); port = sock.getsockname()[1]; sock.close()
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+               "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        return subprocess.call(cmd)
     if args.impl == "reference":
         return run_reference(args, rank, world)
     return run_ours(args, rank, local_rank, world)

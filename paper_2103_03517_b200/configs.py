@@ -14,7 +14,7 @@ import time
 
 import numpy as np
 
-from . import analysis, binding, inputs
+from . import analysis, binding, inputs, replicas
 
 
 def _sync():
@@ -34,16 +34,24 @@ def c1(device="cuda:0"):
     return out
 
 
-def c2(device="cuda:0", L=64, equil=5000, sample=5000):
+def _c2_point(point, seed, device):
+    """One temperature point of c2: its own handle, +z start, `seed` = 42 + k (replicas.point_seed)."""
+    T, L, equil, sample = point
+    g = binding.Lattice(L, L, L, Ku=0.01, cone0=0.5, adaptive=True, seed=seed, device=device)
+    g.sweep(T, equil); g.reset_accumulators(); g.sweep(T, sample)
+    ob = g.observables()
+    chi = analysis.susceptibilities(ob, T)
+    g.close()
+    return {"m": ob.sum_m[0] / ob.n_samples, "chi_l": float(chi[0]), "chi_t": float(0.5 * (chi[1] + chi[2]))}
+
+
+def c2(device=None, L=64, equil=5000, sample=5000, dist=None):
+    """16 independent temperature points: dealt over the ranks by replicas.run_points (one rank: the plain loop)."""
     Ts = [0.1 * k for k in range(1, 17)]
-    m, chi_l, chi_t = [], [], []
-    for k, T in enumerate(Ts, start=1):
-        g = binding.Lattice(L, L, L, Ku=0.01, cone0=0.5, adaptive=True, seed=42 + k, device=device)   # +z start at every T
-        g.sweep(T, equil); g.reset_accumulators(); g.sweep(T, sample)
-        ob = g.observables()
-        chi = analysis.susceptibilities(ob, T)
-        m.append(ob.sum_m[0] / ob.n_samples); chi_l.append(float(chi[0])); chi_t.append(float(0.5 * (chi[1] + chi[2])))
-        g.close()
+    res = replicas.run_points([(T, L, equil, sample) for T in Ts], _c2_point, base_seed=42, dist=dist, device=device)
+    if res is None:
+        return None                                           # not rank 0
+    m, chi_l, chi_t = [r["m"] for r in res], [r["chi_l"] for r in res], [r["chi_t"] for r in res]
     tc_peak = Ts[int(np.argmax(chi_l))]
     below = [i for i, T in enumerate(Ts) if T < tc_peak and m[i] > 0.3]
     tc_fit, beta, _ = analysis.fit_bloch([Ts[i] for i in below], [m[i] for i in below])
@@ -69,18 +77,28 @@ def c3(device="cuda:0", L=224, sweeps=2000):
     return out
 
 
-def c4(device="cuda:0", L=128, sweeps=5000, discard=1000):
+def _c4_point(point, seed, device):
+    """One (T, theta) point of c4: +z start rotated onto e_C (C-12), seed 42 at every point as BASELINE.json states."""
+    T, th, L, sweeps, discard = point
+    g = binding.Lattice(L, L, L, Ku=0.05, cone0=0.5, adaptive=True, seed=42, device=device)
+    g.constrained_sweep(T, th, 0.0, discard); g.reset_accumulators(); g.constrained_sweep(T, th, 0.0, sweeps - discard)
+    ob = g.observables()
+    g.close()
+    return {"tau_y": ob.sum_torque[1] / ob.n_samples, "m": ob.sum_m[0] / ob.n_samples}
+
+
+def c4(device=None, L=128, sweeps=5000, discard=1000, dist=None):
+    """33 independent (T, theta) points through replicas.run_points."""
     thetas = np.deg2rad(np.arange(0, 91, 9))                  # 0..90 deg in 10 steps (C-20)
+    temps = (0.3, 0.8, 1.2)
+    res = replicas.run_points([(T, float(th), L, sweeps, discard) for T in temps for th in thetas], _c4_point, base_seed=42, dist=dist, device=device)
+    if res is None:
+        return None
     out = {"config": f"c4 {L}^3, Ku=0.05, constrained, theta=0..90 deg (11 points), T in (0.3, 0.8, 1.2), {sweeps} sweeps per point", "points": []}
     Ks, ms = [], []
-    for T in (0.3, 0.8, 1.2):
-        tau, mm = [], []
-        for th in thetas:
-            g = binding.Lattice(L, L, L, Ku=0.05, cone0=0.5, adaptive=True, seed=42, device=device)   # +z, rotated onto e_C (C-12)
-            g.constrained_sweep(T, th, 0.0, discard); g.reset_accumulators(); g.constrained_sweep(T, th, 0.0, sweeps - discard)
-            ob = g.observables()
-            tau.append(ob.sum_torque[1] / ob.n_samples); mm.append(ob.sum_m[0] / ob.n_samples)
-            g.close()
+    for i, T in enumerate(temps):
+        tau = [r["tau_y"] for r in res[i * len(thetas):(i + 1) * len(thetas)]]
+        mm = [r["m"] for r in res[i * len(thetas):(i + 1) * len(thetas)]]
         fit = thetas <= np.deg2rad(45.5)                     # towards the hard plane the uniform state of so large a lattice is not
         K = analysis.anisotropy_from_torque(thetas[fit], np.array(tau)[fit])   # stable over 5000 sweeps (|M| drops, domains): fit the stable branch
         Ks.append(K); ms.append(float(np.mean(np.array(mm)[fit])))
@@ -104,14 +122,25 @@ def c5(device="cuda:0", nx=2048, ny=2048, nz=4, sweeps=3000):
 
 
 def main(argv=None):
+    """python -m paper_2103_03517_b200.configs [c1 ...]; under torchrun the point loops of c2 / c4 are dealt over the ranks
+    (replicas), the single-lattice configs run on rank 0 only."""
     names = (argv or sys.argv[1:]) or ["c1", "c2", "c3", "c4", "c5"]
     table = {"c1": c1, "c2": c2, "c3": c3, "c4": c4, "c5": c5}
+    dist = replicas.init_distributed()
+    rank, local_rank, _ = replicas.world()
+    dev = f"cuda:{local_rank}"
     for n in names:
         t0 = time.perf_counter()
-        res = table[n]()
+        if n in ("c2", "c4"):
+            res = table[n](device=dev, dist=dist)
+        else:
+            res = table[n](device=dev) if rank == 0 else None
         _sync()
-        res["wall_s"] = round(time.perf_counter() - t0, 2)
-        print(json.dumps(res), flush=True)
+        if res is not None:
+            res["wall_s"] = round(time.perf_counter() - t0, 2)
+            print(json.dumps(res), flush=True)
+    if dist is not None:
+        dist.barrier(); dist.destroy_process_group()
     return 0
 
 
