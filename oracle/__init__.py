@@ -59,6 +59,8 @@ def lib():
     L.orc_cone_move.argtypes = [vp, dbl, dbl, dbl, vp]; L.orc_cone_move.restype = None
     L.orc_create.argtypes = [i32, i32, i32, vp, dbl, dbl, vp, dbl, vp, vp, vp, vp, i32, dbl, i32, u64]
     L.orc_create.restype = vp
+    L.orc_create_bcc.argtypes = [i32, i32, i32, vp, dbl, dbl, vp, dbl, vp, dbl, i32, u64]
+    L.orc_create_bcc.restype = vp
     L.orc_destroy.argtypes = [vp]; L.orc_destroy.restype = None
     for name in ("orc_set_spins", "orc_set_spins_f32", "orc_get_spins", "orc_init_uniform"):
         getattr(L, name).argtypes = [vp, vp]; getattr(L, name).restype = None
@@ -115,12 +117,23 @@ class Oracle:
     """One lattice + Hamiltonian + RNG seed, state in fp64 (lexicographic [N,3])."""
 
     def __init__(self, nx, ny, nz, periodic=(1, 1, 1), J=1.0, Ku=0.0, eu=(0, 0, 1), Kc=0.0, B=(0, 0, 0),
-                 bond_mask=None, region=None, region_axis=None, cone0=0.5, adaptive=True, seed=42):
+                 bond_mask=None, region=None, region_axis=None, cone0=0.5, adaptive=True, seed=42, structure="sc"):
         self.L = lib()
         self.shape = (nx, ny, nz)
-        self.N = nx * ny * nz
+        self.structure = structure
+        self.N = nx * ny * nz * (2 if structure == "bcc" else 1)
         per = np.asarray(periodic, dtype=np.int32)
         eu_ = np.asarray(eu, dtype=np.float64); B_ = np.asarray(B, dtype=np.float64)
+        if structure == "bcc":       # P:34: two sc sublattices = two colours; site = sublattice*nx*ny*nz + cell (reading C-30)
+            if bond_mask is not None or region is not None:
+                raise ValueError("bcc mode has no bond mask / regions")
+            self._mask = self._region = self._axis = None
+            self.h = self.L.orc_create_bcc(nx, ny, nz, _p(per), J, Ku, _p(eu_), Kc, _p(B_), float(cone0), int(bool(adaptive)), int(seed))
+            if not self.h:
+                raise ValueError("orc_create_bcc rejected the lattice")
+            return
+        if structure != "sc":
+            raise ValueError("structure must be 'sc' or 'bcc'")
         self._mask = None if bond_mask is None else np.ascontiguousarray(bond_mask, dtype=np.uint8).ravel()
         self._region = None if region is None else np.ascontiguousarray(region, dtype=np.uint16).ravel()
         self._axis = None if region_axis is None else np.ascontiguousarray(region_axis, dtype=np.float64)

@@ -26,6 +26,8 @@ static const double PI = 3.14159265358979323846;
 
 struct orc_ctx {
     int nx, ny, nz, periodic[3];
+    int structure;          /* 0 = simple cubic (the paper's lattice); 1 = body-centred cubic, see "bcc mode" below */
+    int64_t Ncell;          /* nx*ny*nz: sc N = Ncell; bcc N = 2 Ncell (site = sublattice*Ncell + cell)                    */
     int64_t N;
     double J, Ku, eu[3], Kc, B[3];
     uint8_t* mask;          /* NULL = all bonds allowed by the boundary conditions */
@@ -139,6 +141,51 @@ static void exchange_field(const orc_ctx* c, int x, int y, int z, double h[3])
     }
 }
 
+/* ------------------------------------------------------------------ bcc mode (reading C-30; "this approach can be
+ * extended to other crystal structures ... by considering the atomistic lattice as being composed of ... sub-lattices
+ * (e.g. 2 simple cubic sub-lattices for bcc ...)").  The conventional cubic cell (i,j,k) holds sublattice A (colour 0) at its
+ * corner (i,j,k) and sublattice B (colour 1) at its centre (i+1/2, j+1/2, k+1/2).  The 8 nearest neighbours of a site all lie
+ * in the OTHER sublattice, so the two sublattices are the two non-interacting subsets of the checkerboard scheme:
+ *   A(i,j,k) -- B(i-dx, j-dy, k-dz),   B(i,j,k) -- A(i+dx, j+dy, k+dz),   dx,dy,dz in {0,1}   (bond index k8 = dx + 2dy + 4dz).
+ * Site index = sublattice*Ncell + (i + nx*(j + ny*k)).  Periodic wrap per axis (n = 1: the same neighbour twice, as L = 2
+ * does in sc); an open axis drops the bonds that leave the box.  No bond mask, no regions, no anti-periodic wrap here. */
+static int64_t bcc_neighbour(const orc_ctx* c, int64_t site, int k8)
+{
+    int sub = (int)(site / c->Ncell); int64_t cell = site % c->Ncell;
+    int p[3] = { (int)(cell % c->nx), (int)((cell / c->nx) % c->ny), (int)(cell / ((int64_t)c->nx * c->ny)) };
+    int dim[3] = { c->nx, c->ny, c->nz }, d[3] = { k8 & 1, (k8 >> 1) & 1, (k8 >> 2) & 1 };
+    for (int a = 0; a < 3; ++a) {
+        p[a] += sub ? d[a] : -d[a];
+        if (p[a] < 0 || p[a] >= dim[a]) {
+            if (!c->periodic[a]) return -1;
+            p[a] = (p[a] + dim[a]) % dim[a];
+        }
+    }
+    return (int64_t)(1 - sub) * c->Ncell + p[0] + (int64_t)c->nx * (p[1] + (int64_t)c->ny * p[2]);
+}
+
+/* exchange field of ANY site, either structure (sc: decode the site and use the six-direction sum above) */
+static void field_at(const orc_ctx* c, int64_t site, double h[3])
+{
+    if (c->structure == 0) {
+        exchange_field(c, (int)(site % c->nx), (int)((site / c->nx) % c->ny), (int)(site / ((int64_t)c->nx * c->ny)), h);
+        return;
+    }
+    h[0] = h[1] = h[2] = 0.0;
+    for (int k = 0; k < 8; ++k) {
+        int64_t j = bcc_neighbour(c, site, k);
+        if (j < 0) continue;
+        for (int a = 0; a < 3; ++a) h[a] += c->J * c->S[3 * j + a];
+    }
+}
+
+/* colour of a site: sc (x+y+z) mod 2 with red = even first (C-10); bcc the sublattice */
+static int colour_of(const orc_ctx* c, int64_t site)
+{
+    if (c->structure) return (int)(site / c->Ncell);
+    return (int)((site % c->nx + (site / c->nx) % c->ny + site / ((int64_t)c->nx * c->ny)) & 1);
+}
+
 static const double* easy_axis(const orc_ctx* c, int64_t site)
 {
     return c->region ? &c->region_axis[3 * (int64_t)c->region[site]] : c->eu;
@@ -158,9 +205,8 @@ static double site_energy_h(const orc_ctx* c, int64_t site, const double h[3], c
 
 double orc_site_energy(const orc_ctx* c, int64_t site, const double S[3])
 {
-    int x = (int)(site % c->nx), y = (int)((site / c->nx) % c->ny), z = (int)(site / ((int64_t)c->nx * c->ny));
     double h[3];
-    exchange_field(c, x, y, z, h);
+    field_at(c, site, h);
     return site_energy_h(c, site, h, S);
 }
 
@@ -169,6 +215,23 @@ double orc_site_energy(const orc_ctx* c, int64_t site, const double S[3])
 double orc_total_energy(const orc_ctx* c)
 {
     double E = 0.0;
+    if (c->structure) {                      /* bcc: every bond joins an A and a B site: visit the 8 bonds of every A site */
+        for (int64_t i = 0; i < c->N; ++i) {
+            const double* S = &c->S[3 * i];
+            if (i < c->Ncell)
+                for (int k = 0; k < 8; ++k) {
+                    int64_t j = bcc_neighbour(c, i, k);
+                    if (j < 0) continue;
+                    const double* Sj = &c->S[3 * j];
+                    E -= c->J * (S[0] * Sj[0] + S[1] * Sj[1] + S[2] * Sj[2]);
+                }
+            double se = S[0] * c->eu[0] + S[1] * c->eu[1] + S[2] * c->eu[2];
+            double x2 = S[0] * S[0], y2 = S[1] * S[1], z2 = S[2] * S[2];
+            E += -c->Ku * se * se + c->Kc * (x2 * y2 + x2 * z2 + y2 * z2)
+                 - (S[0] * c->B[0] + S[1] * c->B[1] + S[2] * c->B[2]);
+        }
+        return E;
+    }
     for (int z = 0; z < c->nz; ++z) for (int y = 0; y < c->ny; ++y) for (int x = 0; x < c->nx; ++x) {
         int64_t i = site_index(c, x, y, z);
         const double* S = &c->S[3 * i];
@@ -202,7 +265,7 @@ orc_ctx* orc_create(int nx, int ny, int nz, const int periodic[3],
     orc_ctx* c = (orc_ctx*)calloc(1, sizeof(orc_ctx));
     c->nx = nx; c->ny = ny; c->nz = nz;
     for (int a = 0; a < 3; ++a) c->periodic[a] = periodic[a];
-    c->N = (int64_t)nx * ny * nz;
+    c->N = (int64_t)nx * ny * nz; c->Ncell = c->N; c->structure = 0;
     c->J = J; c->Ku = Ku; c->Kc = Kc;
     double n = sqrt(eu[0] * eu[0] + eu[1] * eu[1] + eu[2] * eu[2]);
     for (int a = 0; a < 3; ++a) { c->eu[a] = (n > 0) ? eu[a] / n : (a == 2); c->B[a] = B[a]; }
@@ -217,6 +280,27 @@ orc_ctx* orc_create(int nx, int ny, int nz, const int periodic[3],
             for (int a = 0; a < 3; ++a) c->region_axis[3 * r + a] = v[a] / m;
         }
     }
+    c->cone = cone0_rad; c->adaptive = adaptive; c->seed = seed; c->sweep = 0; c->sampling = 1;
+    c->S = (double*)malloc(sizeof(double) * 3 * c->N);
+    for (int64_t i = 0; i < c->N; ++i) { c->S[3 * i] = 0; c->S[3 * i + 1] = 0; c->S[3 * i + 2] = 1; }
+    return c;
+}
+
+/* bcc lattice of nx x ny x nz conventional cells, 2 nx ny nz spins (bcc mode above).  Any dimension may be periodic (1) or
+ * open (0) and need not be even: the two sublattices are the two colours whatever the size. */
+orc_ctx* orc_create_bcc(int nx, int ny, int nz, const int periodic[3],
+                        double J, double Ku, const double eu[3], double Kc, const double B[3],
+                        double cone0_rad, int adaptive, uint64_t seed)
+{
+    if (nx < 1 || ny < 1 || nz < 1) return NULL;
+    for (int a = 0; a < 3; ++a) if (periodic[a] < 0 || periodic[a] > 1) return NULL;
+    orc_ctx* c = (orc_ctx*)calloc(1, sizeof(orc_ctx));
+    c->nx = nx; c->ny = ny; c->nz = nz; c->structure = 1;
+    for (int a = 0; a < 3; ++a) c->periodic[a] = periodic[a];
+    c->Ncell = (int64_t)nx * ny * nz; c->N = 2 * c->Ncell;
+    c->J = J; c->Ku = Ku; c->Kc = Kc;
+    double n = sqrt(eu[0] * eu[0] + eu[1] * eu[1] + eu[2] * eu[2]);
+    for (int a = 0; a < 3; ++a) { c->eu[a] = (n > 0) ? eu[a] / n : (a == 2); c->B[a] = B[a]; }
     c->cone = cone0_rad; c->adaptive = adaptive; c->seed = seed; c->sweep = 0; c->sampling = 1;
     c->S = (double*)malloc(sizeof(double) * 3 * c->N);
     for (int64_t i = 0; i < c->N; ++i) { c->S[3 * i] = 0; c->S[3 * i + 1] = 0; c->S[3 * i + 2] = 1; }
@@ -266,6 +350,10 @@ static void site_uniforms_tag(const orc_ctx* c, int x, int y, int z, uint32_t ta
 {
     int64_t first = site_index(c, x & ~2, y, z);
     int half = (x >> 1) & 1;
+    if (c->structure) {      /* bcc (C-30): the same-sublattice x-neighbours i and i ^ 1 share the block; (x,y,z) = cell, colour = sublattice */
+        first = (int64_t)colour * c->Ncell + site_index(c, x & ~1, y, z);
+        half = x & 1;
+    }
     uint32_t r[4];
     draw(c, (uint32_t)first, tag, colour, sweep, r);
     uint32_t w0 = r[2 * half], w1 = r[2 * half + 1];
@@ -288,11 +376,12 @@ void orc_pair_uniforms(const orc_ctx* c, int x, int y, int z, int colour, uint64
 static int metropolis_update(orc_ctx* c, int x, int y, int z, int colour, double T, double* xdec)
 {
     int64_t i = site_index(c, x, y, z);                       /* P:155  i = Get_Red(Black)SpinIndex(index) */
+    if (c->structure) i += (int64_t)colour * c->Ncell;        /* bcc: (x,y,z) is the cell, colour the sublattice */
     double u0, u1, u2;
     orc_site_uniforms(c, x, y, z, colour, c->sweep, &u0, &u1, &u2);   /* P:156-157 UniformRandom() x 3 (C-8, C-26) */
     double* S = &c->S[3 * i], Sn[3], h[3];
     orc_cone_move(S, c->cone, u0, u1, Sn);                    /* P:156  S_new = UniformRandom_RotateSpin(S_i, theta) */
-    exchange_field(c, x, y, z, h);
+    field_at(c, i, h);
     double dE = site_energy_h(c, i, h, Sn) - site_energy_h(c, i, h, S);   /* P:158  E(S_new) - E(S_i) */
     double xd = dE / T + log(u2);                             /* P:157-158  P < exp(-dE/kT)  <=>  dE/T + ln P < 0  (C-8) */
     if (xdec) xdec[i] = xd;
@@ -305,9 +394,9 @@ int64_t orc_half_sweep(orc_ctx* c, double T, int colour, double* xdec, uint8_t* 
     int64_t count = 0;
     c->aligned = 0;   /* an unconstrained pass moves M off e_C: the next constrained sweep re-aligns (reading C-12) */
     for (int z = 0; z < c->nz; ++z) for (int y = 0; y < c->ny; ++y) for (int x = 0; x < c->nx; ++x) {
-        if (((x + y + z) & 1) != colour) continue;            /* red = even (C-10) */
+        if (!c->structure && ((x + y + z) & 1) != colour) continue;   /* sc: red = even (C-10); bcc: every cell holds one site of each colour */
         int a = metropolis_update(c, x, y, z, colour, T, xdec);
-        if (acc) acc[site_index(c, x, y, z)] = (uint8_t)a;
+        if (acc) acc[site_index(c, x, y, z) + (c->structure ? (int64_t)colour * c->Ncell : 0)] = (uint8_t)a;
         count += a;
     }
     return count;
@@ -332,11 +421,10 @@ void orc_profile_x(const orc_ctx* c, double* out)
 static void measure(const orc_ctx* c, orc_obs* o)
 {
     double M[3] = { 0, 0, 0 }, Eex = 0, Ean = 0, Ez = 0, tq[3] = { 0, 0, 0 };
-    for (int z = 0; z < c->nz; ++z) for (int y = 0; y < c->ny; ++y) for (int x = 0; x < c->nx; ++x) {
-        int64_t i = site_index(c, x, y, z);
+    for (int64_t i = 0; i < c->N; ++i) {                      /* lexicographic site order (sc: x fastest) */
         const double* S = &c->S[3 * i];
         double h[3];
-        exchange_field(c, x, y, z, h);
+        field_at(c, i, h);
         for (int a = 0; a < 3; ++a) M[a] += S[a];
         Eex += -0.5 * (S[0] * h[0] + S[1] * h[1] + S[2] * h[2]);          /* every bond once (C-1) */
         const double* e = easy_axis(c, i);
@@ -410,8 +498,9 @@ void orc_sweep_random_order(orc_ctx* c, double T, int64_t n)
         int64_t count = 0;
         for (int64_t k = 0; k < c->N; ++k) {
             int64_t s = order[k];
-            int x = (int)(s % c->nx), y = (int)((s / c->nx) % c->ny), z = (int)(s / ((int64_t)c->nx * c->ny));
-            count += metropolis_update(c, x, y, z, (x + y + z) & 1, T, NULL);
+            int64_t cell = s % c->Ncell;
+            int x = (int)(cell % c->nx), y = (int)((cell / c->nx) % c->ny), z = (int)(cell / ((int64_t)c->nx * c->ny));
+            count += metropolis_update(c, x, y, z, colour_of(c, s), T, NULL);
         }
         orc_end_sweep(c, count);
     }
@@ -423,6 +512,7 @@ void orc_sweep_random_order(orc_ctx* c, double T, int64_t n)
 /* colour-linear index: a = (x>>1) + (nx/2)*(y + ny*z) enumerates the sites of one colour (nx even). */
 int64_t orc_site_of(const orc_ctx* c, int colour, int64_t a)
 {
+    if (c->structure) return (int64_t)colour * c->Ncell + a;   /* bcc: a sublattice is stored contiguously */
     int hx = c->nx / 2;
     int xh = (int)(a % hx); int64_t row = a / hx;
     int y = (int)(row % c->ny), z = (int)(row / c->ny);
@@ -440,6 +530,7 @@ int64_t orc_site_of(const orc_ctx* c, int colour, int64_t a)
  * Replaces the paper's shuffled index array; requirements R1-R4 in DESIGN.md. */
 int orc_pairing(const orc_ctx* c, uint64_t sweep, int colour, int64_t* partner, uint8_t* is_leader)
 {
+    if (c->structure) return -1;                             /* the constrained path is built for the sc lattice only */
     if (c->nx & 1) return -1;
     int64_t Nc = c->N / 2;
     if (Nc & 1) return -1;                                   /* C-15 */

@@ -57,6 +57,12 @@ orc_ctx* orc_create(int nx, int ny, int nz, const int periodic[3],
                     const uint8_t* bond_mask, const uint16_t* region,
                     const double* region_axis, int n_regions,
                     double cone0_rad, int adaptive, uint64_t seed);
+/* Body-centred cubic lattice (two simple cubic sublattices = the two colours; reading C-30 in DESIGN.md): nx x ny x nz
+ * conventional cells, 2 nx ny nz spins, 8 nearest neighbours, site = sublattice*nx*ny*nz + (i + nx*(j + ny*k)).
+ * periodic[a] in {0,1}; no mask / regions; the constrained calls return an error in this mode. */
+orc_ctx* orc_create_bcc(int nx, int ny, int nz, const int periodic[3],
+                        double J, double Ku, const double eu[3], double Kc, const double B[3],
+                        double cone0_rad, int adaptive, uint64_t seed);
 void orc_destroy(orc_ctx*);
 /* periodic[a]: 0 open faces, 1 periodic, 2 anti-periodic (the spin across the wrap enters as -S_j). */
 /* Slice-averaged magnetisation along x: out[3*x + a], a = x,y,z component. */
