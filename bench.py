@@ -178,6 +178,17 @@ def time_other_paths(binding, torch, local_rank, sweeps=100):
     out["c5_film_2048x2048x4_T0.5"] = {"value": ups, "unit": UNIT, "us_per_sweep": 1e3 * ms / sweeps, "algorithmic_GBs": 39 * ups / 1e9,
                                        "kernel": "pass_kernel<4, uniaxial, masked> (generic)"}
     g.close()
+    # bcc lattice: 176^3 conventional cells = 10.9 M spins, 8 neighbours, the two sublattices as colours
+    Lb = 176
+    g = binding.Lattice(Lb, Lb, Lb, Ku=0.01, cone0=0.5, adaptive=True, seed=42, structure="bcc", device=f"cuda:{local_rank}")
+    g.init_spins(2); g.sweep(1.8, 10)
+    torch.cuda.synchronize()
+    e0.record(); g.sweep(1.8, sweeps); e1.record(); torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    ups = g.N * sweeps / (ms * 1e-3)
+    out["bcc_176^3_cells_Ku0.01_T1.8"] = {"value": ups, "unit": UNIT, "us_per_sweep": 1e3 * ms / sweeps, "algorithmic_GBs": BYTES_PER_UPDATE * ups / 1e9,
+                                        "kernel": "pass_kernel<4, uniaxial, bcc> (generic gather, 8 neighbours)"}
+    g.close()
     return out
 
 

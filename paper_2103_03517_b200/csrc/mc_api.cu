@@ -33,6 +33,12 @@ bool valid_lattice(const mc_lattice* lat)
 {
     if (!lat) return false;
     const int dim[3] = { lat->nx, lat->ny, lat->nz };
+    if (lat->structure == MC_BCC) {          // P:34, C-30: fully periodic, rows of float4 items
+        for (int a = 0; a < 3; ++a) if (dim[a] < 1 || lat->periodic[a] != 1) return false;
+        if (lat->nx % 4) return false;
+        return 2.0 * (double)lat->nx * lat->ny * lat->nz < 2147483648.0;
+    }
+    if (lat->structure != MC_SC) return false;
     for (int a = 0; a < 3; ++a) {
         if (dim[a] < 1) return false;
         if (lat->periodic[a] && (dim[a] & 1)) return false;
@@ -46,7 +52,8 @@ bool valid_lattice(const mc_lattice* lat)
 Layout make_layout(const mc_lattice* lat, const mc_hamiltonian* ham)
 {
     Layout L{};
-    const size_t Nc = (size_t)lat->nx / 2 * lat->ny * lat->nz;
+    const bool bcc = lat->structure == MC_BCC;
+    const size_t Nc = bcc ? (size_t)lat->nx * lat->ny * lat->nz : (size_t)lat->nx / 2 * lat->ny * lat->nz;
     L.plane = (long long)round_up(Nc, 64);
     L.mask_plane = (long long)round_up(Nc, 256);
     L.region_plane = (long long)round_up(Nc, 128);
@@ -60,7 +67,7 @@ Layout make_layout(const mc_lattice* lat, const mc_hamiltonian* ham)
     L.trace = off;    off += round_up((size_t)TRACE_CAP * 6 * sizeof(double), ALIGN);
     // staging: the [N][3] fp32 lexicographic image of the state during mc_set_spins / mc_get_spins, or the [N] fp32 + [N] u8
     // outputs of a half-sweep hook, or the 3 nx int64 sums of mc_profile_x -- the library allocates nothing itself
-    const size_t N = (size_t)lat->nx * lat->ny * lat->nz;
+    const size_t N = 2 * Nc;
     L.staging_bytes = round_up(N * 3 * sizeof(float), ALIGN) + round_up((size_t)lat->nx * 3 * sizeof(long long), ALIGN);
     L.staging = off;  off += L.staging_bytes;
     L.total = off;
@@ -164,6 +171,7 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     *out = nullptr;
     if (!valid_lattice(lat) || !ham || !dev_workspace) return MC_EINVAL;
     if (ham->region && (ham->n_regions < 1 || ham->n_regions > 65536 || !ham->region_axis)) return MC_EINVAL;
+    if (lat->structure == MC_BCC && (ham->bond_mask || ham->region)) return MC_EINVAL;
     if (((uintptr_t)dev_workspace) % ALIGN) return MC_EINVAL;
     const Layout L = make_layout(lat, ham);
     if (workspace_bytes < L.total) return MC_EINVAL;
@@ -189,11 +197,13 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     if (cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return bail(MC_ECUDA, "cannot query the device");
 
     const int nx = lat->nx, ny = lat->ny, nz = lat->nz;
-    const uint32_t N = (uint32_t)nx * ny * nz, R = nx / 2, Nc = N / 2;
+    const bool bcc = lat->structure == MC_BCC;
+    const uint32_t N = (uint32_t)nx * ny * nz * (bcc ? 2u : 1u), R = bcc ? nx : nx / 2, Nc = N / 2;
     char* ws = (char*)dev_workspace;
     Params& P = ctx->P;
     P.nx = nx; P.ny = ny; P.nz = nz; P.R = (int)R; P.Nc = Nc; P.N = N; P.invN = 1.0 / (double)N;
     P.anti_x = lat->periodic[0] == 2 ? 1 : 0;
+    P.bcc = bcc ? 1 : 0;
     P.plane = L.plane; P.S = (float*)(ws + L.spins);
     P.mask = nullptr; P.mask_plane = L.mask_plane; P.region = nullptr; P.region_plane = L.region_plane; P.axis = nullptr;
     P.J = (float)ham->J; P.Ku = (float)ham->Ku; P.Kc = (float)ham->Kc;
@@ -214,13 +224,13 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     ctx->aniso = (ham->Ku != 0.0 ? 1 : 0) | (ham->Kc != 0.0 ? 2 : 0);
     ctx->field = ham->B[0] != 0.0 || ham->B[1] != 0.0 || ham->B[2] != 0.0;
     ctx->masked = needs_mask(lat, ham);
-    ctx->vec = (nx % 8 == 0) ? 4 : 1;
+    ctx->vec = (bcc || nx % 8 == 0) ? 4 : 1;
     ctx->geom.RV = R / ctx->vec; ctx->geom.n_items = Nc / ctx->vec;
     ctx->geom.div_rv = make_div(ctx->geom.RV); ctx->geom.div_nz = make_div((uint32_t)nz);
     { uint32_t sh = 0; while (sh < 5 && ny % (2 << sh) == 0) ++sh; ctx->geom.yb_shift = sh; }      // up to 32 rows per block
 
     // pairing geometry (C-11); the constrained path needs an even colour population (C-15)
-    ctx->pair_ok = (Nc % 2 == 0) && Nc >= 2;
+    ctx->pair_ok = (Nc % 2 == 0) && Nc >= 2 && !bcc;          // the constrained path is built for the sc lattice
     if (ctx->pair_ok) {
         PairGeom& G = ctx->pgeom;
         uint32_t Bc = 32; while (Nc % (2 * Bc)) Bc >>= 1;
@@ -469,7 +479,7 @@ int mc_constrained_sweep(mc_ctx* ctx, double T, double theta, double phi, int64_
 {
     CHECK_CTX();
     if (!(T > 0.0) || n < 0) return fail(ctx, MC_EINVAL, "mc_constrained_sweep: need T > 0 and n >= 0");
-    if (!ctx->pair_ok) return fail(ctx, MC_EINVAL, "mc_constrained_sweep: odd number of sites per colour (C-15)");
+    if (!ctx->pair_ok) return fail(ctx, MC_EINVAL, "mc_constrained_sweep: needs a simple cubic lattice with an even number of sites per colour (C-15)");
     int rc;
     if (!ctx->aligned || theta != ctx->theta || phi != ctx->phi) { if ((rc = mc_align_to(ctx, theta, phi))) return rc; }
     if (n == 0) return MC_OK;
@@ -509,7 +519,7 @@ static int hook_common(mc_ctx* ctx, int colour, float* host_x, uint8_t* host_acc
     const int nx = ctx->P.nx, ny = ctx->P.ny;
     for (uint32_t s = 0; s < N; ++s) {
         const int x = s % nx, y = (s / nx) % ny, z = s / ((uint32_t)nx * ny);
-        if (((x + y + z) & 1) != colour) continue;
+        if ((ctx->P.bcc ? (int)(s >= ctx->P.Nc) : ((x + y + z) & 1)) != colour) continue;      // bcc: colour = sublattice
         if (host_x) host_x[s] = hx[s];
         if (host_acc) host_acc[s] = ha[s];
     }
@@ -579,6 +589,7 @@ int mc_profile_x(mc_ctx* ctx, double* host_profile)
 {
     CHECK_CTX();
     if (!host_profile) return fail(ctx, MC_EINVAL, "mc_profile_x: null pointer");
+    if (ctx->P.bcc) return fail(ctx, MC_EINVAL, "mc_profile_x: simple cubic lattices only");
     const int nx = ctx->P.nx;
     const size_t bytes = (size_t)nx * 3 * sizeof(long long);
     long long* tmp = (long long*)((char*)ctx->staging + ctx->staging_bytes - round_up(bytes, ALIGN));   // tail of the staging area

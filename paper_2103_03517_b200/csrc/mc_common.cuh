@@ -45,6 +45,7 @@ struct DevState {
 struct Params {
     int nx, ny, nz, R;               // R = nx/2 sites of one colour per row
     int anti_x;                      // 1: anti-periodic boundary along x (domain-wall box); the wrap bond sees -S_j
+    int bcc;                         // 1: body-centred cubic (C-30): colour = sublattice, R = nx cells per row, 8 neighbours
     uint32_t Nc;                     // sites per colour
     uint32_t N;
     double invN;                     // 1 / N (host-computed: keeps an fp64 division off the finalising thread)
@@ -213,6 +214,61 @@ __device__ __forceinline__ void exchange_field(const Params& P, const ItemPos& q
     }
 #pragma unroll
     for (int k = 0; k < VEC; ++k) h[k] = { hc[0][k], hc[1][k], hc[2][k] };
+}
+
+// --------------------------------------------------------------------------------------------------------------
+// bcc (C-30): the two simple cubic sublattices are the two colours; each is stored as a full nx x ny x nz grid in
+// cell order a = i + nx (j + ny k) (R = nx).  The 8 neighbours of A(i,j,k) are B(i-dx, j-dy, k-dz), those of B(i,j,k) are
+// A(i+dx, j+dy, k+dz): the cells i and i -+ 1 of four rows of the other sublattice.  An item is 4 consecutive cells of a row:
+// per row one float4 plus the one value just outside the item.  Fully periodic lattices only.
+// Site ids (Philox counters, debug outputs): sublattice*Ncell + cell; the cells i, i ^ 1 share a Philox block (C-30).
+// --------------------------------------------------------------------------------------------------------------
+struct BccPos {
+    uint32_t a0, site0;              // cell index of the first cell of the item; its site id
+    uint32_t row[4];                 // first cell of the rows (j, k), (j', k), (j, k'), (j', k') of the other sublattice; ' = -1 (A) / +1 (B)
+    uint32_t xe;                     // in-row cell of the value outside the item: i0 - 1 (A) or i0 + 4 (B), wrapped
+    uint32_t i0;
+};
+__device__ __forceinline__ BccPos bcc_locate(const Params& P, const Geom& G, uint32_t item, int colour)
+{
+    uint32_t rowp, xq, z, y;
+    G.div_rv.divmod(item, rowp, xq);
+    const uint32_t nx = (uint32_t)P.nx, ny = (uint32_t)P.ny, nz = (uint32_t)P.nz;
+    z = rowp / ny; y = rowp - z * ny;
+    BccPos q;
+    q.i0 = xq * 4u;
+    q.a0 = rowp * nx + q.i0;
+    q.site0 = (uint32_t)colour * P.Nc + q.a0;
+    const uint32_t y2 = colour ? (y + 1 == ny ? 0u : y + 1) : (y == 0 ? ny - 1 : y - 1);
+    const uint32_t z2 = colour ? (z + 1 == nz ? 0u : z + 1) : (z == 0 ? nz - 1 : z - 1);
+    q.row[0] = (z * ny + y) * nx;  q.row[1] = (z * ny + y2) * nx;
+    q.row[2] = (z2 * ny + y) * nx; q.row[3] = (z2 * ny + y2) * nx;
+    q.xe = colour ? (q.i0 + 4 == nx ? 0u : q.i0 + 4) : (q.i0 == 0 ? nx - 1 : q.i0 - 1);
+    return q;
+}
+// h = sum of the 8 neighbours (WITHOUT the factor J), in a fixed order: rows 0..3, in each the cell i then the cell i -+ 1
+__device__ __forceinline__ void bcc_exchange_field(const Params& P, const BccPos& q, int colour, Vec3 (&h)[4])
+{
+    const float* O = P.S + (long long)(1 - colour) * 3 * P.plane;
+    float hc[3][4];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float* Oc = O + (long long)c * P.plane;
+        f2 lo = splat(0.0f), hi = splat(0.0f);
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const Pack<4> o = ld_nc<4>(Oc + q.row[r] + q.i0);
+            const float ex = __ldg(Oc + q.row[r] + q.xe);
+            // shifted neighbour: cell i - 1 (sublattice A) or i + 1 (sublattice B)
+            const f2 slo = colour ? make_float2(o.v[1], o.v[2]) : make_float2(ex, o.v[0]);
+            const f2 shi = colour ? make_float2(o.v[3], ex) : make_float2(o.v[1], o.v[2]);
+            lo = add2(lo, add2(make_float2(o.v[0], o.v[1]), slo));
+            hi = add2(hi, add2(make_float2(o.v[2], o.v[3]), shi));
+        }
+        hc[c][0] = lo.x; hc[c][1] = lo.y; hc[c][2] = hi.x; hc[c][3] = hi.y;
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) h[k] = { hc[0][k], hc[1][k], hc[2][k] };
 }
 
 // easy axes of the VEC sites of an item: uniform, or per grain through the region table (config c5)

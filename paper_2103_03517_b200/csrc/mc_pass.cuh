@@ -15,7 +15,8 @@ namespace mc {
 #ifndef MC_PASS_MIN_BLOCKS
 #define MC_PASS_MIN_BLOCKS 3      // <= 80 registers: three CTAs per SM (c5 film: one 354, two 185, three 166 us per sweep)
 #endif
-template <int VEC, int ANISO, bool MASKED, int MODE>
+// BCC: the bcc lattice of P:34 (mc_common.cuh): VEC = 4 consecutive cells of one sublattice, site stride 1 instead of 2.
+template <int VEC, int ANISO, bool MASKED, int MODE, bool BCC = false>
 __global__ void __launch_bounds__(BLOCK, MC_PASS_MIN_BLOCKS)
 pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, int colour, float invT, int flags,
             float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
@@ -37,10 +38,19 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
 
     const uint32_t stride = gridDim.x * BLOCK;
     for (uint32_t item = blockIdx.x * BLOCK + threadIdx.x; item < G.n_items; item += stride) {
-        const ItemPos q = locate<VEC>(P, G, item, colour);
-        const Pack<VEC> sx = ld_rw<VEC>(Sc + q.a0), sy = ld_rw<VEC>(Sc + P.plane + q.a0), sz = ld_rw<VEC>(Sc + 2 * P.plane + q.a0);
+        static_assert(!BCC || (VEC == 4 && !MASKED), "the bcc pass is the VEC = 4, unmasked instantiation");
+        constexpr uint32_t SS = BCC ? 1u : 2u;                    // site-id stride between the sites of an item
+        ItemPos q;
         Vec3 h[VEC], e[VEC];
-        exchange_field<VEC, MASKED>(P, q, colour, h);
+        if (BCC) {
+            const BccPos b = bcc_locate(P, G, item, colour);
+            q.a0 = b.a0; q.site0 = b.site0; q.xh0 = b.i0; q.par = 0u;
+            if (VEC == 4) bcc_exchange_field(P, b, colour, reinterpret_cast<Vec3(&)[4]>(h));
+        } else {
+            q = locate<VEC>(P, G, item, colour);
+            exchange_field<VEC, MASKED>(P, q, colour, h);
+        }
+        const Pack<VEC> sx = ld_rw<VEC>(Sc + q.a0), sy = ld_rw<VEC>(Sc + P.plane + q.a0), sz = ld_rw<VEC>(Sc + 2 * P.plane + q.a0);
         if (ANISO & 1) easy_axes<VEC>(P, q, colour, e);
         Pack<VEC> nxv = sx, nyv = sy, nzv = sz;
         float f[NQ];
@@ -56,7 +66,7 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
                 w0[0] = half ? r2 : r0; w1[0] = half ? r3 : r1;
             } else {
 #pragma unroll
-                for (int k = 0; k + 1 < VEC; k += 2) philox4x32_10(key, q.site0 + 2u * k, c1, c2, c3, w0[k], w1[k], w0[k + 1], w1[k + 1]);
+                for (int k = 0; k + 1 < VEC; k += 2) philox4x32_10(key, q.site0 + SS * k, c1, c2, c3, w0[k], w1[k], w0[k + 1], w1[k + 1]);
             }
         }
         if (VEC == 4 && MODE == MODE_SWEEP) {
@@ -85,8 +95,8 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
                 S.z = make_float2(ok0 ? Sn.z.x : S.z.x, ok1 ? Sn.z.y : S.z.y);
                 nxv.v[kp] = S.x.x; nxv.v[kp + 1] = S.x.y; nyv.v[kp] = S.y.x; nyv.v[kp + 1] = S.y.y; nzv.v[kp] = S.z.x; nzv.v[kp + 1] = S.z.y;
                 cnt += (int)ok0 + (int)ok1;
-                if (dbg_x)   { dbg_x[q.site0 + 2u * kp] = xx.x; dbg_x[q.site0 + 2u * kp + 2u] = xx.y; }
-                if (dbg_acc) { dbg_acc[q.site0 + 2u * kp] = (uint8_t)ok0; dbg_acc[q.site0 + 2u * kp + 2u] = (uint8_t)ok1; }
+                if (dbg_x)   { dbg_x[q.site0 + SS * kp] = xx.x; dbg_x[q.site0 + SS * kp + SS] = xx.y; }
+                if (dbg_acc) { dbg_acc[q.site0 + SS * kp] = (uint8_t)ok0; dbg_acc[q.site0 + SS * kp + SS] = (uint8_t)ok1; }
                 f2s[0] = add2(f2s[0], S.x); f2s[1] = add2(f2s[1], S.y); f2s[2] = add2(f2s[2], S.z);
                 if (colour == 1) f2s[3] = sub2(f2s[3], dot3p(S, hJ));
                 if (ANISO) f2s[4] = add2(f2s[4], onsite_from<ANISO>(ok0, ok1, s4S, s4v, euS, euv, P.Ku, P.Kc));
@@ -108,8 +118,8 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
                 const bool ok = x < 0.0f;
                 if (ok) { S = Sn; nxv.v[k] = Sn.x; nyv.v[k] = Sn.y; nzv.v[k] = Sn.z; }
                 cnt += ok;
-                if (dbg_x)   dbg_x[q.site0 + 2u * k] = x;
-                if (dbg_acc) dbg_acc[q.site0 + 2u * k] = (uint8_t)ok;
+                if (dbg_x)   dbg_x[q.site0 + SS * k] = x;
+                if (dbg_acc) dbg_acc[q.site0 + SS * k] = (uint8_t)ok;
             }
             f[0] += S.x; f[1] += S.y; f[2] += S.z;
             if (colour == 1) f[3] -= dot3(S, hJ);
