@@ -125,7 +125,7 @@ class Lattice:
 
     def __init__(self, nx, ny, nz, periodic=(1, 1, 1), J=1.0, Ku=0.0, eu=(0, 0, 1), Kc=0.0, B=(0, 0, 0),
                  bond_mask=None, region=None, region_axis=None, cone0=0.5, adaptive=True, seed=42,
-                 device="cuda:0", stream=None, structure="sc"):
+                 device="cuda:0", stream=None, structure="sc", guard_bytes=0):
         import torch  # device memory and streams only
         self.L = load()
         self.shape = (int(nx), int(ny), int(nz))
@@ -137,7 +137,12 @@ class Lattice:
             raise McError(MC_EINVAL, "mc_workspace_bytes rejected the lattice / Hamiltonian")
         self.device = torch.device(device)
         with torch.cuda.device(self.device):
-            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            # guard_bytes > 0 (tests): the workspace sits between two canary zones that check_guards() verifies -- an
+            # out-of-bounds write of any kernel shows up there (compute-sanitizer is not available on every pool)
+            g = (int(guard_bytes) + 255) // 256 * 256
+            self._alloc = torch.full((nbytes + 2 * g,), 0xA5, dtype=torch.uint8, device=self.device)
+            self._guard = g
+            self.workspace = self._alloc[g: g + nbytes]
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             out = C.c_void_p()
             rc = self.L.mc_create(C.byref(lat), C.byref(ham), int(seed), self.workspace.data_ptr(), nbytes,
@@ -146,6 +151,13 @@ class Lattice:
             raise McError(rc, "mc_create failed (see stderr)")
         self.h = out
         self.workspace_bytes = nbytes
+
+    def check_guards(self):
+        """True if no byte of the canary zones around the workspace has been written (guard_bytes > 0)."""
+        import torch
+        torch.cuda.synchronize(self.device)
+        g, n = self._guard, self.workspace_bytes
+        return bool((self._alloc[:g] == 0xA5).all().item()) and bool((self._alloc[g + n:] == 0xA5).all().item())
 
     def _chk(self, rc):
         if rc != MC_OK:

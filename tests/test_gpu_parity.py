@@ -479,3 +479,38 @@ def test_negative_zero_sz_takes_the_sign_bit_frame_on_every_path(mods):
         for colour in (0, 1):
             _check_half_sweep(o, g, 1.0, colour, shape)
         g.close()
+
+
+def test_no_kernel_writes_outside_the_workspace(mods):
+    """Canary zones of 1 MiB on both sides of the caller's workspace stay intact through every kernel of the library, on
+    lattices whose sizes are not multiples of any tile (the last plane / row / item is where an index error would land):
+    colour passes (generic, staged, masked, bcc), pair passes, upload / readback, hooks, measurement, rotation, profile."""
+    oracle, binding, inputs = mods
+    G = 1 << 20
+    runs = [dict(shape=(16, 16, 16), ham=dict(Ku=0.01)), dict(shape=(2, 2, 2), ham=dict(Ku=0.1)), dict(shape=(6, 4, 4), ham=dict(Kc=0.2)),
+            dict(shape=(2, 1, 1), ham=dict(periodic=(0, 0, 0))), dict(shape=(8, 6, 5), ham=dict(periodic=(1, 0, 0), Ku=0.05)),
+            dict(shape=(64, 64, 64), ham=dict(Kc=0.01)), dict(shape=(96, 40, 36), ham=dict(Ku=0.1), path=2),
+            dict(shape=(80, 30, 58), ham=dict(periodic=(2, 1, 1), Ku=0.05), path=2),
+            dict(shape=(12, 5, 7), ham=dict(Ku=0.2, structure="bcc")), dict(shape=(4, 1, 1), ham=dict(structure="bcc"))]
+    for r in runs:
+        g = binding.Lattice(*r["shape"], cone0=0.8, adaptive=True, seed=3, guard_bytes=G, **r["ham"])
+        if "path" in r: g.debug_set_path(r["path"])
+        g.set_spins(inputs.random_unit_spins(g.N, seed=1)); g.sweep(1.0, 3)
+        g.half_sweep(1.0, 0, want_detail=True); g.half_sweep(1.0, 1); g.end_sweep()
+        g.init_spins(0); g.sweep(0.5, 2)
+        sc = r["ham"].get("structure", "sc") == "sc"
+        if sc and (g.N // 2) % 2 == 0:
+            try:
+                g.constrained_sweep(0.5, 0.4, 0.2, 3)
+            except binding.McError:
+                pass                                            # lattices the pairing does not cover
+        if sc: g.profile_x()
+        g.observables(); g.get_spins(); g.trace()
+        assert g.check_guards(), r
+        g.close()
+    shape = (64, 48, 4)                                         # the film: bond mask + grain table + open faces
+    mask, region, axes = inputs.voronoi_film(*shape, mean_diameter=12, seed=3)
+    g = binding.Lattice(*shape, periodic=(1, 1, 0), Ku=0.02, bond_mask=mask, region=region, region_axis=axes, guard_bytes=G)
+    g.sweep(0.5, 3); g.observables()
+    assert g.check_guards()
+    g.close()
