@@ -14,20 +14,18 @@ template <int RT, bool DEBUG, bool ANTI = false> TileFn pick_tile_rt(int aniso, 
         case 6: return tile_pass_kernel<3, false, RT, DEBUG, ANTI>;  default: return tile_pass_kernel<3, true, RT, DEBUG, ANTI>;
     }
 }
-// Row lengths with a specialised instantiation (every shared-memory offset an immediate): R = nx/2 of BASELINE's
-// periodic configs c2 (64^3), c4 (128^3) and c3 (224^3), plus 192^3.  Any other R runs the run-time-R instantiation.
-// The decision-variable debug outputs of the test hooks exist only in the run-time-R instantiation (same arithmetic).
+// Row lengths with a specialised instantiation: MC_TILE_RT_LIST (mc_tile.cuh).  Any other R, the anti-periodic wrap and the
+// decision-variable debug outputs of the test hooks run the run-time-R instantiation (same arithmetic, same slab shape).
 TileFn pick_tile(int R, int Ty, int npass, bool debug, int aniso, bool field, bool anti)
 {
     if (anti) return debug ? pick_tile_rt<0, true, true>(aniso, field) : pick_tile_rt<0, false, true>(aniso, field);
     if (debug) return pick_tile_rt<0, true>(aniso, field);
-    if (Ty != TILE_TY_RT || npass != TILE_NPASS_RT) return pick_tile_rt<0, false>(aniso, field);
+    if (!tile_has_rt(R) || Ty != tile_ty_rt(R) || npass != TILE_NPASS_RT) return pick_tile_rt<0, false>(aniso, field);
     switch (R) {
-        case 32:  return pick_tile_rt<32, false>(aniso, field);
-        case 96:  return pick_tile_rt<96, false>(aniso, field);
-        case 64:  return pick_tile_rt<64, false>(aniso, field);
-        case 112: return pick_tile_rt<112, false>(aniso, field);
-        default:  return pick_tile_rt<0, false>(aniso, field);
+#define MC_TILE_X(r) case r: return pick_tile_rt<r, false>(aniso, field);
+        MC_TILE_RT_LIST(MC_TILE_X)
+#undef MC_TILE_X
+        default: return pick_tile_rt<0, false>(aniso, field);
     }
 }
 
@@ -54,10 +52,9 @@ bool plan_tile(mc_ctx* c)
     const size_t smem_cap = (size_t)(220 * 1024) / TILE_MIN_BLOCKS - 3 * 1024;   // TILE_MIN_BLOCKS CTAs per SM
     auto slot_bytes = [&](int ty) { return (size_t)3 * (ty + 2) * R * sizeof(float); };
     if (lat.ny % (2 * RP) == 0 && TILE_NSLOT * slot_bytes(2 * RP) <= smem_cap) NP = 2;
-    // row lengths with a compile-time specialisation (R = 32, 64, 96, 112) take its slab shape when it fits
-    if ((R == 32 || R == 64 || R == 96 || R == 112) && lat.ny % TILE_TY_RT == 0 && PR * (TILE_TY_RT / TILE_NPASS_RT) <= max_threads) {
-        RP = TILE_TY_RT / TILE_NPASS_RT; NP = TILE_NPASS_RT;
-    }
+    // row lengths with a compile-time specialisation take its slab shape when it tiles ny
+    const bool spec = tile_has_rt(R) && tile_rp_rt(R) >= 1 && lat.ny % tile_ty_rt(R) == 0;
+    if (spec) { RP = tile_rp_rt(R); NP = TILE_NPASS_RT; }
     G.RP = RP; G.NPASS = NP; G.Ty = RP * NP;
     G.n_slabs = lat.ny / G.Ty;
     G.slot_floats = 3 * (G.Ty + 2) * R;
@@ -80,7 +77,7 @@ bool plan_tile(mc_ctx* c)
     G.n_segs = n_segs; G.Lz = lat.nz / n_segs; G.Lz_rem = lat.nz % n_segs;
     if ((long long)G.n_slabs * G.n_segs > c->P.max_blocks) return false;
     c->tile_possible = true;
-    const bool specialised = (R == 32 || R == 64 || R == 96 || R == 112) && G.Ty == TILE_TY_RT && G.NPASS == TILE_NPASS_RT && !c->P.anti_x;
+    const bool specialised = spec && !c->P.anti_x;
     c->tile_ok = specialised && c->P.Nc >= 65536u;             // small lattices are launch-bound: the generic kernel has less prologue
     return c->tile_ok;
 }

@@ -33,8 +33,22 @@ constexpr int TILE_NSLOT = 4;
 #endif
 constexpr int TILE_MAX_THREADS = MC_TILE_MAX_THREADS;   // launch bounds of the tiled pass: threads per CTA ...
 constexpr int TILE_MIN_BLOCKS = MC_TILE_MIN_BLOCKS;     // ... and CTAs per SM the register allocation must allow
-constexpr int TILE_TY_RT = MC_TILE_TY_RT;               // slab height of the compile-time-R specialisations
-constexpr int TILE_NPASS_RT = 2;                        // ... which a thread covers in this many passes (unrolled)
+constexpr int TILE_NPASS_RT = 2;                        // passes (row groups) a thread of a compile-time-R specialisation covers per plane (unrolled)
+// Slab shape of the specialisation for R colour-sites per row: RP rows per pass = as many as TILE_MAX_THREADS threads cover
+// (one thread = one x-adjacent pair), at most MC_TILE_TY_RT / 2; slab height Ty = 2 RP.  R <= 112: 8 x 2 = 16 rows.
+__host__ __device__ constexpr int tile_rp_rt(int R) { return R <= 0 ? 0 : ((TILE_MAX_THREADS / (R / 2)) < (MC_TILE_TY_RT / 2) ? (TILE_MAX_THREADS / (R / 2)) : (MC_TILE_TY_RT / 2)); }
+__host__ __device__ constexpr int tile_ty_rt(int R) { return TILE_NPASS_RT * tile_rp_rt(R); }
+// Row lengths R = nx / 2 with a specialised instantiation (every shared-memory offset an immediate, both passes unrolled).
+#ifndef MC_TILE_RT_LIST
+#define MC_TILE_RT_LIST(X) X(32) X(96) X(112)
+#endif
+inline bool tile_has_rt(int R)
+{
+#define MC_TILE_X(r) if (R == r) return true;
+    MC_TILE_RT_LIST(MC_TILE_X)
+#undef MC_TILE_X
+    return false;
+}
 
 struct TileGeom {
     int R, PR;                 // colour-sites per row, pairs per row
@@ -135,8 +149,8 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
     const int y0 = slab * G.Ty;
     const int Lz = G.Lz + (seg < G.Lz_rem ? 1 : 0);
     const int z0 = seg * G.Lz + (seg < G.Lz_rem ? seg : G.Lz_rem);
-    const int nrows = (RT ? TILE_TY_RT : G.Ty) + 2;                 // the specialisations fix the slab height ...
-    const int NPASS = RT ? TILE_NPASS_RT : G.NPASS, RP = RT ? TILE_TY_RT / TILE_NPASS_RT : G.RP;   // ... and its split into passes
+    const int nrows = (RT ? tile_ty_rt(RT) : G.Ty) + 2;             // the specialisations fix the slab height ...
+    const int NPASS = RT ? TILE_NPASS_RT : G.NPASS, RP = RT ? tile_rp_rt(RT) : G.RP;   // ... and its split into passes
     const int CS = nrows * R;
     const int slot_floats = 3 * CS;
 
