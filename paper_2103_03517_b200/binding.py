@@ -140,7 +140,9 @@ class Lattice:
             # guard_bytes > 0 (tests): the workspace sits between two canary zones that check_guards() verifies -- an
             # out-of-bounds write of any kernel shows up there (compute-sanitizer is not available on every pool)
             g = (int(guard_bytes) + 255) // 256 * 256
-            self._alloc = torch.full((nbytes + 2 * g,), 0xA5, dtype=torch.uint8, device=self.device)
+            self._alloc = torch.empty(nbytes + 2 * g, dtype=torch.uint8, device=self.device)
+            if g:
+                self._alloc[:g] = 0xA5; self._alloc[g + nbytes:] = 0xA5
             self._guard = g
             self.workspace = self._alloc[g: g + nbytes]
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
