@@ -162,6 +162,7 @@ int mc_profile_x(mc_ctx* ctx, double* host_profile);
 #define MC_PATH_AUTO     0
 #define MC_PATH_GENERIC  1
 #define MC_PATH_STAGED   2
+#define MC_PATH_MARCH    3
 int mc_debug_set_path(mc_ctx* ctx, int path);
 
 /* Number of kernel launches this handle has enqueued since creation (bench.py's gpu_launches). */

@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libmc_b200.so")
 
 MC_OK, MC_EINVAL, MC_ECUDA, MC_ESTATE = 0, -1, -2, -3
 MC_TRACE_CAPACITY = 16384
-MC_PATH_AUTO, MC_PATH_GENERIC, MC_PATH_STAGED = 0, 1, 2
+MC_PATH_AUTO, MC_PATH_GENERIC, MC_PATH_STAGED, MC_PATH_MARCH = 0, 1, 2, 3
 MC_SC, MC_BCC = 0, 1
 
 # every symbol include/mc.h declares (tests/test_abi.py checks the header against this list and the .so)

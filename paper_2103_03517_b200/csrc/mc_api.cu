@@ -88,6 +88,8 @@ FastDiv make_div(uint32_t d)
 
 }  // namespace
 
+namespace mc { FastDiv host_make_div(uint32_t d) { return make_div(d); } }
+
 namespace {
 
 #define CU(call) MC_CU(call)
@@ -103,6 +105,7 @@ struct DeviceGuard {
 int launch_pass(mc_ctx* ctx, int mode, int colour, float invT, int flags, float* dx, uint8_t* da)
 {
     if (mode == MODE_SWEEP && ctx->tile_ok) return launch_pass_tile(ctx, colour, invT, flags, dx, da);
+    if (mode == MODE_SWEEP && ctx->march_ok) return launch_pass_march(ctx, colour, invT, flags, dx, da);
     return launch_pass_generic(ctx, mode, colour, invT, flags, dx, da);
 }
 
@@ -204,6 +207,7 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     P.nx = nx; P.ny = ny; P.nz = nz; P.R = (int)R; P.Nc = Nc; P.N = N; P.invN = 1.0 / (double)N;
     P.anti_x = lat->periodic[0] == 2 ? 1 : 0;
     P.bcc = bcc ? 1 : 0;
+    P.per_mask = (lat->periodic[0] ? 1 : 0) | (lat->periodic[1] ? 2 : 0) | (lat->periodic[2] ? 4 : 0);
     P.plane = L.plane; P.S = (float*)(ws + L.spins);
     P.mask = nullptr; P.mask_plane = L.mask_plane; P.region = nullptr; P.region_plane = L.region_plane; P.axis = nullptr;
     P.J = (float)ham->J; P.Ku = (float)ham->Ku; P.Kc = (float)ham->Kc;
@@ -302,6 +306,7 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     }
 
     plan_tile(ctx);
+    plan_march(ctx);
 
     // ---- device state
     DevState st; memset(&st, 0, sizeof st);
@@ -328,11 +333,14 @@ int64_t mc_launch_count(const mc_ctx* ctx) { return ctx ? ctx->launches : 0; }
 int mc_debug_set_path(mc_ctx* ctx, int path)
 {
     CHECK_CTX();
-    if (path == MC_PATH_AUTO) { const bool keep = ctx->tile_possible; plan_tile(ctx); ctx->tile_possible = keep || ctx->tile_possible; }
-    else if (path == MC_PATH_GENERIC) ctx->tile_ok = false;
+    if (path == MC_PATH_AUTO) { const bool keep = ctx->tile_possible; plan_tile(ctx); ctx->tile_possible = keep || ctx->tile_possible; plan_march(ctx); }
+    else if (path == MC_PATH_GENERIC) { ctx->tile_ok = false; ctx->march_ok = false; }
     else if (path == MC_PATH_STAGED) {
         if (!ctx->tile_possible) return fail(ctx, MC_EINVAL, "mc_debug_set_path: the staged pass does not cover this lattice / Hamiltonian");
-        ctx->tile_ok = true;
+        ctx->tile_ok = true; ctx->march_ok = false;
+    } else if (path == MC_PATH_MARCH) {
+        if (!ctx->march_possible) return fail(ctx, MC_EINVAL, "mc_debug_set_path: the z-march pass does not cover this lattice / Hamiltonian");
+        ctx->march_ok = true; ctx->tile_ok = false;
     } else return fail(ctx, MC_EINVAL, "mc_debug_set_path: unknown path");
     ctx->path = path;
     return MC_OK;

@@ -45,6 +45,7 @@ struct DevState {
 struct Params {
     int nx, ny, nz, R;               // R = nx/2 sites of one colour per row
     int anti_x;                      // 1: anti-periodic boundary along x (domain-wall box); the wrap bond sees -S_j
+    int per_mask;                    // bit a set: axis a (x, y, z) is periodic (or anti-periodic)
     int bcc;                         // 1: body-centred cubic (C-30): colour = sublattice, R = nx cells per row, 8 neighbours
     uint32_t Nc;                     // sites per colour
     uint32_t N;
@@ -84,7 +85,17 @@ template <> __device__ __forceinline__ Pack<4> ld_nc<4>(const float* p)
     const float4 t = __ldg(reinterpret_cast<const float4*>(p));
     Pack<4> r; r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w; return r;
 }
+template <> __device__ __forceinline__ Pack<2> ld_nc<2>(const float* p)
+{
+    const float2 t = __ldg(reinterpret_cast<const float2*>(p));
+    Pack<2> r; r.v[0] = t.x; r.v[1] = t.y; return r;
+}
 template <int VEC> __device__ __forceinline__ Pack<VEC> ld_rw(const float* p);
+template <> __device__ __forceinline__ Pack<2> ld_rw<2>(const float* p)
+{
+    const float2 t = *reinterpret_cast<const float2*>(p);
+    Pack<2> r; r.v[0] = t.x; r.v[1] = t.y; return r;
+}
 template <> __device__ __forceinline__ Pack<1> ld_rw<1>(const float* p) { Pack<1> r; r.v[0] = *p; return r; }
 template <> __device__ __forceinline__ Pack<4> ld_rw<4>(const float* p)
 {
@@ -92,6 +103,7 @@ template <> __device__ __forceinline__ Pack<4> ld_rw<4>(const float* p)
     Pack<4> r; r.v[0] = t.x; r.v[1] = t.y; r.v[2] = t.z; r.v[3] = t.w; return r;
 }
 template <int VEC> __device__ __forceinline__ void st_rw(float* p, const Pack<VEC>& r);
+template <> __device__ __forceinline__ void st_rw<2>(float* p, const Pack<2>& r) { *reinterpret_cast<float2*>(p) = make_float2(r.v[0], r.v[1]); }
 template <> __device__ __forceinline__ void st_rw<1>(float* p, const Pack<1>& r) { *p = r.v[0]; }
 template <> __device__ __forceinline__ void st_rw<4>(float* p, const Pack<4>& r)
 {

@@ -6,6 +6,7 @@
 #include "mc_common.cuh"
 #include "mc_pair.cuh"      // PairGeom
 #include "mc_tile.cuh"      // TileGeom
+#include "mc_march.cuh"     // MarchGeom
 
 #include <cstdio>
 
@@ -20,6 +21,7 @@ struct mc_ctx {
     mc::PairGeom pgeom;
     bool pair_ok;
     bool tile_possible, tile_ok; mc::TileGeom tgeom; int tile_threads; size_t tile_smem;   // staged colour pass (mc_tile.cuh)
+    bool march_possible, march_ok; mc::MarchGeom mgeom;     // register-carried z-march colour pass (mc_march.cuh)
     int path;                         // MC_PATH_AUTO / GENERIC / STAGED (mc_debug_set_path)
     bool field;
     int vec, aniso;
@@ -75,6 +77,11 @@ inline int grid_for(const mc_ctx* c, uint32_t n_threads_needed, int resident_per
 int launch_pass_generic(mc_ctx* ctx, int mode, int colour, float invT, int flags, float* dx, uint8_t* da);
 // ---- mc_pair.cu: constrained pair pass
 int launch_pair_generic(mc_ctx* ctx, int colour, float invT, int flags, float* dx, uint8_t* da);
+// ---- mc_march.cu: register-carried z-march colour pass; plan_march fills ctx->march_* at creation
+bool plan_march(mc_ctx* ctx);
+int launch_pass_march(mc_ctx* ctx, int colour, float invT, int flags, float* dx, uint8_t* da);
+// magic-number division for the kernels' FastDiv (mc_api.cu)
+FastDiv host_make_div(uint32_t d);
 // ---- mc_tile.cu: staged colour pass (TMA-fed shared-memory plane ring); plan_tile fills ctx->tile_* at creation
 bool plan_tile(mc_ctx* ctx);
 int launch_pass_tile(mc_ctx* ctx, int colour, float invT, int flags, float* dx, uint8_t* da);

@@ -103,6 +103,39 @@ def test_half_sweep_parity_forced_generic_pass(mods, shape, T, cone, ham):
     test_half_sweep_parity_random_state(mods, shape, T, cone, ham, path=1)      # MC_PATH_GENERIC
 
 
+# the register-carried march (MC_PATH_MARCH = 3): bulk z-march, ragged segments, masked / open faces, and the thin-film y-march
+MARCH_CASES = [
+    ((40, 12, 18), 1.44, 2.0, dict(Kc=0.01)),                                                # z-march, 4 segments + remainder
+    ((24, 10, 16), 0.7, 1.2, dict(Kc=0.3, Ku=0.1, eu=(0.5, 0.5, 0.7), B=(0.1, -0.05, 0.2))),  # every term
+    ((64, 64, 64), 0.1, 0.3, dict(Ku=0.01)),                                                 # low T
+    ((16, 6, 17), 0.9, 1.0, dict(periodic=(1, 0, 0), Ku=0.05, Kc=0.1)),                      # masked: open y and z faces, odd nz
+    ((512, 24, 4), 0.8, 0.9, dict(periodic=(1, 1, 0), Ku=0.1)),                              # thin film: y-march (a block = 64 items x 4 planes), open z
+    ((256, 9, 8), 1.0, 1.2, dict(periodic=(0, 0, 1), Kc=0.2)),                               # y-march with open x and y, periodic z, odd ny
+]
+
+
+@pytest.mark.parametrize("shape,T,cone,ham", MARCH_CASES)
+def test_half_sweep_parity_forced_march_pass(mods, shape, T, cone, ham):
+    test_half_sweep_parity_random_state(mods, shape, T, cone, ham, path=3)      # MC_PATH_MARCH
+
+
+def test_march_pass_is_bit_identical_to_the_generic_pass(mods):
+    """Same packed arithmetic in the same order: after sweeps on both paths the spins are equal bit for bit (the fused sums are
+    not: their fp32 partial sums group the sites differently before the exact fixed-point reduction)."""
+    oracle, binding, inputs = mods
+    cases = [((64, 48, 40), dict(Kc=0.05, Ku=0.02)), ((32, 16, 24), dict(periodic=(1, 0, 1), Ku=0.1)), ((512, 16, 4), dict(periodic=(1, 1, 0), Ku=0.1))]
+    mask, region, axes = inputs.voronoi_film(512, 16, 4, mean_diameter=12, seed=3)
+    cases.append(((512, 16, 4), dict(periodic=(1, 1, 0), Ku=0.02, bond_mask=mask, region=region, region_axis=axes)))
+    for shape, ham in cases:
+        out = []
+        for path in (1, 3):
+            g = binding.Lattice(*shape, cone0=0.8, adaptive=True, seed=11, **ham)
+            g.debug_set_path(path)
+            g.set_spins(inputs.random_unit_spins(g.N, seed=2)); g.sweep(0.9, 7)
+            out.append((g.get_spins(), g.trace()[:, :2])); g.close()
+        assert (out[0][0] == out[1][0]).all() and (out[0][1] == out[1][1]).all(), shape      # spins; acceptance and cone per sweep
+
+
 @pytest.mark.parametrize("shape,T,cone,ham", CASES)
 def test_half_sweep_parity_random_state(mods, shape, T, cone, ham, path=None):
     oracle, binding, inputs = mods
