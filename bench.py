@@ -192,6 +192,37 @@ def time_other_paths(binding, torch, local_rank, sweeps=100):
     return out
 
 
+def scan_sizes(args):
+    """--scan-sizes L1,L2,...: unconstrained sweeps (c3 Hamiltonian, random start) on L^3 lattices with the planner's kernel and
+    with the generic gather; one JSON line per size (the table of BASELINE.md section 4)."""
+    import torch
+    from paper_2103_03517_b200 import binding, build, inputs
+    build.build()
+    peak, _ = measured_peaks()
+    names = {1: "generic", 2: "staged", 3: "march"}
+    for L in [int(v) for v in args.scan_sizes.split(",")]:
+        N = L ** 3
+        row = {"L": L, "spins": N}
+        spins = inputs.random_unit_spins(N, seed=42)
+        for label, path in (("auto", None), ("generic", binding.MC_PATH_GENERIC)):
+            g = binding.Lattice(L, L, L, seed=42, cone0=0.5, adaptive=True, **HAM)
+            if path is not None: g.debug_set_path(path)
+            g.set_spins(spins); g.sweep(1.2, 30); torch.cuda.synchronize()
+            n = max(20, min(200, int(2e9 / N)))
+            best = None
+            for rep in range(3):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(); g.sweep(1.2, n); e1.record(); torch.cuda.synchronize()
+                us = e0.elapsed_time(e1) * 1e3 / n
+                best = us if best is None else min(best, us)
+            ups = N / (best * 1e-6)
+            row[label] = {"kernel": names[g.debug_get_path()], "us_per_sweep": round(best, 2), "updates_per_s": ups,
+                          "frac_of_measured_peak": BYTES_PER_UPDATE * ups / 1e9 / peak}
+            g.close()
+        print(json.dumps(row), flush=True)
+    return 0
+
+
 def run_ours(args, rank, local_rank, world):
     import torch
     if not torch.cuda.is_available():
@@ -301,6 +332,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=6)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-paths", action="store_true")
+    ap.add_argument("--scan-sizes", default="", help="comma-separated L: time L^3 lattices with the planner's kernel and the generic pass, then exit")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3                                   # timing rule: W >= 3
@@ -312,6 +344,8 @@ def main():
         cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
                "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
         return subprocess.call(cmd)
+    if args.scan_sizes:
+        return scan_sizes(args)
     if args.impl == "reference":
         return run_reference(args, rank, world)
     return run_ours(args, rank, local_rank, world)

@@ -164,6 +164,8 @@ int mc_profile_x(mc_ctx* ctx, double* host_profile);
 #define MC_PATH_STAGED   2
 #define MC_PATH_MARCH    3
 int mc_debug_set_path(mc_ctx* ctx, int path);
+/* The kernel the colour pass of mc_sweep currently launches: MC_PATH_GENERIC, MC_PATH_STAGED or MC_PATH_MARCH (never AUTO). */
+int mc_debug_get_path(const mc_ctx* ctx);
 
 /* Number of kernel launches this handle has enqueued since creation (bench.py's gpu_launches). */
 int64_t mc_launch_count(const mc_ctx* ctx);

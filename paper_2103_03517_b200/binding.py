@@ -23,7 +23,7 @@ MC_SC, MC_BCC = 0, 1
 SYMBOLS = [
     "mc_workspace_bytes", "mc_create", "mc_destroy", "mc_init_spins", "mc_set_spins", "mc_get_spins", "mc_set_cone",
     "mc_set_sweep", "mc_sweep", "mc_constrained_sweep", "mc_half_sweep", "mc_constrained_half_sweep", "mc_end_sweep",
-    "mc_align_to", "mc_observables", "mc_reset_accumulators", "mc_trace", "mc_profile_x", "mc_debug_set_path", "mc_launch_count", "mc_last_error", "mc_version",
+    "mc_align_to", "mc_observables", "mc_reset_accumulators", "mc_trace", "mc_profile_x", "mc_debug_set_path", "mc_debug_get_path", "mc_launch_count", "mc_last_error", "mc_version",
 ]
 
 
@@ -88,6 +88,7 @@ def load():
     L.mc_trace.argtypes = [vp, i64, vp, vp]; L.mc_trace.restype = i32
     L.mc_profile_x.argtypes = [vp, vp]; L.mc_profile_x.restype = i32
     L.mc_debug_set_path.argtypes = [vp, i32]; L.mc_debug_set_path.restype = i32
+    L.mc_debug_get_path.argtypes = [vp]; L.mc_debug_get_path.restype = i32
     L.mc_launch_count.argtypes = [vp]; L.mc_launch_count.restype = i64
     L.mc_last_error.argtypes = [vp]; L.mc_last_error.restype = C.c_char_p
     L.mc_version.argtypes = []; L.mc_version.restype = C.c_char_p
@@ -230,4 +231,5 @@ class Lattice:
         return rows[: k.value].copy()
 
     def debug_set_path(self, path): self._chk(self.L.mc_debug_set_path(self.h, int(path)))
+    def debug_get_path(self): return int(self.L.mc_debug_get_path(self.h))
     def launch_count(self): return int(self.L.mc_launch_count(self.h))

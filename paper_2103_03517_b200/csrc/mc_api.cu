@@ -346,6 +346,12 @@ int mc_debug_set_path(mc_ctx* ctx, int path)
     return MC_OK;
 }
 
+int mc_debug_get_path(const mc_ctx* ctx)
+{
+    if (!ctx) return MC_EINVAL;
+    return ctx->tile_ok ? MC_PATH_STAGED : (ctx->march_ok ? MC_PATH_MARCH : MC_PATH_GENERIC);
+}
+
 int mc_init_spins(mc_ctx* ctx, int mode, const double dir[3])
 {
     CHECK_CTX();

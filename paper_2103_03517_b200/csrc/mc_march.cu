@@ -49,10 +49,17 @@ bool plan_march(mc_ctx* c)
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void*)pick_march(c->aniso, c->masked, G.axis, false), MARCH_BLOCK, 0) != cudaSuccess || per_sm < 1) { cudaGetLastError(); return false; }
     const long long resident = (long long)c->sm_count * per_sm * MARCH_BLOCK;
     const long long columns = (long long)ns * G.RV;
-    long long n_segs = resident / columns;
-    if (n_segs > nm / 4) n_segs = nm / 4;               // a thread amortises its two prologue steps over >= 4 steps
-    if (n_segs < (nm + 63) / 64) n_segs = (nm + 63) / 64;   // ... and sums at most 256 sites in fp32 before the fixed-point conversion
-    if (n_segs < 1) n_segs = 1;
+    // segments along the march axis: the count that minimises (waves of resident threads) x (steps per thread + the prologue,
+    // two loads-only steps counted as half a step); at most 256 steps per thread (1024 sites in its fp32 partial sums), at
+    // least 4 (the prologue has to be amortised)
+    long long n_lo = (nm + 255) / 256, n_hi = nm / 4 > 0 ? nm / 4 : 1, n_segs = n_lo;
+    double best = 1e300;
+    for (long long n = n_lo; n <= n_hi; ++n) {
+        const double waves = (double)((columns * n + resident - 1) / resident);
+        const double cost = waves * ((double)((nm + n - 1) / n) + 0.5);
+        if (cost < best) { best = cost; n_segs = n; }
+    }
+    const double efficiency = (double)nm * (double)columns / (double)resident / best;   // 1 = every slot busy for the whole pass
     G.n_segs = (int)n_segs; G.Lm = nm / G.n_segs; G.Lm_rem = nm % G.n_segs;
     const long long nt = columns * n_segs;
     if (nt > 0x7fffffffLL || (nt + MARCH_BLOCK - 1) / MARCH_BLOCK > 0x7fffffffLL) return false;
@@ -62,7 +69,8 @@ bool plan_march(mc_ctx* c)
     c->march_possible = true;
     // default for bulk lattices without side data (measured: +4..9 % over the gather at 128^3 .. 512^3); the staged pass keeps
     // the row lengths it is specialised for; masked lattices stay on the gather (the c5 film: 185 against 163 us per sweep)
-    c->march_ok = G.Lm >= 4 && c->P.Nc >= 65536u && !c->tile_ok && !c->masked;
+    // ... and lattices whose columns fill the machine badly (small ones; sizes that leave a sixth of the slots empty: 320^3)
+    c->march_ok = G.Lm >= 4 && efficiency >= 0.85 && !c->tile_ok && !c->masked;
     return c->march_ok;
 }
 
