@@ -1,9 +1,7 @@
-"""B200-native red-black checkerboard Metropolis for classical Heisenberg spins (arXiv 2103.03517).
+"""B200-native checkerboard Metropolis for classical Heisenberg spins (arXiv 2103.03517): the hot path behind a C ABI.
 
-The product is the C-ABI shared library ``libmc_b200.so`` (hand-written CUDA for sm_100a, declared in
-``include/mc.h``); :mod:`paper_2103_03517_b200.binding` is a thin ctypes layer over it with the same
-names.  Importing this package does not load the CUDA library; the first use of the binding does, and
-fails loudly if it is missing -- there is no CPU fallback.
+`binding` -- ctypes layer over libmc_b200.so (include/mc.h); `build` -- nvcc build of the library; `inputs` -- seeded
+synthetic inputs (no method arithmetic); `replicas` -- independent points over several GPUs; `configs` -- the BASELINE.json
+workloads; `analysis` -- host-side fits.  There is no CPU fallback and nothing here imports the oracle.
 """
-
-__all__ = ["binding", "inputs", "build", "harness"]
+__all__ = ["analysis", "binding", "build", "configs", "inputs", "replicas"]
