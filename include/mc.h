@@ -105,7 +105,9 @@ int mc_destroy(mc_ctx* ctx);     /* frees the host handle only; the workspace st
  * Philox(ctr = (i, 3, 0, 0), key = seed): z = 2 u0 - 1, phi = 2 pi u1; BASELINE.json configs[2]).  Asynchronous. */
 int mc_init_spins(mc_ctx* ctx, int mode, const double dir[3]);
 /* Upload / download the spin state as [N][3] fp32 in lexicographic site order (x fastest).  mc_set_spins
- * normalises every spin.  Both synchronise the stream. */
+ * normalises every spin whose squared length differs from 1 by more than 4e-7; a spin that is unit to fp32 rounding (anything
+ * mc_get_spins returned) is stored unchanged, so get -> set restores the state bit for bit: with mc_set_sweep and mc_set_cone
+ * that is a checkpoint (the RNG is counter-based: there is no other state).  Both synchronise the stream. */
 int mc_set_spins(mc_ctx* ctx, const float* host_xyz);
 int mc_get_spins(mc_ctx* ctx, float* host_xyz);
 /* Set the cone half-angle / the sweep counter (checkpoint restore, parity tests).  Asynchronous. */
@@ -137,7 +139,8 @@ int mc_constrained_half_sweep(mc_ctx* ctx, double T, double theta, double phi, i
 /* Closes a sweep assembled from half-sweep hooks: controller step with the accepted count of the two passes,
  * sweep counter += 1 (what mc_sweep does after its black pass).  Asynchronous. */
 int mc_end_sweep(mc_ctx* ctx);
-/* Rigid rotation of all spins taking M/|M| onto e_C (C-12), exposed for parity tests.  Synchronous. */
+/* Rigid rotation of all spins taking M/|M| onto e_C (C-12), exposed for parity tests.  No rotation is applied when M already
+ * lies within 3e-7 rad of e_C (the accuracy of the fp32 state): a restored constrained run continues bit for bit.  Synchronous. */
 int mc_align_to(mc_ctx* ctx, double theta, double phi);
 
 /* Synchronises the stream and returns the observables of the current state plus the accumulators.

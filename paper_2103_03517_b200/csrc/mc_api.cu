@@ -464,7 +464,10 @@ int mc_align_to(mc_ctx* ctx, double theta, double phi)
     const double c = u[0] * e[0] + u[1] * e[1] + u[2] * e[2];
     double Rm[9] = { 1, 0, 0, 0, 1, 0, 0, 0, 1 };
     bool identity = false;
-    if (s < 1e-300) {
+    // M already along e_C to the accuracy of the fp32 state (e.g. a restored checkpoint of a constrained run): no rotation,
+    // so that the restored run continues bit for bit
+    if (s < 3e-7 && c > 0) identity = true;
+    else if (s < 1e-300) {
         if (c > 0) identity = true;
         else {
             double t[3] = { 1, 0, 0 }; if (fabs(u[0]) > 0.9) { t[0] = 0; t[1] = 1; }

@@ -56,8 +56,11 @@ __global__ void lex_to_split_kernel(const __grid_constant__ Params P, const floa
     uint32_t c = (x + y + z) & 1u, a = row * (uint32_t)P.R + (x >> 1);
     if (P.bcc) { c = s >= P.Nc ? 1u : 0u; a = s - c * P.Nc; }      // bcc: site = sublattice * Ncell + cell
     float vx = lex[3ull * s], vy = lex[3ull * s + 1], vz = lex[3ull * s + 2];
+    // a spin that is already unit to fp32 rounding (what mc_get_spins returns) is stored as it is: upload(download(state)) is
+    // the identity, so a checkpoint restores bit for bit; anything else is normalised
     const float n2 = vx * vx + vy * vy + vz * vz;
-    const float inv = (n2 > 0.0f) ? (float)(1.0 / sqrt((double)n2)) : 0.0f;
+    const bool unit = fabsf(n2 - 1.0f) <= 4.0e-7f;
+    const float inv = unit ? 1.0f : ((n2 > 0.0f) ? (float)(1.0 / sqrt((double)n2)) : 0.0f);
     float* Sc = P.S + (long long)c * 3 * P.plane;
     Sc[a] = vx * inv; Sc[P.plane + a] = vy * inv; Sc[2 * P.plane + a] = (n2 > 0.0f) ? vz * inv : 1.0f;
 }

@@ -547,3 +547,25 @@ def test_no_kernel_writes_outside_the_workspace(mods):
     g.sweep(0.5, 3); g.observables()
     assert g.check_guards()
     g.close()
+
+
+def test_checkpoint_restore_in_the_middle_of_a_run(mods):
+    """a run interrupted after 7 of 15 sweeps and restored into a fresh handle from (spins, sweep counter, cone)
+    continues bit for bit -- the RNG is counter-based, the upload of a downloaded state is the identity.  Unconstrained
+    (staged, march and generic lattices) and constrained."""
+    oracle, binding, inputs = mods
+    for shape, ham, constrained in (((64, 64, 64), dict(Kc=0.01), False), ((64, 48, 40), dict(Ku=0.05), False),
+                                    ((24, 10, 6), dict(Ku=0.1, B=(0.0, 0.1, 0.0)), False), ((32, 16, 16), dict(Ku=0.05), True)):
+        step = (lambda g, n: g.constrained_sweep(0.8, 0.5, 0.2, n)) if constrained else (lambda g, n: g.sweep(1.1, n))
+        a = binding.Lattice(*shape, cone0=0.7, adaptive=True, seed=9, **ham)
+        if not constrained: a.set_spins(inputs.random_unit_spins(a.N, seed=4))
+        step(a, 7)
+        snap, ob = a.get_spins(), a.observables()
+        step(a, 8)
+        b = binding.Lattice(*shape, cone0=0.7, adaptive=True, seed=9, **ham)
+        b.set_spins(snap); b.set_sweep(ob.sweep); b.set_cone(ob.cone_rad)
+        assert (b.get_spins() == snap).all()                                # the upload changed nothing
+        step(b, 8)                                                          # constrained: M already lies along e_C, the library does not rotate
+        assert (a.get_spins() == b.get_spins()).all(), shape
+        assert (a.trace()[-8:] == b.trace()).all()
+        a.close(); b.close()
