@@ -209,4 +209,133 @@ march_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Marc
     }
 }
 
+// --------------------------------------------------------------------------------------------------------------
+// bcc (C-30): the same march for the two-sublattice lattice.  A thread owns 4 consecutive cells of a row of its
+// sublattice and marches along k.  Its 8 neighbours per cell are the cells i and i -+ 1 of the rows j, j -+ 1 of the
+// planes k and k -+ 1 of the other sublattice (- for sublattice A, + for B): two of the four rows were the in-plane rows
+// of the previous step (A: plane k - 1 is the last step's plane k; B: plane k is the last step's plane k + 1), so
+// they are carried in registers and a step loads two rows (float4 + the one cell outside the item, per component)
+// instead of four.  Summation order of bcc_exchange_field (rows (k,j), (k,j'), (k',j), (k',j')): bit-identical spins.
+// --------------------------------------------------------------------------------------------------------------
+struct BccRow { Pack<4> o; float ex; };
+
+template <int ANISO, int COLOUR, bool DEBUG>
+__global__ void __launch_bounds__(MARCH_BLOCK, MC_MARCH_MIN_BLOCKS)
+march_bcc_kernel(const __grid_constant__ Params P, const __grid_constant__ MarchGeom G, int, float invT, int flags,
+                 float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
+{
+    constexpr int colour = COLOUR;           // the sublattice decides which rows are carried: compile-time, so that they stay registers
+    DevState* st = P.st;
+    grid_dependency_sync();
+    const unsigned long long sweep = st->sweep;
+    const float omc = st->one_minus_cos;
+    const PhiloxKey& key = P.key;
+    const uint32_t c1 = TAG_MOVE | ((uint32_t)colour << 8), c2 = (uint32_t)sweep, c3 = (uint32_t)(sweep >> 32);
+
+    f2 aM[3] = { splat(0.f), splat(0.f), splat(0.f) }, aEx = splat(0.f), aAn = splat(0.f), aZe = splat(0.f);
+    int cnt = 0;
+    const uint32_t t = blockIdx.x * MARCH_BLOCK + threadIdx.x;
+    if (t < G.n_threads) {
+        const int nx = P.nx, ny = P.ny, nz = P.nz;
+        uint32_t rowq, xq, seg, y;
+        G.div_rv.divmod(t, rowq, xq); G.div_ns.divmod(rowq, seg, y);
+        const int Lm = G.Lm + ((int)seg < G.Lm_rem ? 1 : 0);
+        const int k0 = (int)seg * G.Lm + ((int)seg < G.Lm_rem ? (int)seg : G.Lm_rem);
+        const int i0 = 4 * (int)xq;
+        const long long ms = (long long)ny * nx;                           // cells per plane
+        const int y2 = colour ? ((int)y + 1 == ny ? 0 : (int)y + 1) : (y == 0 ? ny - 1 : (int)y - 1);
+        const long long a0 = ((long long)k0 * ny + y) * nx + i0;
+        const float* O = P.S + (long long)(1 - colour) * 3 * P.plane;
+        float* pS = P.S + (long long)colour * 3 * P.plane + a0;
+        const float* pR0 = O + a0;                                          // other sublattice, plane k: row j and row j'
+        const float* pR1 = O + ((long long)k0 * ny + y2) * nx + i0;
+        const int exoff = colour ? (i0 + 4 == nx ? -i0 : 4) : (i0 == 0 ? nx - 1 : -1);   // the cell outside the item: i0 + 4 (B) or i0 - 1 (A)
+        uint32_t site0 = (uint32_t)colour * P.Nc + (uint32_t)a0;
+        const Vec3 B = { P.B[0], P.B[1], P.B[2] };
+        const V3p B2 = splat3(B);
+        const V3p e2 = splat3(Vec3{ P.eu[0], P.eu[1], P.eu[2] });
+        auto load_rows = [&](long long d, BccRow (&r0)[3], BccRow (&r1)[3]) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                r0[c].o = ld_nc<4>(pR0 + c * P.plane + d); r0[c].ex = __ldg(pR0 + c * P.plane + d + exoff);
+                r1[c].o = ld_nc<4>(pR1 + c * P.plane + d); r1[c].ex = __ldg(pR1 + c * P.plane + d + exoff);
+            }
+        };
+        // carried rows: A carries plane k - 1 (the previous step's plane k), B carries plane k (the previous step's plane k + 1)
+        BccRow car0[3], car1[3];
+        load_rows(colour ? 0 : (k0 == 0 ? (long long)(nz - 1) * ms : -ms), car0, car1);
+        for (int j = 0; j < Lm; ++j) {
+            const int k = k0 + j;
+            BccRow new0[3], new1[3];
+            Pack<4> sx = ld_rw<4>(pS), sy = ld_rw<4>(pS + P.plane), sz = ld_rw<4>(pS + 2 * P.plane);
+            load_rows(colour ? (k + 1 == nz ? -(long long)(nz - 1) * ms : ms) : 0, new0, new1);   // B: plane k + 1; A: plane k
+            float hc[3][4];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                // rows in the order (k, j), (k, j'), (k', j), (k', j'): plane k is the new load for A and the carried one for B
+                const BccRow* rows[4] = { colour ? &car0[c] : &new0[c], colour ? &car1[c] : &new1[c], colour ? &new0[c] : &car0[c], colour ? &new1[c] : &car1[c] };
+                f2 lo = splat(0.0f), hi = splat(0.0f);
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const Pack<4>& o = rows[r]->o; const float ex = rows[r]->ex;
+                    const f2 slo = colour ? make_float2(o.v[1], o.v[2]) : make_float2(ex, o.v[0]);
+                    const f2 shi = colour ? make_float2(o.v[3], ex) : make_float2(o.v[1], o.v[2]);
+                    lo = add2(lo, add2(make_float2(o.v[0], o.v[1]), slo));
+                    hi = add2(hi, add2(make_float2(o.v[2], o.v[3]), shi));
+                }
+                hc[c][0] = lo.x; hc[c][1] = lo.y; hc[c][2] = hi.x; hc[c][3] = hi.y;
+            }
+            uint32_t w0[4], w1[4];
+#pragma unroll
+            for (int kk = 0; kk < 4; kk += 2) philox4x32_10(key, site0 + (uint32_t)kk, c1, c2, c3, w0[kk], w1[kk], w0[kk + 1], w1[kk + 1]);
+            Pack<4> nxv = sx, nyv = sy, nzv = sz;
+#pragma unroll
+            for (int kp = 0; kp < 4; kp += 2) {
+                V3p S = { make_float2(sx.v[kp], sx.v[kp + 1]), make_float2(sy.v[kp], sy.v[kp + 1]), make_float2(sz.v[kp], sz.v[kp + 1]) };
+                const V3p hp = { make_float2(hc[0][kp], hc[0][kp + 1]), make_float2(hc[1][kp], hc[1][kp + 1]), make_float2(hc[2][kp], hc[2][kp + 1]) };
+                const f2 J2 = splat(P.J);
+                const V3p hJ = { mul2(J2, hp.x), mul2(J2, hp.y), mul2(J2, hp.z) };
+                const V3p ep = (ANISO & 1) ? e2 : B2;
+                V3p d, Sn;
+                cone_move2(S, omc, make_float2(uniform01(w0[kp]), uniform01(w0[kp + 1])),
+                           make_float2(uniform_azimuth(w0[kp], w1[kp]), uniform_azimuth(w0[kp + 1], w1[kp + 1])), d, Sn);
+                const V3p hB = { add2(hJ.x, B2.x), add2(hJ.y, B2.y), add2(hJ.z, B2.z) };
+                f2 s4S, s4v, euS, euv;
+                const f2 dE = delta_energy2_keep<ANISO>(S, d, hB, P.Ku, ep, P.Kc, s4S, s4v, euS, euv);
+                const f2 xx = fma2(dE, splat(invT), make_float2(__logf(uniform01(w1[kp])), __logf(uniform01(w1[kp + 1]))));
+                const bool ok0 = xx.x < 0.0f, ok1 = xx.y < 0.0f;
+                S.x = make_float2(ok0 ? Sn.x.x : S.x.x, ok1 ? Sn.x.y : S.x.y);
+                S.y = make_float2(ok0 ? Sn.y.x : S.y.x, ok1 ? Sn.y.y : S.y.y);
+                S.z = make_float2(ok0 ? Sn.z.x : S.z.x, ok1 ? Sn.z.y : S.z.y);
+                nxv.v[kp] = S.x.x; nxv.v[kp + 1] = S.x.y; nyv.v[kp] = S.y.x; nyv.v[kp + 1] = S.y.y; nzv.v[kp] = S.z.x; nzv.v[kp + 1] = S.z.y;
+                cnt += (int)ok0 + (int)ok1;
+                if (DEBUG) {
+                    if (dbg_x)   { dbg_x[site0 + kp] = xx.x; dbg_x[site0 + kp + 1u] = xx.y; }
+                    if (dbg_acc) { dbg_acc[site0 + kp] = (uint8_t)ok0; dbg_acc[site0 + kp + 1u] = (uint8_t)ok1; }
+                }
+                aM[0] = add2(aM[0], S.x); aM[1] = add2(aM[1], S.y); aM[2] = add2(aM[2], S.z);
+                if (colour == 1) aEx = sub2(aEx, dot3p(S, hJ));
+                if (ANISO) aAn = add2(aAn, onsite_from<ANISO>(ok0, ok1, s4S, s4v, euS, euv, P.Ku, P.Kc));
+                aZe = sub2(aZe, dot3p(S, B2));
+            }
+            st_rw<4>(pS, nxv); st_rw<4>(pS + P.plane, nyv); st_rw<4>(pS + 2 * P.plane, nzv);
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { car0[c] = new0[c]; car1[c] = new1[c]; }
+            pS += ms; pR0 += ms; pR1 += ms; site0 += (uint32_t)ms;
+        }
+    }
+    float f[NQ];
+    f[0] = aM[0].x + aM[0].y; f[1] = aM[1].x + aM[1].y; f[2] = aM[2].x + aM[2].y;
+    f[3] = aEx.x + aEx.y; f[4] = aAn.x + aAn.y; f[5] = aZe.x + aZe.y;
+    f[6] = f[7] = f[8] = 0.0f;
+    long long acc[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) acc[q] = 0;
+    fx_flush(acc, f, P.fx_scale);
+    block_reduce(acc, cnt, P, 0);
+    if (flags & F_FINALIZE) {
+        if (last_block_done(st)) final_reduce(P, 0, flags);
+    }
+}
+
 }  // namespace mc

@@ -19,10 +19,12 @@ def mods():
     return oracle, binding, inputs
 
 
-def _pair(mods, shape, seed=42, cone=0.5, sweep=0, adaptive=False, **ham):
+def _pair(mods, shape, seed=42, cone=0.5, sweep=0, adaptive=False, path=None, **ham):
     oracle, binding, inputs = mods
     o = oracle.Oracle(*shape, seed=seed, cone0=cone, adaptive=adaptive, structure="bcc", **ham)
     g = binding.Lattice(*shape, seed=seed, cone0=cone, adaptive=adaptive, structure="bcc", **ham)
+    if path is not None:
+        g.debug_set_path(path)
     o.set_sweep(sweep); g.set_sweep(sweep)
     return o, g
 
@@ -57,10 +59,35 @@ CASES = [
 ]
 
 
-@pytest.mark.parametrize("shape,T,cone,ham", CASES)
-def test_bcc_half_sweep_parity(mods, shape, T, cone, ham):
+MARCH_CASES = [
+    ((16, 16, 16), 2.0, 0.8, dict(Ku=0.05)),
+    ((12, 5, 9), 0.9, 1.0, dict(Ku=0.2, eu=(0.3, -0.5, 0.81), Kc=0.1, B=(0.1, -0.05, 0.2))),  # odd ny and nz, two segments + remainder
+    ((64, 40, 24), 0.3, 0.4, dict(Ku=0.01)),
+    ((8, 2, 8), 3.0, np.pi, dict(Kc=0.2)),                                                    # 2-cell periodic y: the two rows of a plane coincide
+]
+
+
+@pytest.mark.parametrize("shape,T,cone,ham", MARCH_CASES)
+def test_bcc_half_sweep_parity_forced_march_pass(mods, shape, T, cone, ham):
+    test_bcc_half_sweep_parity(mods, shape, T, cone, ham, path=3)                               # MC_PATH_MARCH
+
+
+def test_bcc_march_pass_is_bit_identical_to_the_generic_pass(mods):
     oracle, binding, inputs = mods
-    o, g = _pair(mods, shape, cone=cone, sweep=(5 << 32) | 777, **ham)
+    for shape, ham in (((32, 24, 20), dict(Ku=0.05, Kc=0.02)), ((16, 7, 11), dict(B=(0.0, 0.1, 0.2)))):
+        out = []
+        for path in (1, 3):
+            g = binding.Lattice(*shape, cone0=0.8, adaptive=True, seed=11, structure="bcc", **ham)
+            g.debug_set_path(path)
+            g.set_spins(inputs.random_unit_spins(g.N, seed=2)); g.sweep(1.7, 7)
+            out.append((g.get_spins(), g.trace()[:, :2])); g.close()
+        assert (out[0][0] == out[1][0]).all() and (out[0][1] == out[1][1]).all(), shape
+
+
+@pytest.mark.parametrize("shape,T,cone,ham", CASES)
+def test_bcc_half_sweep_parity(mods, shape, T, cone, ham, path=None):
+    oracle, binding, inputs = mods
+    o, g = _pair(mods, shape, cone=cone, sweep=(5 << 32) | 777, path=path, **ham)
     g.set_spins(inputs.random_unit_spins(g.N, seed=8))
     worst = 0.0
     for colour in (0, 1, 0, 1):
@@ -110,8 +137,8 @@ def test_bcc_sweep_equals_hooks_and_controller(mods):
 
 
 def test_bcc_ensemble_matches_oracle_and_orders_below_tc(mods):
-    """m(T) of an equilibrated run: GPU against the oracle within 3 standard errors at T = 1.6 (ordered) and 2.4 (above the bcc
-    T_C = 2.054: a simple cubic sweep would still be ordered at 1.6 but also at ... no: it disorders at 1.44)."""
+    """m(T) of an equilibrated run: GPU against the oracle within 3 standard errors at T = 1.6 (ordered: a simple cubic lattice is
+    already disordered there, T_C = 1.44) and at T = 2.4 (above the bcc T_C = 2.054)."""
     from stats_util import blocked_mean_se
     oracle, binding, inputs = mods
     shape = (8, 8, 8)
