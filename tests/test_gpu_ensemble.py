@@ -330,3 +330,11 @@ def test_full_size_c4_constrained_half_sweep_parity(mods, L, colour):
     fin = lead & np.isfinite(x_o) & np.isfinite(x_g)
     print(f"\nfull size {L}^3 constrained: pairs {lead.sum()}, accepted {acc_g[lead].mean():.3f}, flips {differ.sum()}, max |dx| {np.abs(x_g[fin]-x_o[fin]).max():.2e}")
     g.close()
+
+
+def test_full_size_march_pass_half_sweep_parity(mods):
+    """256^3 = 16.8 M spins: the lattice size class whose default kernel is the register-carried march pass (9 z-segments per
+    column, one resident wave) -- one colour pass against the oracle, in the launch configuration mc_sweep uses."""
+    oracle, binding, inputs = mods
+    g = binding.Lattice(256, 256, 256, Kc=0.01); assert g.debug_get_path() == binding.MC_PATH_MARCH; g.close()
+    _full_size_half_sweep(mods, (256, 256, 256), 1.2, 1.2, 7, dict(Kc=0.01), colour=1)
