@@ -61,6 +61,8 @@ def lib():
     L.orc_create.restype = vp
     L.orc_create_bcc.argtypes = [i32, i32, i32, vp, dbl, dbl, vp, dbl, vp, dbl, i32, u64]
     L.orc_create_bcc.restype = vp
+    L.orc_create_fcc.argtypes = [i32, i32, i32, vp, dbl, dbl, vp, dbl, vp, dbl, i32, u64]
+    L.orc_create_fcc.restype = vp
     L.orc_destroy.argtypes = [vp]; L.orc_destroy.restype = None
     for name in ("orc_set_spins", "orc_set_spins_f32", "orc_get_spins", "orc_init_uniform"):
         getattr(L, name).argtypes = [vp, vp]; getattr(L, name).restype = None
@@ -121,19 +123,20 @@ class Oracle:
         self.L = lib()
         self.shape = (nx, ny, nz)
         self.structure = structure
-        self.N = nx * ny * nz * (2 if structure == "bcc" else 1)
+        self.N = nx * ny * nz * {"sc": 1, "bcc": 2, "fcc": 4}[structure]
         per = np.asarray(periodic, dtype=np.int32)
         eu_ = np.asarray(eu, dtype=np.float64); B_ = np.asarray(B, dtype=np.float64)
-        if structure == "bcc":       # two sc sublattices = two colours; site = sublattice*nx*ny*nz + cell (reading C-30)
+        if structure in ("bcc", "fcc"):   # sc sublattices = colours; site = sublattice*nx*ny*nz + cell (readings C-30, C-31)
             if bond_mask is not None or region is not None:
-                raise ValueError("bcc mode has no bond mask / regions")
+                raise ValueError("bcc / fcc mode has no bond mask / regions")
             self._mask = self._region = self._axis = None
-            self.h = self.L.orc_create_bcc(nx, ny, nz, _p(per), J, Ku, _p(eu_), Kc, _p(B_), float(cone0), int(bool(adaptive)), int(seed))
+            make = self.L.orc_create_bcc if structure == "bcc" else self.L.orc_create_fcc
+            self.h = make(nx, ny, nz, _p(per), J, Ku, _p(eu_), Kc, _p(B_), float(cone0), int(bool(adaptive)), int(seed))
             if not self.h:
-                raise ValueError("orc_create_bcc rejected the lattice")
+                raise ValueError("orc_create_bcc / orc_create_fcc rejected the lattice")
             return
         if structure != "sc":
-            raise ValueError("structure must be 'sc' or 'bcc'")
+            raise ValueError("structure must be 'sc', 'bcc' or 'fcc'")
         self._mask = None if bond_mask is None else np.ascontiguousarray(bond_mask, dtype=np.uint8).ravel()
         self._region = None if region is None else np.ascontiguousarray(region, dtype=np.uint16).ravel()
         self._axis = None if region_axis is None else np.ascontiguousarray(region_axis, dtype=np.float64)

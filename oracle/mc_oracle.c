@@ -26,8 +26,9 @@ static const double PI = 3.14159265358979323846;
 
 struct orc_ctx {
     int nx, ny, nz, periodic[3];
-    int structure;          /* 0 = simple cubic (the paper's lattice); 1 = body-centred cubic, see "bcc mode" below */
-    int64_t Ncell;          /* nx*ny*nz: sc N = Ncell; bcc N = 2 Ncell (site = sublattice*Ncell + cell)                    */
+    int structure;          /* 0 = simple cubic (the paper's lattice); 1 = body-centred cubic, 2 = face-centred cubic, see "bcc / fcc mode" */
+    int n_colours;          /* non-interacting subsets swept one after the other: 2 (sc checkerboard, bcc sublattices), 4 (fcc sublattices)  */
+    int64_t Ncell;          /* nx*ny*nz: sc N = Ncell; bcc N = 2 Ncell, fcc N = 4 Ncell (site = sublattice*Ncell + cell)                     */
     int64_t N;
     double J, Ku, eu[3], Kc, B[3];
     uint8_t* mask;          /* NULL = all bonds allowed by the boundary conditions */
@@ -164,7 +165,34 @@ static int64_t bcc_neighbour(const orc_ctx* c, int64_t site, int k8)
     return (int64_t)(1 - sub) * c->Ncell + p[0] + (int64_t)c->nx * (p[1] + (int64_t)c->ny * p[2]);
 }
 
-/* exchange field of ANY site, either structure (sc: decode the site and use the six-direction sum above) */
+/* ------------------------------------------------------------------ fcc mode (reading C-31; "4 simple cubic
+ * sub-lattices for fcc").  The conventional cubic cell (i,j,k) holds four sites: sublattice 0 at the corner, 1 at (0,1/2,1/2),
+ * 2 at (1/2,0,1/2), 3 at (1/2,1/2,0) from it.  The 12 nearest neighbours (distance a/sqrt 2) of a site are 4 in each of the
+ * OTHER three sublattices, none in its own: the four sublattices are four non-interacting subsets, swept as four colours.
+ * Towards sublattice b the offsets of a and b differ along exactly two axes; along such an axis the neighbour's cell index is
+ * {i-1, i} if a sits at 0 and b at 1/2, {i, i+1} the other way round; along the third axis it is i.
+ * Bond index k12 = 4*r + d1 + 2*d2 with r = the rank of b among the other sublattices.  Wrap / open faces as in bcc mode. */
+static const int FCC_OFF[4][3] = { { 0, 0, 0 }, { 0, 1, 1 }, { 1, 0, 1 }, { 1, 1, 0 } };   /* in half lattice constants */
+static int64_t fcc_neighbour(const orc_ctx* c, int64_t site, int k12, int* b_out)
+{
+    int a = (int)(site / c->Ncell); int64_t cell = site % c->Ncell;
+    int r = k12 >> 2, b = r + (r >= a ? 1 : 0);               /* the r-th sublattice other than a */
+    int p[3] = { (int)(cell % c->nx), (int)((cell / c->nx) % c->ny), (int)(cell / ((int64_t)c->nx * c->ny)) };
+    int dim[3] = { c->nx, c->ny, c->nz }, d[2] = { k12 & 1, (k12 >> 1) & 1 }, nd = 0;
+    for (int ax = 0; ax < 3; ++ax) {
+        if (FCC_OFF[a][ax] == FCC_OFF[b][ax]) continue;
+        int step = d[nd++];                                   /* 0 or 1 */
+        p[ax] += FCC_OFF[a][ax] ? step : -step;               /* a at 1/2: {i, i+1};  a at 0: {i, i-1} */
+        if (p[ax] < 0 || p[ax] >= dim[ax]) {
+            if (!c->periodic[ax]) return -1;
+            p[ax] = (p[ax] + dim[ax]) % dim[ax];
+        }
+    }
+    if (b_out) *b_out = b;
+    return (int64_t)b * c->Ncell + p[0] + (int64_t)c->nx * (p[1] + (int64_t)c->ny * p[2]);
+}
+
+/* exchange field of ANY site, any structure (sc: decode the site and use the six-direction sum above) */
 static void field_at(const orc_ctx* c, int64_t site, double h[3])
 {
     if (c->structure == 0) {
@@ -172,6 +200,14 @@ static void field_at(const orc_ctx* c, int64_t site, double h[3])
         return;
     }
     h[0] = h[1] = h[2] = 0.0;
+    if (c->structure == 2) {
+        for (int k = 0; k < 12; ++k) {
+            int64_t j = fcc_neighbour(c, site, k, NULL);
+            if (j < 0) continue;
+            for (int a = 0; a < 3; ++a) h[a] += c->J * c->S[3 * j + a];
+        }
+        return;
+    }
     for (int k = 0; k < 8; ++k) {
         int64_t j = bcc_neighbour(c, site, k);
         if (j < 0) continue;
@@ -215,6 +251,23 @@ double orc_site_energy(const orc_ctx* c, int64_t site, const double S[3])
 double orc_total_energy(const orc_ctx* c)
 {
     double E = 0.0;
+    if (c->structure == 2) {                 /* fcc: a bond joins two different sublattices: visit it from the lower one */
+        for (int64_t i = 0; i < c->N; ++i) {
+            const double* S = &c->S[3 * i];
+            int a = (int)(i / c->Ncell);
+            for (int k = 0; k < 12; ++k) {
+                int b; int64_t j = fcc_neighbour(c, i, k, &b);
+                if (j < 0 || b < a) continue;
+                const double* Sj = &c->S[3 * j];
+                E -= c->J * (S[0] * Sj[0] + S[1] * Sj[1] + S[2] * Sj[2]);
+            }
+            double se = S[0] * c->eu[0] + S[1] * c->eu[1] + S[2] * c->eu[2];
+            double x2 = S[0] * S[0], y2 = S[1] * S[1], z2 = S[2] * S[2];
+            E += -c->Ku * se * se + c->Kc * (x2 * y2 + x2 * z2 + y2 * z2)
+                 - (S[0] * c->B[0] + S[1] * c->B[1] + S[2] * c->B[2]);
+        }
+        return E;
+    }
     if (c->structure) {                      /* bcc: every bond joins an A and a B site: visit the 8 bonds of every A site */
         for (int64_t i = 0; i < c->N; ++i) {
             const double* S = &c->S[3 * i];
@@ -265,7 +318,7 @@ orc_ctx* orc_create(int nx, int ny, int nz, const int periodic[3],
     orc_ctx* c = (orc_ctx*)calloc(1, sizeof(orc_ctx));
     c->nx = nx; c->ny = ny; c->nz = nz;
     for (int a = 0; a < 3; ++a) c->periodic[a] = periodic[a];
-    c->N = (int64_t)nx * ny * nz; c->Ncell = c->N; c->structure = 0;
+    c->N = (int64_t)nx * ny * nz; c->Ncell = c->N; c->structure = 0; c->n_colours = 2;
     c->J = J; c->Ku = Ku; c->Kc = Kc;
     double n = sqrt(eu[0] * eu[0] + eu[1] * eu[1] + eu[2] * eu[2]);
     for (int a = 0; a < 3; ++a) { c->eu[a] = (n > 0) ? eu[a] / n : (a == 2); c->B[a] = B[a]; }
@@ -295,13 +348,27 @@ orc_ctx* orc_create_bcc(int nx, int ny, int nz, const int periodic[3],
     if (nx < 1 || ny < 1 || nz < 1) return NULL;
     for (int a = 0; a < 3; ++a) if (periodic[a] < 0 || periodic[a] > 1) return NULL;
     orc_ctx* c = (orc_ctx*)calloc(1, sizeof(orc_ctx));
-    c->nx = nx; c->ny = ny; c->nz = nz; c->structure = 1;
+    c->nx = nx; c->ny = ny; c->nz = nz; c->structure = 1; c->n_colours = 2;
     for (int a = 0; a < 3; ++a) c->periodic[a] = periodic[a];
     c->Ncell = (int64_t)nx * ny * nz; c->N = 2 * c->Ncell;
     c->J = J; c->Ku = Ku; c->Kc = Kc;
     double n = sqrt(eu[0] * eu[0] + eu[1] * eu[1] + eu[2] * eu[2]);
     for (int a = 0; a < 3; ++a) { c->eu[a] = (n > 0) ? eu[a] / n : (a == 2); c->B[a] = B[a]; }
     c->cone = cone0_rad; c->adaptive = adaptive; c->seed = seed; c->sweep = 0; c->sampling = 1;
+    c->S = (double*)malloc(sizeof(double) * 3 * c->N);
+    for (int64_t i = 0; i < c->N; ++i) { c->S[3 * i] = 0; c->S[3 * i + 1] = 0; c->S[3 * i + 2] = 1; }
+    return c;
+}
+
+/* fcc lattice of nx x ny x nz conventional cells, 4 nx ny nz spins, four colours (fcc mode above) */
+orc_ctx* orc_create_fcc(int nx, int ny, int nz, const int periodic[3],
+                        double J, double Ku, const double eu[3], double Kc, const double B[3],
+                        double cone0_rad, int adaptive, uint64_t seed)
+{
+    orc_ctx* c = orc_create_bcc(nx, ny, nz, periodic, J, Ku, eu, Kc, B, cone0_rad, adaptive, seed);
+    if (!c) return NULL;
+    c->structure = 2; c->n_colours = 4; c->N = 4 * c->Ncell;
+    free(c->S);
     c->S = (double*)malloc(sizeof(double) * 3 * c->N);
     for (int64_t i = 0; i < c->N; ++i) { c->S[3 * i] = 0; c->S[3 * i + 1] = 0; c->S[3 * i + 2] = 1; }
     return c;
@@ -479,6 +546,7 @@ void orc_sweep(orc_ctx* c, double T, int64_t n)
     for (int64_t it = 0; it < n; ++it) {
         int64_t count = orc_half_sweep(c, T, 0, NULL, NULL);  /* P:166 */
         count += orc_half_sweep(c, T, 1, NULL, NULL);         /* P:167 */
+        for (int col = 2; col < c->n_colours; ++col) count += orc_half_sweep(c, T, col, NULL, NULL);   /* fcc: two more subsets (P:34) */
         orc_end_sweep(c, count);
     }
 }

@@ -63,6 +63,11 @@ orc_ctx* orc_create(int nx, int ny, int nz, const int periodic[3],
 orc_ctx* orc_create_bcc(int nx, int ny, int nz, const int periodic[3],
                         double J, double Ku, const double eu[3], double Kc, const double B[3],
                         double cone0_rad, int adaptive, uint64_t seed);
+/* Face-centred cubic lattice (four simple cubic sublattices = FOUR colours; reading C-31): 4 nx ny nz spins, 12 nearest
+ * neighbours, 4 in each other sublattice; site = sublattice*nx*ny*nz + cell; a sweep is four colour passes 0, 1, 2, 3. */
+orc_ctx* orc_create_fcc(int nx, int ny, int nz, const int periodic[3],
+                        double J, double Ku, const double eu[3], double Kc, const double B[3],
+                        double cone0_rad, int adaptive, uint64_t seed);
 void orc_destroy(orc_ctx*);
 /* periodic[a]: 0 open faces, 1 periodic, 2 anti-periodic (the spin across the wrap enters as -S_j). */
 /* Slice-averaged magnetisation along x: out[3*x + a], a = x,y,z component. */
