@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libmc_b200.so")
 MC_OK, MC_EINVAL, MC_ECUDA, MC_ESTATE = 0, -1, -2, -3
 MC_TRACE_CAPACITY = 16384
 MC_PATH_AUTO, MC_PATH_GENERIC, MC_PATH_STAGED, MC_PATH_MARCH = 0, 1, 2, 3
-MC_SC, MC_BCC = 0, 1
+MC_SC, MC_BCC, MC_FCC = 0, 1, 2
 
 # every symbol include/mc.h declares (tests/test_abi.py checks the header against this list and the .so)
 SYMBOLS = [
@@ -104,7 +104,7 @@ def make_structs(shape, periodic=(1, 1, 1), J=1.0, Ku=0.0, eu=(0, 0, 1), Kc=0.0,
                  bond_mask=None, region=None, region_axis=None, cone0=0.5, adaptive=True, structure="sc"):
     """Fills mc_lattice / mc_hamiltonian; returns them plus the arrays that must stay alive during mc_create."""
     lat = McLattice(int(shape[0]), int(shape[1]), int(shape[2]), (C.c_int32 * 3)(*[int(p) for p in periodic]),   # 0 open, 1 periodic, 2 anti-periodic (x)
-                    {"sc": MC_SC, "bcc": MC_BCC}[structure])
+                    {"sc": MC_SC, "bcc": MC_BCC, "fcc": MC_FCC}[structure])
     keep = []
     def arr(a, dt):
         if a is None:
@@ -130,7 +130,7 @@ class Lattice:
         import torch  # device memory and streams only
         self.L = load()
         self.shape = (int(nx), int(ny), int(nz))
-        self.N = int(nx) * int(ny) * int(nz) * (2 if structure == "bcc" else 1)      # bcc: two spins per conventional cell
+        self.N = int(nx) * int(ny) * int(nz) * {"sc": 1, "bcc": 2, "fcc": 4}[structure]      # spins per conventional cell
         self.h = None
         lat, ham, keep = make_structs(self.shape, periodic, J, Ku, eu, Kc, B, bond_mask, region, region_axis, cone0, adaptive, structure)
         nbytes = self.L.mc_workspace_bytes(C.byref(lat), C.byref(ham))

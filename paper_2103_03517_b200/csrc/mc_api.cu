@@ -33,10 +33,10 @@ bool valid_lattice(const mc_lattice* lat)
 {
     if (!lat) return false;
     const int dim[3] = { lat->nx, lat->ny, lat->nz };
-    if (lat->structure == MC_BCC) {          // P:34, C-30: fully periodic, rows of float4 items
+    if (lat->structure == MC_BCC || lat->structure == MC_FCC) {          // P:34, C-30 / C-31: fully periodic, rows of float4 items
         for (int a = 0; a < 3; ++a) if (dim[a] < 1 || lat->periodic[a] != 1) return false;
         if (lat->nx % 4) return false;
-        return 2.0 * (double)lat->nx * lat->ny * lat->nz < 2147483648.0;
+        return (lat->structure == MC_FCC ? 4.0 : 2.0) * (double)lat->nx * lat->ny * lat->nz < 2147483648.0;
     }
     if (lat->structure != MC_SC) return false;
     for (int a = 0; a < 3; ++a) {
@@ -52,14 +52,15 @@ bool valid_lattice(const mc_lattice* lat)
 Layout make_layout(const mc_lattice* lat, const mc_hamiltonian* ham)
 {
     Layout L{};
-    const bool bcc = lat->structure == MC_BCC;
-    const size_t Nc = bcc ? (size_t)lat->nx * lat->ny * lat->nz : (size_t)lat->nx / 2 * lat->ny * lat->nz;
+    const bool sub = lat->structure == MC_BCC || lat->structure == MC_FCC;      // sublattices as colours, each a full grid of cells
+    const size_t ncol = lat->structure == MC_FCC ? 4 : 2;
+    const size_t Nc = sub ? (size_t)lat->nx * lat->ny * lat->nz : (size_t)lat->nx / 2 * lat->ny * lat->nz;
     L.plane = (long long)round_up(Nc, 64);
     L.mask_plane = (long long)round_up(Nc, 256);
     L.region_plane = (long long)round_up(Nc, 128);
     L.max_blocks = MAX_BLOCKS;
     size_t off = 0;
-    L.spins = off;    off += round_up((size_t)6 * L.plane * sizeof(float), ALIGN);
+    L.spins = off;    off += round_up((size_t)3 * ncol * L.plane * sizeof(float), ALIGN);
     L.mask = off;     if (needs_mask(lat, ham)) off += round_up((size_t)2 * L.mask_plane, ALIGN);
     L.region = off;   if (ham->region) off += round_up((size_t)2 * L.region_plane * sizeof(uint16_t), ALIGN);
     L.axis = off;     if (ham->region) off += round_up((size_t)ham->n_regions * sizeof(float4), ALIGN);
@@ -67,7 +68,7 @@ Layout make_layout(const mc_lattice* lat, const mc_hamiltonian* ham)
     L.trace = off;    off += round_up((size_t)TRACE_CAP * 6 * sizeof(double), ALIGN);
     // staging: the [N][3] fp32 lexicographic image of the state during mc_set_spins / mc_get_spins, or the [N] fp32 + [N] u8
     // outputs of a half-sweep hook, or the 3 nx int64 sums of mc_profile_x -- the library allocates nothing itself
-    const size_t N = 2 * Nc;
+    const size_t N = ncol * Nc;
     L.staging_bytes = round_up(N * 3 * sizeof(float), ALIGN) + round_up((size_t)lat->nx * 3 * sizeof(long long), ALIGN);
     L.staging = off;  off += L.staging_bytes;
     L.total = off;
@@ -126,8 +127,8 @@ int launch_state(mc_ctx* ctx, int what, double a = 0, double b = 0, double c = 0
 int measure(mc_ctx* ctx)
 {
     int rc;
-    if ((rc = launch_pass(ctx, MODE_MEASURE, 0, 0.0f, F_TORQUE, nullptr, nullptr))) return rc;
-    if ((rc = launch_pass(ctx, MODE_MEASURE, 1, 0.0f, F_TORQUE | F_FINALIZE, nullptr, nullptr))) return rc;
+    for (int col = 0; col < ctx->P.ncol; ++col)
+        if ((rc = launch_pass(ctx, MODE_MEASURE, col, 0.0f, F_TORQUE | (col + 1 == ctx->P.ncol ? F_FINALIZE : 0), nullptr, nullptr))) return rc;
     ctx->ml_valid = true;
     return MC_OK;
 }
@@ -174,7 +175,7 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     *out = nullptr;
     if (!valid_lattice(lat) || !ham || !dev_workspace) return MC_EINVAL;
     if (ham->region && (ham->n_regions < 1 || ham->n_regions > 65536 || !ham->region_axis)) return MC_EINVAL;
-    if (lat->structure == MC_BCC && (ham->bond_mask || ham->region)) return MC_EINVAL;
+    if (lat->structure != MC_SC && (ham->bond_mask || ham->region)) return MC_EINVAL;
     if (((uintptr_t)dev_workspace) % ALIGN) return MC_EINVAL;
     const Layout L = make_layout(lat, ham);
     if (workspace_bytes < L.total) return MC_EINVAL;
@@ -200,13 +201,14 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     if (cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return bail(MC_ECUDA, "cannot query the device");
 
     const int nx = lat->nx, ny = lat->ny, nz = lat->nz;
-    const bool bcc = lat->structure == MC_BCC;
-    const uint32_t N = (uint32_t)nx * ny * nz * (bcc ? 2u : 1u), R = bcc ? nx : nx / 2, Nc = N / 2;
+    const bool bcc = lat->structure == MC_BCC, fcc = lat->structure == MC_FCC;
+    const uint32_t ncol = fcc ? 4u : 2u;
+    const uint32_t Nc = (bcc || fcc) ? (uint32_t)nx * ny * nz : (uint32_t)nx / 2 * ny * nz, N = ncol * Nc, R = (bcc || fcc) ? nx : nx / 2;
     char* ws = (char*)dev_workspace;
     Params& P = ctx->P;
     P.nx = nx; P.ny = ny; P.nz = nz; P.R = (int)R; P.Nc = Nc; P.N = N; P.invN = 1.0 / (double)N;
     P.anti_x = lat->periodic[0] == 2 ? 1 : 0;
-    P.bcc = bcc ? 1 : 0;
+    P.bcc = bcc ? 1 : 0; P.fcc = fcc ? 1 : 0; P.ncol = (int)ncol;
     P.per_mask = (lat->periodic[0] ? 1 : 0) | (lat->periodic[1] ? 2 : 0) | (lat->periodic[2] ? 4 : 0);
     P.plane = L.plane; P.S = (float*)(ws + L.spins);
     P.mask = nullptr; P.mask_plane = L.mask_plane; P.region = nullptr; P.region_plane = L.region_plane; P.axis = nullptr;
@@ -228,13 +230,13 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     ctx->aniso = (ham->Ku != 0.0 ? 1 : 0) | (ham->Kc != 0.0 ? 2 : 0);
     ctx->field = ham->B[0] != 0.0 || ham->B[1] != 0.0 || ham->B[2] != 0.0;
     ctx->masked = needs_mask(lat, ham);
-    ctx->vec = (bcc || nx % 8 == 0) ? 4 : 1;
+    ctx->vec = (bcc || fcc || nx % 8 == 0) ? 4 : 1;
     ctx->geom.RV = R / ctx->vec; ctx->geom.n_items = Nc / ctx->vec;
     ctx->geom.div_rv = make_div(ctx->geom.RV); ctx->geom.div_nz = make_div((uint32_t)nz);
     { uint32_t sh = 0; while (sh < 5 && ny % (2 << sh) == 0) ++sh; ctx->geom.yb_shift = sh; }      // up to 32 rows per block
 
     // pairing geometry (C-11); the constrained path needs an even colour population (C-15)
-    ctx->pair_ok = (Nc % 2 == 0) && Nc >= 2 && !bcc;          // the constrained path is built for the sc lattice
+    ctx->pair_ok = (Nc % 2 == 0) && Nc >= 2 && !bcc && !fcc;  // the constrained path is built for the sc lattice
     if (ctx->pair_ok) {
         PairGeom& G = ctx->pgeom;
         uint32_t Bc = 32; while (Nc % (2 * Bc)) Bc >>= 1;
@@ -439,8 +441,9 @@ int mc_sweep(mc_ctx* ctx, double T, int64_t n)
     }
     for (int64_t i = 0; i < n; ++i) {
         int rc;
-        if ((rc = launch_pass(ctx, MODE_SWEEP, 0, invT, 0, nullptr, nullptr))) return rc;
-        if ((rc = launch_pass(ctx, MODE_SWEEP, 1, invT, F_FINALIZE, nullptr, nullptr))) return rc;
+        for (int col = 0; col + 1 < ctx->P.ncol; ++col)
+            if ((rc = launch_pass(ctx, MODE_SWEEP, col, invT, 0, nullptr, nullptr))) return rc;                         // P:166 (fcc: three of four subsets)
+        if ((rc = launch_pass(ctx, MODE_SWEEP, ctx->P.ncol - 1, invT, F_FINALIZE, nullptr, nullptr))) return rc;
     }
     if (n > 0) ctx->ml_valid = true;      // finalize refreshed M_L = M.e_C
     return MC_OK;
@@ -536,7 +539,7 @@ static int hook_common(mc_ctx* ctx, int colour, float* host_x, uint8_t* host_acc
     const int nx = ctx->P.nx, ny = ctx->P.ny;
     for (uint32_t s = 0; s < N; ++s) {
         const int x = s % nx, y = (s / nx) % ny, z = s / ((uint32_t)nx * ny);
-        if ((ctx->P.bcc ? (int)(s >= ctx->P.Nc) : ((x + y + z) & 1)) != colour) continue;      // bcc: colour = sublattice
+        if (((ctx->P.bcc || ctx->P.fcc) ? (int)(s / ctx->P.Nc) : ((x + y + z) & 1)) != colour) continue;      // bcc / fcc: colour = sublattice
         if (host_x) host_x[s] = hx[s];
         if (host_acc) host_acc[s] = ha[s];
     }
@@ -548,7 +551,7 @@ static int hook_common(mc_ctx* ctx, int colour, float* host_x, uint8_t* host_acc
 int mc_half_sweep(mc_ctx* ctx, double T, int colour, float* host_x, uint8_t* host_acc)
 {
     CHECK_CTX();
-    if (!(T > 0.0) || (colour != 0 && colour != 1)) return fail(ctx, MC_EINVAL, "mc_half_sweep: need T > 0 and colour in {0,1}");
+    if (!(T > 0.0) || colour < 0 || colour >= ctx->P.ncol) return fail(ctx, MC_EINVAL, "mc_half_sweep: need T > 0 and a colour of the lattice (0, 1; fcc: 0..3)");
     return hook_common(ctx, colour, host_x, host_acc, false, (float)(1.0 / T));
 }
 
@@ -606,7 +609,7 @@ int mc_profile_x(mc_ctx* ctx, double* host_profile)
 {
     CHECK_CTX();
     if (!host_profile) return fail(ctx, MC_EINVAL, "mc_profile_x: null pointer");
-    if (ctx->P.bcc) return fail(ctx, MC_EINVAL, "mc_profile_x: simple cubic lattices only");
+    if (ctx->P.bcc || ctx->P.fcc) return fail(ctx, MC_EINVAL, "mc_profile_x: simple cubic lattices only");
     const int nx = ctx->P.nx;
     const size_t bytes = (size_t)nx * 3 * sizeof(long long);
     long long* tmp = (long long*)((char*)ctx->staging + ctx->staging_bytes - round_up(bytes, ALIGN));   // tail of the staging area

@@ -46,6 +46,8 @@ struct Params {
     int nx, ny, nz, R;               // R = nx/2 sites of one colour per row
     int anti_x;                      // 1: anti-periodic boundary along x (domain-wall box); the wrap bond sees -S_j
     int per_mask;                    // bit a set: axis a (x, y, z) is periodic (or anti-periodic)
+    int fcc;                         // 1: face-centred cubic (C-31): FOUR colours = sublattices, R = nx, 12 neighbours
+    int ncol;                        // colours swept per Monte Carlo iteration: 2 (sc, bcc), 4 (fcc)
     int bcc;                         // 1: body-centred cubic (C-30): colour = sublattice, R = nx cells per row, 8 neighbours
     uint32_t Nc;                     // sites per colour
     uint32_t N;
@@ -281,6 +283,76 @@ __device__ __forceinline__ void bcc_exchange_field(const Params& P, const BccPos
     }
 #pragma unroll
     for (int k = 0; k < 4; ++k) h[k] = { hc[0][k], hc[1][k], hc[2][k] };
+}
+
+// --------------------------------------------------------------------------------------------------------------
+// fcc (C-31): four simple cubic sublattices = FOUR colours, each a full nx x ny x nz grid in cell order (R = nx):
+// sublattice 0 at the cell corner, 1 at (0,1/2,1/2), 2 at (1/2,0,1/2), 3 at (1/2,1/2,0).  A site has 4 neighbours in each
+// OTHER sublattice b: the offsets of a and b differ along two axes; along such an axis the neighbour's cell index is
+// {i, i - 1} if a sits at 0 and b at 1/2, {i, i + 1} the other way round.  An item is 4 consecutive cells of a row; if x
+// is one of the two axes a sublattice costs 2 rows x (float4 + the one cell outside the item), else 4 rows x float4.
+// hl collects the neighbours in sublattices b < a only: E_exch = -J sum_a sum_{i in a} S_i . hl_i counts every bond once,
+// in the pass of its higher colour, when both ends are final.
+// --------------------------------------------------------------------------------------------------------------
+struct FccPos { uint32_t a0, site0, i0, y, z; };
+__device__ __forceinline__ FccPos fcc_locate(const Params& P, const Geom& G, uint32_t item, int colour)
+{
+    uint32_t rowp, xq;
+    G.div_rv.divmod(item, rowp, xq);
+    FccPos q;
+    q.z = rowp / (uint32_t)P.ny; q.y = rowp - q.z * (uint32_t)P.ny;
+    q.i0 = xq * 4u;
+    q.a0 = rowp * (uint32_t)P.nx + q.i0;
+    q.site0 = (uint32_t)colour * P.Nc + q.a0;
+    return q;
+}
+__device__ __forceinline__ void fcc_exchange_field(const Params& P, const FccPos& q, int colour, Vec3 (&h)[4], Vec3 (&hl)[4])
+{
+    const uint32_t nx = (uint32_t)P.nx, ny = (uint32_t)P.ny, nz = (uint32_t)P.nz;
+    const uint32_t offm_tab = 0x3560u;                               // offsets as bit masks (bit 0 x, 1 y, 2 z): sublattice 0: 0, 1: 6, 2: 5, 3: 3
+    const uint32_t oa = (offm_tab >> (4 * colour)) & 7u;
+    float hc[3][4], hlc[3][4];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { hc[c][k] = 0.0f; hlc[c][k] = 0.0f; }
+#pragma unroll
+    for (int r = 0; r < 3; ++r) {
+        const int b = r + (r >= colour ? 1 : 0);
+        const uint32_t ob = (offm_tab >> (4 * b)) & 7u, D = oa ^ ob;
+        const float* O = P.S + (long long)b * 3 * P.plane;
+        // the second row / plane of the pair along a differing axis: +1 if a sits at 1/2, -1 if at 0
+        const uint32_t y2 = (D & 2u) ? ((oa & 2u) ? (q.y + 1 == ny ? 0u : q.y + 1) : (q.y == 0 ? ny - 1 : q.y - 1)) : q.y;
+        const uint32_t z2 = (D & 4u) ? ((oa & 4u) ? (q.z + 1 == nz ? 0u : q.z + 1) : (q.z == 0 ? nz - 1 : q.z - 1)) : q.z;
+        const bool xs = (D & 1u) != 0, xplus = (oa & 1u) != 0;
+        const uint32_t xe = xplus ? (q.i0 + 4 == nx ? 0u : q.i0 + 4) : (q.i0 == 0 ? nx - 1 : q.i0 - 1);
+        const uint32_t rows[4] = { (q.z * ny + q.y) * nx, (q.z * ny + y2) * nx, (z2 * ny + q.y) * nx, (z2 * ny + y2) * nx };
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const float* Oc = O + (long long)c * P.plane;
+            float s[4] = { 0.f, 0.f, 0.f, 0.f };
+            if (xs) {                                                // x and one of y, z differ: rows (y,z) and (y2,z2); cells i and i -+ 1
+#pragma unroll
+                for (int rr = 0; rr < 4; rr += 3) {
+                    const Pack<4> o = ld_nc<4>(Oc + rows[rr] + q.i0);
+                    const float ex = __ldg(Oc + rows[rr] + xe);
+                    s[0] += o.v[0] + (xplus ? o.v[1] : ex);   s[1] += o.v[1] + (xplus ? o.v[2] : o.v[0]);
+                    s[2] += o.v[2] + (xplus ? o.v[3] : o.v[1]); s[3] += o.v[3] + (xplus ? ex : o.v[2]);
+                }
+            } else {                                                 // y and z differ: the four rows, cell i
+#pragma unroll
+                for (int rr = 0; rr < 4; ++rr) {
+                    const Pack<4> o = ld_nc<4>(Oc + rows[rr] + q.i0);
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) s[k] += o.v[k];
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) { hc[c][k] += s[k]; if (b < colour) hlc[c][k] += s[k]; }
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { h[k] = { hc[0][k], hc[1][k], hc[2][k] }; hl[k] = { hlc[0][k], hlc[1][k], hlc[2][k] }; }
 }
 
 // easy axes of the VEC sites of an item: uniform, or per grain through the region table (config c5)

@@ -17,11 +17,11 @@ template <int VEC, int MODE> PassFn pick_pass(int aniso, bool masked)
     }
 }
 
-template <int MODE> PassFn pick_pass_bcc(int aniso)
+template <int MODE, int LAT> PassFn pick_pass_lat(int aniso)
 {
     switch (aniso) {
-        case 0: return pass_kernel<4, 0, false, MODE, true>;  case 1: return pass_kernel<4, 1, false, MODE, true>;
-        case 2: return pass_kernel<4, 2, false, MODE, true>;  default: return pass_kernel<4, 3, false, MODE, true>;
+        case 0: return pass_kernel<4, 0, false, MODE, LAT>;  case 1: return pass_kernel<4, 1, false, MODE, LAT>;
+        case 2: return pass_kernel<4, 2, false, MODE, LAT>;  default: return pass_kernel<4, 3, false, MODE, LAT>;
     }
 }
 
@@ -31,7 +31,8 @@ int launch_pass_generic(mc_ctx* ctx, int mode, int colour, float invT, int flags
 {
     PassFn fn = (ctx->vec == 4) ? (mode == MODE_SWEEP ? pick_pass<4, MODE_SWEEP>(ctx->aniso, ctx->masked) : pick_pass<4, MODE_MEASURE>(ctx->aniso, ctx->masked))
                                 : (mode == MODE_SWEEP ? pick_pass<1, MODE_SWEEP>(ctx->aniso, ctx->masked) : pick_pass<1, MODE_MEASURE>(ctx->aniso, ctx->masked));
-    if (ctx->P.bcc) fn = mode == MODE_SWEEP ? pick_pass_bcc<MODE_SWEEP>(ctx->aniso) : pick_pass_bcc<MODE_MEASURE>(ctx->aniso);
+    if (ctx->P.bcc) fn = mode == MODE_SWEEP ? pick_pass_lat<MODE_SWEEP, 1>(ctx->aniso) : pick_pass_lat<MODE_MEASURE, 1>(ctx->aniso);
+    if (ctx->P.fcc) fn = mode == MODE_SWEEP ? pick_pass_lat<MODE_SWEEP, 2>(ctx->aniso) : pick_pass_lat<MODE_MEASURE, 2>(ctx->aniso);
     const int grid = grid_for(ctx, ctx->geom.n_items, MC_PASS_MIN_BLOCKS);
     MC_CU(launch_dependent(fn, grid, BLOCK, 0, ctx->stream, ctx->P, ctx->geom, colour, invT, flags, dx, da));
     ctx->launches += 1;

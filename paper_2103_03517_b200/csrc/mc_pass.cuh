@@ -15,8 +15,9 @@ namespace mc {
 #ifndef MC_PASS_MIN_BLOCKS
 #define MC_PASS_MIN_BLOCKS 3      // <= 80 registers: three CTAs per SM (c5 film: one 354, two 185, three 166 us per sweep)
 #endif
-// BCC: the bcc lattice of P:34 (mc_common.cuh): VEC = 4 consecutive cells of one sublattice, site stride 1 instead of 2.
-template <int VEC, int ANISO, bool MASKED, int MODE, bool BCC = false>
+// LAT: 0 simple cubic; 1 bcc, 2 fcc (mc_common.cuh): VEC = 4 consecutive cells of one sublattice, site stride 1 instead of 2;
+// fcc: four colours, the exchange energy of a bond is summed in the pass of its higher colour (hl).
+template <int VEC, int ANISO, bool MASKED, int MODE, int LAT = 0>
 __global__ void __launch_bounds__(BLOCK, MC_PASS_MIN_BLOCKS)
 pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, int colour, float invT, int flags,
             float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
@@ -38,14 +39,18 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
 
     const uint32_t stride = gridDim.x * BLOCK;
     for (uint32_t item = blockIdx.x * BLOCK + threadIdx.x; item < G.n_items; item += stride) {
-        static_assert(!BCC || (VEC == 4 && !MASKED), "the bcc pass is the VEC = 4, unmasked instantiation");
-        constexpr uint32_t SS = BCC ? 1u : 2u;                    // site-id stride between the sites of an item
+        static_assert(!LAT || (VEC == 4 && !MASKED), "the bcc / fcc passes are VEC = 4, unmasked instantiations");
+        constexpr uint32_t SS = LAT ? 1u : 2u;                    // site-id stride between the sites of an item
         ItemPos q;
-        Vec3 h[VEC], e[VEC];
-        if (BCC) {
+        Vec3 h[VEC], e[VEC], hl[LAT == 2 ? VEC : 1];
+        if (LAT == 1) {
             const BccPos b = bcc_locate(P, G, item, colour);
             q.a0 = b.a0; q.site0 = b.site0; q.xh0 = b.i0; q.par = 0u;
             if (VEC == 4) bcc_exchange_field(P, b, colour, reinterpret_cast<Vec3(&)[4]>(h));
+        } else if (LAT == 2) {
+            const FccPos b = fcc_locate(P, G, item, colour);
+            q.a0 = b.a0; q.site0 = b.site0; q.xh0 = b.i0; q.par = 0u;
+            if (VEC == 4) fcc_exchange_field(P, b, colour, reinterpret_cast<Vec3(&)[4]>(h), reinterpret_cast<Vec3(&)[4]>(hl));
         } else {
             q = locate<VEC>(P, G, item, colour);
             exchange_field<VEC, MASKED>(P, q, colour, h);
@@ -98,7 +103,10 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
                 if (dbg_x)   { dbg_x[q.site0 + SS * kp] = xx.x; dbg_x[q.site0 + SS * kp + SS] = xx.y; }
                 if (dbg_acc) { dbg_acc[q.site0 + SS * kp] = (uint8_t)ok0; dbg_acc[q.site0 + SS * kp + SS] = (uint8_t)ok1; }
                 f2s[0] = add2(f2s[0], S.x); f2s[1] = add2(f2s[1], S.y); f2s[2] = add2(f2s[2], S.z);
-                if (colour == 1) f2s[3] = sub2(f2s[3], dot3p(S, hJ));
+                if (LAT == 2) {
+                    const V3p hlp = pack3(hl[LAT == 2 ? kp : 0], hl[LAT == 2 ? kp + 1 : 0]);
+                    f2s[3] = sub2(f2s[3], dot3p(S, V3p{ mul2(J2, hlp.x), mul2(J2, hlp.y), mul2(J2, hlp.z) }));
+                } else if (colour == 1) f2s[3] = sub2(f2s[3], dot3p(S, hJ));
                 if (ANISO) f2s[4] = add2(f2s[4], onsite_from<ANISO>(ok0, ok1, s4S, s4v, euS, euv, P.Ku, P.Kc));
                 f2s[5] = sub2(f2s[5], dot3p(S, B2));
             }
@@ -122,7 +130,8 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
                 if (dbg_acc) dbg_acc[q.site0 + SS * k] = (uint8_t)ok;
             }
             f[0] += S.x; f[1] += S.y; f[2] += S.z;
-            if (colour == 1) f[3] -= dot3(S, hJ);
+            if (LAT == 2) { const Vec3& g = hl[LAT == 2 ? k : 0]; f[3] -= dot3(S, Vec3{ P.J * g.x, P.J * g.y, P.J * g.z }); }
+            else if (colour == 1) f[3] -= dot3(S, hJ);
             if (ANISO) f[4] += aniso_energy<ANISO>(S, P.Ku, e[(ANISO & 1) ? k : 0], P.Kc);
             f[5] -= dot3(S, B);
             if (MODE == MODE_MEASURE && (flags & F_TORQUE)) {        // the unconstrained sweep never samples the torque

@@ -47,7 +47,7 @@ def _half(o, g, T, colour):
     assert (changed[mine] == (acc_g[mine] == 1)).all()
     assert np.abs(np.linalg.norm(after_g, axis=1) - 1).max() < 2e-7
     near = mine & (np.abs(x_o) < 2.0)
-    return int(differ.sum()), float(np.abs(x_g[near] - x_o[near]).max())
+    return int(differ.sum()), float(np.abs(x_g[near] - x_o[near]).max()) if near.any() else 0.0
 
 
 CASES = [

@@ -524,7 +524,8 @@ def test_no_kernel_writes_outside_the_workspace(mods):
             dict(shape=(2, 1, 1), ham=dict(periodic=(0, 0, 0))), dict(shape=(8, 6, 5), ham=dict(periodic=(1, 0, 0), Ku=0.05)),
             dict(shape=(64, 64, 64), ham=dict(Kc=0.01)), dict(shape=(96, 40, 36), ham=dict(Ku=0.1), path=2),
             dict(shape=(80, 30, 58), ham=dict(periodic=(2, 1, 1), Ku=0.05), path=2),
-            dict(shape=(12, 5, 7), ham=dict(Ku=0.2, structure="bcc")), dict(shape=(4, 1, 1), ham=dict(structure="bcc"))]
+            dict(shape=(12, 5, 7), ham=dict(Ku=0.2, structure="bcc")), dict(shape=(4, 1, 1), ham=dict(structure="bcc")),
+            dict(shape=(12, 5, 7), ham=dict(Kc=0.1, structure="fcc")), dict(shape=(4, 1, 1), ham=dict(structure="fcc"))]
     for r in runs:
         g = binding.Lattice(*r["shape"], cone0=0.8, adaptive=True, seed=3, guard_bytes=G, **r["ham"])
         if "path" in r: g.debug_set_path(r["path"])
