@@ -198,7 +198,7 @@ def time_other_paths(binding, torch, local_rank, sweeps=100):
     ms = e0.elapsed_time(e1)
     ups = g.N * sweeps / (ms * 1e-3)
     out["fcc_140^3_cells_Ku0.01_T2.8"] = {"value": ups, "unit": UNIT, "us_per_sweep": 1e3 * ms / sweeps, "algorithmic_GBs": 60 * ups / 1e9,
-                                        "kernel": "pass_kernel<4, uniaxial, fcc> (generic gather, 12 neighbours, 4 passes per sweep; 60 B per update: each pass reads the three other sublattices)"}
+                                        "kernel": "pass_kernel<4, uniaxial, fcc, colour> (generic gather, colour as a compile-time constant, 12 neighbours, 4 passes per sweep; 60 B per update: each pass reads the three other sublattices)"}
     g.close()
     return out
 

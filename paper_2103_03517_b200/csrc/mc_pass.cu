@@ -25,6 +25,21 @@ template <int MODE, int LAT> PassFn pick_pass_lat(int aniso)
     }
 }
 
+template <int MODE, int COL> PassFn pick_pass_fcc_c(int aniso)
+{
+    switch (aniso) {
+        case 0: return pass_kernel<4, 0, false, MODE, 2, COL>;  case 1: return pass_kernel<4, 1, false, MODE, 2, COL>;
+        case 2: return pass_kernel<4, 2, false, MODE, 2, COL>;  default: return pass_kernel<4, 3, false, MODE, 2, COL>;
+    }
+}
+template <int MODE> PassFn pick_pass_fcc(int aniso, int colour)
+{
+    switch (colour) {
+        case 0: return pick_pass_fcc_c<MODE, 0>(aniso);  case 1: return pick_pass_fcc_c<MODE, 1>(aniso);
+        case 2: return pick_pass_fcc_c<MODE, 2>(aniso);  default: return pick_pass_fcc_c<MODE, 3>(aniso);
+    }
+}
+
 }  // namespace
 
 int launch_pass_generic(mc_ctx* ctx, int mode, int colour, float invT, int flags, float* dx, uint8_t* da)
@@ -32,7 +47,7 @@ int launch_pass_generic(mc_ctx* ctx, int mode, int colour, float invT, int flags
     PassFn fn = (ctx->vec == 4) ? (mode == MODE_SWEEP ? pick_pass<4, MODE_SWEEP>(ctx->aniso, ctx->masked) : pick_pass<4, MODE_MEASURE>(ctx->aniso, ctx->masked))
                                 : (mode == MODE_SWEEP ? pick_pass<1, MODE_SWEEP>(ctx->aniso, ctx->masked) : pick_pass<1, MODE_MEASURE>(ctx->aniso, ctx->masked));
     if (ctx->P.bcc) fn = mode == MODE_SWEEP ? pick_pass_lat<MODE_SWEEP, 1>(ctx->aniso) : pick_pass_lat<MODE_MEASURE, 1>(ctx->aniso);
-    if (ctx->P.fcc) fn = mode == MODE_SWEEP ? pick_pass_lat<MODE_SWEEP, 2>(ctx->aniso) : pick_pass_lat<MODE_MEASURE, 2>(ctx->aniso);
+    if (ctx->P.fcc) fn = mode == MODE_SWEEP ? pick_pass_fcc<MODE_SWEEP>(ctx->aniso, colour) : pick_pass_fcc<MODE_MEASURE>(ctx->aniso, colour);
     const int grid = grid_for(ctx, ctx->geom.n_items, MC_PASS_MIN_BLOCKS);
     MC_CU(launch_dependent(fn, grid, BLOCK, 0, ctx->stream, ctx->P, ctx->geom, colour, invT, flags, dx, da));
     ctx->launches += 1;

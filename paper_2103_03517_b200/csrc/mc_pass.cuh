@@ -17,11 +17,13 @@ namespace mc {
 #endif
 // LAT: 0 simple cubic; 1 bcc, 2 fcc (mc_common.cuh): VEC = 4 consecutive cells of one sublattice, site stride 1 instead of 2;
 // fcc: four colours, the exchange energy of a bond is summed in the pass of its higher colour (hl).
-template <int VEC, int ANISO, bool MASKED, int MODE, int LAT = 0>
+// COL >= 0: the colour as a compile-time constant (fcc: which rows and shifts a sublattice reads is then resolved by the compiler).
+template <int VEC, int ANISO, bool MASKED, int MODE, int LAT = 0, int COL = -1>
 __global__ void __launch_bounds__(BLOCK, MC_PASS_MIN_BLOCKS)
-pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, int colour, float invT, int flags,
+pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, int colour_rt, float invT, int flags,
             float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
 {
+    const int colour = COL >= 0 ? COL : colour_rt;
     DevState* st = P.st;
     grid_dependency_sync();
     const unsigned long long sweep = st->sweep;
