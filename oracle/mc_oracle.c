@@ -598,8 +598,8 @@ int64_t orc_site_of(const orc_ctx* c, int colour, int64_t a)
  * Replaces the paper's shuffled index array; requirements R1-R4 in DESIGN.md. */
 int orc_pairing(const orc_ctx* c, uint64_t sweep, int colour, int64_t* partner, uint8_t* is_leader)
 {
-    if (c->structure) return -1;                             /* the constrained path is built for the sc lattice only */
-    if (c->nx & 1) return -1;
+    if (c->structure == 2) return -1;                        /* the constrained path sweeps two colours: sc and bcc (not the four of fcc) */
+    if (!c->structure && (c->nx & 1)) return -1;
     int64_t Nc = c->N / 2;
     if (Nc & 1) return -1;                                   /* C-15 */
     int64_t B = 32; while (Nc % (2 * B)) B >>= 1;
@@ -660,7 +660,8 @@ static int pair_update(orc_ctx* c, double T, const double e[3], int colour, int6
                        double* ML, int ml_mode, double* xdec, int may_be_neighbours)
 {
     double u0, u1, u2;                                                    /* P:186, P:193 UniformRandom() x 3 (C-26) */
-    orc_pair_uniforms(c, (int)(si % c->nx), (int)((si / c->nx) % c->ny), (int)(si / ((int64_t)c->nx * c->ny)), colour, c->sweep, &u0, &u1, &u2);
+    const int64_t ci = c->structure ? si % c->Ncell : si;                 /* bcc: the leader's cell (its sublattice is the colour) */
+    orc_pair_uniforms(c, (int)(ci % c->nx), (int)((ci / c->nx) % c->ny), (int)(ci / ((int64_t)c->nx * c->ny)), colour, c->sweep, &u0, &u1, &u2);
     double *Si = &c->S[3 * si], *Sj = &c->S[3 * sj], Sni[3], Snj[3];
     orc_cone_move(Si, c->cone, u0, u1, Sni);
     double Si_par = Si[0] * e[0] + Si[1] * e[1] + Si[2] * e[2];
@@ -683,11 +684,9 @@ static int pair_update(orc_ctx* c, double T, const double e[3], int colour, int6
         for (int a = 0; a < 3; ++a) Snj[a] *= inv;
         MLhat = *ML + Sni_par + Snj_par - Si_par - Sj_par;                /* P:190 */
         if (MLhat > 0.0) {                                                /* C-13 */
-            int xi = (int)(si % c->nx), yi = (int)((si / c->nx) % c->ny), zi = (int)(si / ((int64_t)c->nx * c->ny));
-            int xj = (int)(sj % c->nx), yj = (int)((sj / c->nx) % c->ny), zj = (int)(sj / ((int64_t)c->nx * c->ny));
             double hi[3], hj[3];
-            exchange_field(c, xi, yi, zi, hi);
-            exchange_field(c, xj, yj, zj, hj);
+            field_at(c, si, hi);
+            field_at(c, sj, hj);
             double dE = site_energy_h(c, si, hi, Sni) + site_energy_h(c, sj, hj, Snj)
                       - site_energy_h(c, si, hi, Si) - site_energy_h(c, sj, hj, Sj);   /* P:193 (C-4) */
             if (may_be_neighbours) {
@@ -696,7 +695,7 @@ static int pair_update(orc_ctx* c, double T, const double e[3], int colour, int6
                 double keep[3] = { Si[0], Si[1], Si[2] };
                 double dEi = site_energy_h(c, si, hi, Sni) - site_energy_h(c, si, hi, Si);
                 Si[0] = Sni[0]; Si[1] = Sni[1]; Si[2] = Sni[2];
-                exchange_field(c, xj, yj, zj, hj);
+                field_at(c, sj, hj);
                 dE = dEi + site_energy_h(c, sj, hj, Snj) - site_energy_h(c, sj, hj, Sj);
                 Si[0] = keep[0]; Si[1] = keep[1]; Si[2] = keep[2];
             }
@@ -778,7 +777,10 @@ int orc_constrained_sweep(orc_ctx* c, double T, double theta, double phi, int64_
         double ML = 0.0;                                                  /* P:201 */
         for (int64_t i = 0; i < c->N; ++i) ML += c->S[3 * i] * e[0] + c->S[3 * i + 1] * e[1] + c->S[3 * i + 2] * e[2];
         if (!(ML > 0.0)) { c->torque_sampling = 0; return -1; }
-        if (pairing_mode == 2) { orc_end_sweep(c, serial_any_pair_sweep(c, T, e, &ML)); continue; }
+        if (pairing_mode == 2) {
+            if (c->structure) return -1;                                      /* the serial cross-check mode is written for the sc lattice */
+            orc_end_sweep(c, serial_any_pair_sweep(c, T, e, &ML)); continue;
+        }
         int64_t count = orc_constrained_half_sweep(c, T, e, 0, &ML, ml_mode, pairing_mode, NULL, NULL);   /* P:203 */
         int64_t cb    = orc_constrained_half_sweep(c, T, e, 1, &ML, ml_mode, pairing_mode, NULL, NULL);   /* P:204 (C-5) */
         if (count < 0 || cb < 0) { c->torque_sampling = 0; return -1; }

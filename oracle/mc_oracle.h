@@ -59,7 +59,8 @@ orc_ctx* orc_create(int nx, int ny, int nz, const int periodic[3],
                     double cone0_rad, int adaptive, uint64_t seed);
 /* Body-centred cubic lattice (two simple cubic sublattices = the two colours; reading C-30 in DESIGN.md): nx x ny x nz
  * conventional cells, 2 nx ny nz spins, 8 nearest neighbours, site = sublattice*nx*ny*nz + (i + nx*(j + ny*k)).
- * periodic[a] in {0,1}; no mask / regions; the constrained calls return an error in this mode. */
+ * periodic[a] in {0,1}; no mask / regions.  The constrained calls work as on the sc lattice (two colours, the pairing acts on the
+ * cell order of a sublattice; pairing_mode 2 is sc only). */
 orc_ctx* orc_create_bcc(int nx, int ny, int nz, const int periodic[3],
                         double J, double Ku, const double eu[3], double Kc, const double B[3],
                         double cone0_rad, int adaptive, uint64_t seed);

@@ -89,8 +89,6 @@ def test_ground_state_and_sublattice_colours():
     n1 = o.half_sweep(1.0, 1); S2 = o.get_spins()
     assert n1 > 0 and (S2[:64] == S1[:64]).all() and (S2[64:] != S1[64:]).any()
     assert abs(np.linalg.norm(S2, axis=1) - 1).max() < 1e-12
-    with pytest.raises(ValueError):
-        o.constrained_sweep(1.0, 0.3, 0.0, 1)                    # the constrained path is sc only
 
 
 def test_uniforms_pair_the_x_neighbours_of_a_sublattice():
@@ -154,3 +152,56 @@ def test_curie_temperature_of_the_bcc_heisenberg_model():
     assert U[(5, Ts[2])][0] - U[(8, Ts[2])][0] > 3 * err(Ts[2])
     assert abs(U[(8, Ts[1])][0] - U[(5, Ts[1])][0]) < 3 * err(Ts[1]) + 0.008
     assert abs(U[(8, Ts[1])][0] - 0.62) < 0.03
+
+
+# ------------------------------------------------------------------------------ constrained MC (Table A2) on the bcc lattice
+def test_constrained_pairing_on_a_sublattice():
+    """The analytic pairing (C-11) acts on the cell order of a sublattice: a perfect matching inside the colour, roles
+    randomised, partner varying; colour-linear index a <-> site = sublattice*Ncell + a."""
+    o = oracle.Oracle(8, 4, 4, structure="bcc")
+    Nc = o.N // 2
+    lead_count = np.zeros(Nc); seen = [set() for _ in range(8)]
+    for colour in (0, 1):
+        assert [o.site_of(colour, a) for a in (0, 5, Nc - 1)] == [colour * Nc, colour * Nc + 5, colour * Nc + Nc - 1]
+        for s in range(200):
+            partner, lead = o.pairing(s, colour)
+            a = np.arange(Nc)
+            assert (partner[partner] == a).all() and (partner != a).all()
+            assert lead.sum() == Nc // 2 and (lead[partner] == 1 - lead).all()
+            lead_count += lead
+            for i in range(8): seen[i].add(int(partner[i]))
+    assert np.all(np.abs(lead_count / 400 - 0.5) < 5 * np.sqrt(0.25 / 400)) and min(len(x) for x in seen) > 3
+    with pytest.raises(ValueError):
+        oracle.Oracle(3, 3, 3, structure="bcc").pairing(0, 0)     # odd colour population (C-15)
+    with pytest.raises(ValueError):
+        oracle.Oracle(4, 4, 4, structure="fcc").constrained_sweep(1.0, 0.3, 0.0, 1)   # four colours: not a two-pass constrained sweep
+
+
+def _ctrace(shape, T, theta, n_eq, n_s, seed, **kw):
+    o = oracle.Oracle(*shape, structure="bcc", seed=seed, **kw)
+    o.set_sampling(False); o.constrained_sweep(T, theta, 0.0, n_eq); o.set_sampling(True); o.constrained_sweep(T, theta, 0.0, n_s)
+    return o.trace(), o.observables(), o.get_spins()
+
+
+def test_constrained_direction_is_held_and_isotropic_ensemble_is_unchanged():
+    """P-16 / P-17 on bcc: M/|M| = e_C to 1e-12 and the transverse sum conserved; with an isotropic Hamiltonian the constrained
+    chain samples the unconstrained distribution of |M| and E (8^3 cells = 1024 spins, T = 1.5; the stale-M_L bias is O(1/N))."""
+    th = 0.9; e = np.array([np.sin(th), 0.0, np.cos(th)])
+    fc = _POOL.submit(_ctrace, (8, 8, 8), 1.5, th, 400, 3000, 5, cone0=1.0)
+    fu = _POOL.submit(_trace, (8, 8, 8), 1.5, 400, 3000, 6, cone0=1.0)
+    trc, ob, S = fc.result(); tru = fu.result()
+    M = S.sum(axis=0)
+    assert np.abs(M / np.linalg.norm(M) - e).max() < 1e-12
+    assert np.abs(M - (M @ e) * e).max() < 1e-9
+    for f in (lambda t: np.linalg.norm(t[:, 2:5], axis=1), lambda t: t[:, 5]):
+        a, sa = blocked_mean_se(f(trc)); b, sb = blocked_mean_se(f(tru))
+        assert abs(a - b) < 3 * np.hypot(sa, sb) + 1.5e-3
+
+
+def test_constrained_torque_gives_the_anisotropy_constant():
+    """P-18 on bcc: restoring torque per spin = K(T) sin 2 theta, K(T -> 0) = K_u (Table A2 with the bcc field)."""
+    th = np.pi / 4
+    tr, ob, _ = _ctrace((6, 6, 6), 0.01, th, 300, 600, 8, Ku=0.05, cone0=0.2)
+    K = -(ob.sum_torque[1] / ob.n_samples) / np.sin(2 * th)
+    m = np.linalg.norm(tr[:, 2:5], axis=1).mean()
+    assert abs(K / (0.05 * m ** 3) - 1) < 0.02 and abs(K / 0.05 - 1) < 0.02
