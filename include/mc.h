@@ -57,11 +57,12 @@ typedef struct {
  * B (colour 1) at the cell centres; site = sublattice*nx*ny*nz + (i + nx*(j + ny*k)); the 8 nearest neighbours of a site
  * are in the other sublattice: A(i,j,k) -- B(i-dx,j-dy,k-dz), B(i,j,k) -- A(i+dx,j+dy,k+dz), dx,dy,dz in {0,1}.  The two
  * sublattices are the two colours of the checkerboard scheme.  On the device: every dimension periodic, nx a multiple of 4,
- * no bond mask / regions, unconstrained sweeps only (mc_constrained_sweep, mc_profile_x: MC_EINVAL).
+ * no bond mask / regions; mc_profile_x: MC_EINVAL.  The constrained calls work as on the sc lattice (the pairing of C-11 acts
+ * on the cell order of a sublattice) when nx*ny*nz is a multiple of 8, else MC_EINVAL.
  * MC_FCC ("4 simple cubic sub-lattices for fcc"; reading C-31): N = 4*nx*ny*nz spins; sublattice 0 at the cell corners,
  * 1, 2, 3 at (0,1/2,1/2), (1/2,0,1/2), (1/2,1/2,0) from them; site = sublattice*nx*ny*nz + cell; 12 nearest neighbours, 4 in each
  * OTHER sublattice, so the four sublattices are FOUR colours: a Monte Carlo iteration is four colour passes (mc_half_sweep takes
- * colour 0..3).  Same restrictions as MC_BCC. */
+ * colour 0..3).  Same restrictions as MC_BCC; unconstrained sweeps only (the constrained calls: MC_EINVAL). */
 
 /* Spin Hamiltonian, Eq. (2):  E_i = -sum_j J_ij S_i.S_j - Ku (S_i.e_i)^2 + Kc (Sx^2Sy^2 + Sx^2Sz^2 + Sy^2Sz^2) - S_i.B */
 typedef struct {

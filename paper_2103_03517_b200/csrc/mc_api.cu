@@ -236,12 +236,12 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     { uint32_t sh = 0; while (sh < 5 && ny % (2 << sh) == 0) ++sh; ctx->geom.yb_shift = sh; }      // up to 32 rows per block
 
     // pairing geometry (C-11); the constrained path needs an even colour population (C-15)
-    ctx->pair_ok = (Nc % 2 == 0) && Nc >= 2 && !bcc && !fcc;  // the constrained path is built for the sc lattice
+    ctx->pair_ok = (Nc % 2 == 0) && Nc >= 2 && !fcc;           // two-colour lattices (sc, bcc); fcc has four passes per sweep
     if (ctx->pair_ok) {
         PairGeom& G = ctx->pgeom;
         uint32_t Bc = 32; while (Nc % (2 * Bc)) Bc >>= 1;
         G.B = Bc; G.H = Nc / Bc; G.Bl = Bc < 4 ? Bc : 4; G.Bh = Bc / G.Bl;
-        if (ctx->vec == 4 && Bc < 4) ctx->pair_ok = false;      // cannot happen: nx % 8 == 0 implies 8 | Nc
+        if (ctx->vec == 4 && Bc < 4) ctx->pair_ok = false;      // sc: cannot happen (nx % 8 == 0 implies 8 | Nc); bcc: needs 8 | cells
         G.groups_per_chunk_vec = Bc / ctx->vec;
         G.n_threads = Nc / (2 * ctx->vec);
         G.div_r = make_div(R); G.div_ny = make_div((uint32_t)ny);
@@ -499,7 +499,7 @@ int mc_constrained_sweep(mc_ctx* ctx, double T, double theta, double phi, int64_
 {
     CHECK_CTX();
     if (!(T > 0.0) || n < 0) return fail(ctx, MC_EINVAL, "mc_constrained_sweep: need T > 0 and n >= 0");
-    if (!ctx->pair_ok) return fail(ctx, MC_EINVAL, "mc_constrained_sweep: needs a simple cubic lattice with an even number of sites per colour (C-15)");
+    if (!ctx->pair_ok) return fail(ctx, MC_EINVAL, "mc_constrained_sweep: needs a two-colour lattice (sc, bcc) with an even number of sites per colour (C-15; bcc: cells a multiple of 8)");
     int rc;
     if (!ctx->aligned || theta != ctx->theta || phi != ctx->phi) { if ((rc = mc_align_to(ctx, theta, phi))) return rc; }
     if (n == 0) return MC_OK;
@@ -560,7 +560,7 @@ int mc_constrained_half_sweep(mc_ctx* ctx, double T, double theta, double phi, i
 {
     CHECK_CTX();
     if (!(T > 0.0) || (colour != 0 && colour != 1) || !(M_L > 0.0)) return fail(ctx, MC_EINVAL, "mc_constrained_half_sweep: bad argument");
-    if (!ctx->pair_ok) return fail(ctx, MC_EINVAL, "mc_constrained_half_sweep: odd number of sites per colour (C-15)");
+    if (!ctx->pair_ok) return fail(ctx, MC_EINVAL, "mc_constrained_half_sweep: needs a two-colour lattice with an even number of sites per colour (C-15; bcc: cells a multiple of 8)");
     double e[3]; direction(theta, phi, e);
     int rc;
     if ((rc = launch_state(ctx, ST_EC, e[0], e[1], e[2]))) return rc;

@@ -16,11 +16,19 @@ template <int VEC> PairFn pick_pair(int aniso, bool masked)
     }
 }
 
+PairFn pick_pair_bcc(int aniso)
+{
+    switch (aniso) {
+        case 0: return pair_kernel<4, 0, false, 1>;  case 1: return pair_kernel<4, 1, false, 1>;
+        case 2: return pair_kernel<4, 2, false, 1>;  default: return pair_kernel<4, 3, false, 1>;
+    }
+}
+
 }  // namespace
 
 int launch_pair_generic(mc_ctx* ctx, int colour, float invT, int flags, float* dx, uint8_t* da)
 {
-    PairFn fn = (ctx->vec == 4) ? pick_pair<4>(ctx->aniso, ctx->masked) : pick_pair<1>(ctx->aniso, ctx->masked);
+    PairFn fn = ctx->P.bcc ? pick_pair_bcc(ctx->aniso) : (ctx->vec == 4) ? pick_pair<4>(ctx->aniso, ctx->masked) : pick_pair<1>(ctx->aniso, ctx->masked);
     const int grid = grid_for(ctx, ctx->pgeom.n_threads, MC_PAIR_MIN_BLOCKS);
     MC_CU(launch_dependent(fn, grid, BLOCK, 0, ctx->stream, ctx->P, ctx->pgeom, colour, invT, flags, dx, da));
     ctx->launches += 1;

@@ -46,10 +46,28 @@ __device__ __forceinline__ ItemPos locate_linear(const Params& P, const PairGeom
     return q;
 }
 
+// bcc (C-30): the colour-linear index IS the cell index of the sublattice; rows and the cell outside the item as in bcc_locate
+__device__ __forceinline__ BccPos bcc_locate_linear(const Params& P, const PairGeom& G, uint32_t a0, int colour)
+{
+    uint32_t row, i0, y, z;
+    G.div_r.divmod(a0, row, i0);
+    G.div_ny.divmod(row, z, y);
+    const uint32_t nx = (uint32_t)P.nx, ny = (uint32_t)P.ny, nz = (uint32_t)P.nz;
+    BccPos q;
+    q.i0 = i0; q.a0 = a0; q.site0 = (uint32_t)colour * P.Nc + a0;
+    const uint32_t y2 = colour ? (y + 1 == ny ? 0u : y + 1) : (y == 0 ? ny - 1 : y - 1);
+    const uint32_t z2 = colour ? (z + 1 == nz ? 0u : z + 1) : (z == 0 ? nz - 1 : z - 1);
+    q.row[0] = (z * ny + y) * nx;  q.row[1] = (z * ny + y2) * nx;
+    q.row[2] = (z2 * ny + y) * nx; q.row[3] = (z2 * ny + y2) * nx;
+    q.xe = colour ? (i0 + 4 == nx ? 0u : i0 + 4) : (i0 == 0 ? nx - 1 : i0 - 1);
+    return q;
+}
+
 #ifndef MC_PAIR_MIN_BLOCKS
 #define MC_PAIR_MIN_BLOCKS 2      // <= 128 registers: two CTAs per SM
 #endif
-template <int VEC, int ANISO, bool MASKED>
+// LAT: 0 simple cubic; 1 bcc (VEC = 4 consecutive cells of one sublattice, site-id stride 1, the 8-bond field).
+template <int VEC, int ANISO, bool MASKED, int LAT = 0>
 __global__ void __launch_bounds__(BLOCK, MC_PAIR_MIN_BLOCKS)
 pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G, int colour, float invT, int flags,
             float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
@@ -97,12 +115,25 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
             uint32_t lf = lo + rot; if (lf >= G.Bl) lf -= G.Bl;
             aL = chunkL * G.B + g; aF = chunkF * G.B + hf * G.Bl + lf;
         }
-        const ItemPos qL = locate_linear<VEC>(P, G, aL, colour), qF = locate_linear<VEC>(P, G, aF, colour);
+        static_assert(!LAT || (VEC == 4 && !MASKED), "the bcc pair pass is the VEC = 4, unmasked instantiation");
+        constexpr uint32_t SS = LAT ? 1u : 2u;                     // site-id stride between the sites of an item
+        ItemPos qL, qF;
+        Vec3 hL[VEC], hF[VEC], eL[VEC], eF[VEC];
+        if (LAT == 1) {
+            const BccPos bL = bcc_locate_linear(P, G, aL, colour), bF = bcc_locate_linear(P, G, aF, colour);
+            qL.a0 = aL; qL.site0 = bL.site0; qL.xh0 = bL.i0; qL.par = 0u;
+            qF.a0 = aF; qF.site0 = bF.site0; qF.xh0 = bF.i0; qF.par = 0u;
+            if (VEC == 4) {
+                bcc_exchange_field(P, bL, colour, reinterpret_cast<Vec3(&)[4]>(hL));
+                bcc_exchange_field(P, bF, colour, reinterpret_cast<Vec3(&)[4]>(hF));
+            }
+        } else {
+            qL = locate_linear<VEC>(P, G, aL, colour); qF = locate_linear<VEC>(P, G, aF, colour);
+            exchange_field<VEC, MASKED>(P, qL, colour, hL);
+            exchange_field<VEC, MASKED>(P, qF, colour, hF);
+        }
         const Pack<VEC> lx = ld_rw<VEC>(Sc + aL), ly = ld_rw<VEC>(Sc + P.plane + aL), lz = ld_rw<VEC>(Sc + 2 * P.plane + aL);
         const Pack<VEC> fx = ld_rw<VEC>(Sc + aF), fy = ld_rw<VEC>(Sc + P.plane + aF), fz = ld_rw<VEC>(Sc + 2 * P.plane + aF);
-        Vec3 hL[VEC], hF[VEC], eL[VEC], eF[VEC];
-        exchange_field<VEC, MASKED>(P, qL, colour, hL);
-        exchange_field<VEC, MASKED>(P, qF, colour, hF);
         if (ANISO & 1) { easy_axes<VEC>(P, qL, colour, eL); easy_axes<VEC>(P, qF, colour, eF); }
         Pack<VEC> nlx = lx, nly = ly, nlz = lz, nfx = fx, nfy = fy, nfz = fz;
         if (VEC == 4) {
@@ -142,8 +173,8 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
                     }
                     ej = pack3(e0, e1);
                 }
-                const uint32_t site_i0 = qL.site0 + 2u * kp, site_i1 = site_i0 + 2u;
-                // one Philox block per two pairs: the leaders site_i0 (bit 1 of x clear) and site_i0 + 2 take words (0,1) and (2,3) (C-26)
+                const uint32_t site_i0 = qL.site0 + SS * kp, site_i1 = site_i0 + SS;
+                // one Philox block per two pairs: the leaders site_i0 (bit 1 of x clear; bcc: even cell) and its same-colour x-neighbour take words (0,1) and (2,3) (C-26, C-30)
                 uint32_t a0, a1, b0, b1;
                 philox4x32_10(key, site_i0, c1, c2, c3, a0, a1, b0, b1);
                 V3p di, Sni;
@@ -190,7 +221,7 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
                 sF[kf0][tx] = Snj.x.x; sF[4 + kf0][tx] = Snj.y.x; sF[8 + kf0][tx] = Snj.z.x;
                 sF[kf1][tx] = Snj.x.y; sF[4 + kf1][tx] = Snj.y.y; sF[8 + kf1][tx] = Snj.z.y;
                 cnt += (ok0 ? 2 : 0) + (ok1 ? 2 : 0);                                               // P:195 (C-23)
-                const uint32_t site_j0 = qF.site0 + 2u * kf0, site_j1 = qF.site0 + 2u * kf1;
+                const uint32_t site_j0 = qF.site0 + SS * kf0, site_j1 = qF.site0 + SS * kf1;
                 if (dbg_x)   { dbg_x[site_i0] = x0; dbg_x[site_i1] = x1; }
                 if (dbg_acc) { dbg_acc[site_i0] = (uint8_t)ok0; dbg_acc[site_j0] = (uint8_t)ok0; dbg_acc[site_i1] = (uint8_t)ok1; dbg_acc[site_j1] = (uint8_t)ok1; }
                 // fused sums of the final spins of both members
