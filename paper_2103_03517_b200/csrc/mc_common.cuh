@@ -384,10 +384,11 @@ __device__ __forceinline__ void fx_flush(long long (&acc)[NQ], float (&f)[NQ], f
     for (int q = 0; q < NQ; ++q) { acc[q] += __float2ll_rn(f[q] * scale); f[q] = 0.0f; }
 }
 
-// The generic kernels keep the fixed-point sums of a thread in shared memory (column threadIdx.x of [NQ][BLOCK]: no bank
+// The generic kernels keep the fixed-point sums of a thread in shared memory (column threadIdx.x of [NQ][threads per CTA]: no bank
 // conflicts) instead of 18 registers: they are short of registers (spills), and the sums are touched once per
 // FLUSH_ITEMS items.
-__device__ __forceinline__ void fx_flush_shared(long long (*sacc)[BLOCK], float (&f)[NQ], float scale)
+template <int W>
+__device__ __forceinline__ void fx_flush_shared(long long (*sacc)[W], float (&f)[NQ], float scale)
 {
 #pragma unroll
     for (int q = 0; q < NQ; ++q) { sacc[q][threadIdx.x] += __float2ll_rn(f[q] * scale); f[q] = 0.0f; }

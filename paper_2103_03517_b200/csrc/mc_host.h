@@ -64,9 +64,9 @@ cudaError_t launch_dependent(Fn fn, int grid, int block, size_t smem, cudaStream
 }
 
 // grid of a grid-stride kernel: one resident wave (the CTAs per SM its launch bounds allow)
-inline int grid_for(const mc_ctx* c, uint32_t n_threads_needed, int resident_per_sm)
+inline int grid_for(const mc_ctx* c, uint32_t n_threads_needed, int resident_per_sm, int block = BLOCK)
 {
-    const long long need = ((long long)n_threads_needed + BLOCK - 1) / BLOCK;
+    const long long need = ((long long)n_threads_needed + block - 1) / block;
     long long cap = (long long)c->sm_count * resident_per_sm;
     if (cap > c->P.max_blocks) cap = c->P.max_blocks;
     long long g = need < cap ? need : cap;

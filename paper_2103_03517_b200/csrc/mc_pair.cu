@@ -29,8 +29,8 @@ PairFn pick_pair_bcc(int aniso)
 int launch_pair_generic(mc_ctx* ctx, int colour, float invT, int flags, float* dx, uint8_t* da)
 {
     PairFn fn = ctx->P.bcc ? pick_pair_bcc(ctx->aniso) : (ctx->vec == 4) ? pick_pair<4>(ctx->aniso, ctx->masked) : pick_pair<1>(ctx->aniso, ctx->masked);
-    const int grid = grid_for(ctx, ctx->pgeom.n_threads, MC_PAIR_MIN_BLOCKS);
-    MC_CU(launch_dependent(fn, grid, BLOCK, 0, ctx->stream, ctx->P, ctx->pgeom, colour, invT, flags, dx, da));
+    const int grid = grid_for(ctx, ctx->pgeom.n_threads, MC_PAIR_MIN_BLOCKS, MC_PAIR_BLOCK);
+    MC_CU(launch_dependent(fn, grid, MC_PAIR_BLOCK, 0, ctx->stream, ctx->P, ctx->pgeom, colour, invT, flags, dx, da));
     ctx->launches += 1;
     return MC_OK;
 }

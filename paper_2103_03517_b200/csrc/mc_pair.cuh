@@ -63,12 +63,19 @@ __device__ __forceinline__ BccPos bcc_locate_linear(const Params& P, const PairG
     return q;
 }
 
+template <int V> struct IntC { static constexpr int value = V; };
+
+// 128 threads x 4 CTAs per SM (<= 128 registers).  Measured at 224^3, us per constrained sweep: 256 x 2 114.1, 192 x 2 (166
+// registers) 115.9, 128 x 3 (166 registers) 112.3, 128 x 4 110.4, 96 x 5 115.9, 64 x 8 118.5
+#ifndef MC_PAIR_BLOCK
+#define MC_PAIR_BLOCK 128
+#endif
 #ifndef MC_PAIR_MIN_BLOCKS
-#define MC_PAIR_MIN_BLOCKS 2      // <= 128 registers: two CTAs per SM
+#define MC_PAIR_MIN_BLOCKS 4
 #endif
 // LAT: 0 simple cubic; 1 bcc (VEC = 4 consecutive cells of one sublattice, site-id stride 1, the 8-bond field).
 template <int VEC, int ANISO, bool MASKED, int LAT = 0>
-__global__ void __launch_bounds__(BLOCK, MC_PAIR_MIN_BLOCKS)
+__global__ void __launch_bounds__(MC_PAIR_BLOCK, MC_PAIR_MIN_BLOCKS)
 pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G, int colour, float invT, int flags,
             float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
 {
@@ -90,17 +97,18 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
     float* Sc = P.S + (long long)colour * 3 * P.plane;
     const Vec3 B = { P.B[0], P.B[1], P.B[2] };
 
-    __shared__ long long sacc[NQ][BLOCK];   // exact fixed-point sums of every thread of the block (fx_flush_shared)
-    // VEC = 4: the follower group's spins (rows 0..11 = component * 4 + element) and exchange field (rows 12..23) of every
-    // thread live in shared memory: the leader's element k pairs with element (k + rot) & 3 of the follower group, which is
-    // then one indexed shared-memory access instead of a chain of register selects, and 24 registers less (the kernel spills)
-    __shared__ float sF[VEC == 4 ? 24 : 1][BLOCK];
+    __shared__ long long sacc[NQ][MC_PAIR_BLOCK];   // exact fixed-point sums of every thread of the block (fx_flush_shared)
 #pragma unroll
     for (int q = 0; q < NQ; ++q) sacc[q][threadIdx.x] = 0;
     int cnt = 0;
 
-    const uint32_t stride = gridDim.x * BLOCK;
-    for (uint32_t t = blockIdx.x * BLOCK + threadIdx.x; t < G.n_threads; t += stride) {
+    // VEC = 4: the leader's element k pairs with element (k + rot) & 3 of the follower group.  rot is the same for every thread of
+    // the launch, so the loop is instantiated for its four values and entered through one uniform switch: the pairing inside a
+    // group is then register naming (no select chains, no staging of the follower group in shared memory).
+    const uint32_t stride = gridDim.x * MC_PAIR_BLOCK;
+    auto run = [&](auto rot_c) {
+    constexpr uint32_t ROT = (uint32_t)decltype(rot_c)::value;
+    for (uint32_t t = blockIdx.x * MC_PAIR_BLOCK + threadIdx.x; t < G.n_threads; t += stride) {
         // leader group
         const uint32_t j = t / G.groups_per_chunk_vec, g = t % G.groups_per_chunk_vec;
         const uint32_t chunkL = 2u * j + sigma;
@@ -136,13 +144,6 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
         const Pack<VEC> fx = ld_rw<VEC>(Sc + aF), fy = ld_rw<VEC>(Sc + P.plane + aF), fz = ld_rw<VEC>(Sc + 2 * P.plane + aF);
         if (ANISO & 1) { easy_axes<VEC>(P, qL, colour, eL); easy_axes<VEC>(P, qF, colour, eF); }
         Pack<VEC> nlx = lx, nly = ly, nlz = lz, nfx = fx, nfy = fy, nfz = fz;
-        if (VEC == 4) {
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                sF[e][threadIdx.x] = fx.v[e]; sF[4 + e][threadIdx.x] = fy.v[e]; sF[8 + e][threadIdx.x] = fz.v[e];
-                sF[12 + e][threadIdx.x] = hF[e].x; sF[16 + e][threadIdx.x] = hF[e].y; sF[20 + e][threadIdx.x] = hF[e].z;
-            }
-        }
         float f[NQ];
 #pragma unroll
         for (int k = 0; k < NQ; ++k) f[k] = 0.0f;
@@ -155,24 +156,13 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
             for (int q = 0; q < NQ; ++q) f2s[q] = splat(0.0f);
 #pragma unroll
             for (int kp = 0; kp < 4; kp += 2) {
-                const uint32_t kf0 = (kp + rot) & 3u, kf1 = (kp + 1 + rot) & 3u;
-                const uint32_t tx = threadIdx.x;
+                const int kf0 = (kp + ROT) & 3, kf1 = (kp + 1 + ROT) & 3;               // compile-time after unrolling
                 V3p Si = { make_float2(lx.v[kp], lx.v[kp + 1]), make_float2(ly.v[kp], ly.v[kp + 1]), make_float2(lz.v[kp], lz.v[kp + 1]) };
-                const V3p Sj = { make_float2(sF[kf0][tx], sF[kf1][tx]), make_float2(sF[4 + kf0][tx], sF[4 + kf1][tx]), make_float2(sF[8 + kf0][tx], sF[8 + kf1][tx]) };
-                const V3p hj = { make_float2(sF[12 + kf0][tx], sF[12 + kf1][tx]), make_float2(sF[16 + kf0][tx], sF[16 + kf1][tx]), make_float2(sF[20 + kf0][tx], sF[20 + kf1][tx]) };
+                const V3p Sj = { make_float2(fx.v[kf0 % VEC], fx.v[kf1 % VEC]), make_float2(fy.v[kf0 % VEC], fy.v[kf1 % VEC]), make_float2(fz.v[kf0 % VEC], fz.v[kf1 % VEC]) };
+                const V3p hj = pack3(hF[kf0 % VEC], hF[kf1 % VEC]);
                 const V3p hi = pack3(hL[kp], hL[kp + 1]);
                 V3p ei = eC2, ej = eC2;                      // placeholders when ANISO & 1 == 0
-                if (ANISO & 1) {
-                    ei = pack3(eL[kp], eL[kp + 1]);
-                    Vec3 e0 = eF[0], e1 = eF[0];
-#pragma unroll
-                    for (int s2 = 1; s2 < 4; ++s2) {
-                        const bool p0 = kf0 == (uint32_t)s2, p1 = kf1 == (uint32_t)s2;
-                        e0.x = p0 ? eF[s2].x : e0.x; e0.y = p0 ? eF[s2].y : e0.y; e0.z = p0 ? eF[s2].z : e0.z;
-                        e1.x = p1 ? eF[s2].x : e1.x; e1.y = p1 ? eF[s2].y : e1.y; e1.z = p1 ? eF[s2].z : e1.z;
-                    }
-                    ej = pack3(e0, e1);
-                }
+                if (ANISO & 1) { ei = pack3(eL[kp], eL[kp + 1]); ej = pack3(eF[kf0 % VEC], eF[kf1 % VEC]); }
                 const uint32_t site_i0 = qL.site0 + SS * kp, site_i1 = site_i0 + SS;
                 // one Philox block per two pairs: the leaders site_i0 (bit 1 of x clear; bcc: even cell) and its same-colour x-neighbour take words (0,1) and (2,3) (C-26, C-30)
                 uint32_t a0, a1, b0, b1;
@@ -218,8 +208,8 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
                                   make_float2(ok0 ? Snj_new.y.x : Sj.y.x, ok1 ? Snj_new.y.y : Sj.y.y),
                                   make_float2(ok0 ? Snj_new.z.x : Sj.z.x, ok1 ? Snj_new.z.y : Sj.z.y) };
                 nlx.v[kp] = Si.x.x; nlx.v[kp + 1] = Si.x.y; nly.v[kp] = Si.y.x; nly.v[kp + 1] = Si.y.y; nlz.v[kp] = Si.z.x; nlz.v[kp + 1] = Si.z.y;
-                sF[kf0][tx] = Snj.x.x; sF[4 + kf0][tx] = Snj.y.x; sF[8 + kf0][tx] = Snj.z.x;
-                sF[kf1][tx] = Snj.x.y; sF[4 + kf1][tx] = Snj.y.y; sF[8 + kf1][tx] = Snj.z.y;
+                nfx.v[kf0 % VEC] = Snj.x.x; nfy.v[kf0 % VEC] = Snj.y.x; nfz.v[kf0 % VEC] = Snj.z.x;
+                nfx.v[kf1 % VEC] = Snj.x.y; nfy.v[kf1 % VEC] = Snj.y.y; nfz.v[kf1 % VEC] = Snj.z.y;
                 cnt += (ok0 ? 2 : 0) + (ok1 ? 2 : 0);                                               // P:195 (C-23)
                 const uint32_t site_j0 = qF.site0 + SS * kf0, site_j1 = qF.site0 + SS * kf1;
                 if (dbg_x)   { dbg_x[site_i0] = x0; dbg_x[site_i1] = x1; }
@@ -240,26 +230,10 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
         }
 #pragma unroll
         for (int k = 0; k < (VEC == 4 ? 0 : VEC); ++k) {
-            // leader element k pairs with follower element kf = (k + rot) mod Bl of the follower group (VEC = 4)
+            // VEC = 1: one pair per thread, the scalar form of the packed arithmetic above (the rotation is in aF)
             Vec3 Si = { lx.v[k], ly.v[k], lz.v[k] };
-            Vec3 Sj, hj, ej; uint32_t site_j;
-            if (VEC == 4) {
-                const uint32_t kf = (k + rot) & 3u;
-                Sj = { sF[kf][threadIdx.x], sF[4 + kf][threadIdx.x], sF[8 + kf][threadIdx.x] };
-                hj = { sF[12 + kf][threadIdx.x], sF[16 + kf][threadIdx.x], sF[20 + kf][threadIdx.x] };
-                Vec3 ee = eF[0];
-                if (ANISO & 1) {
-#pragma unroll
-                    for (int s = 1; s < 4; ++s) {
-                        const bool pick = kf == (uint32_t)s;
-                        ee.x = pick ? eF[s].x : ee.x; ee.y = pick ? eF[s].y : ee.y; ee.z = pick ? eF[s].z : ee.z;
-                    }
-                }
-                ej = ee;
-                site_j = qF.site0 + 2u * ((k + rot) & 3u);
-            } else {
-                Sj = { fx.v[0], fy.v[0], fz.v[0] }; hj = hF[0]; ej = eF[0]; site_j = qF.site0;
-            }
+            const Vec3 Sj = { fx.v[0], fy.v[0], fz.v[0] }, hj = hF[0], ej = eF[0];
+            const uint32_t site_j = qF.site0;
             const uint32_t site_i = qL.site0 + 2u * k;
             uint32_t w0, w1;                                                           // the leader's 64 bits (C-26)
             {
@@ -305,10 +279,7 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
             }
             if (ok) {
                 Si = Sni; nlx.v[k] = Sni.x; nly.v[k] = Sni.y; nlz.v[k] = Sni.z;
-                if (VEC == 4) {
-                    const uint32_t kf = (k + rot) & 3u;
-                    sF[kf][threadIdx.x] = Snj.x; sF[4 + kf][threadIdx.x] = Snj.y; sF[8 + kf][threadIdx.x] = Snj.z;
-                } else { nfx.v[0] = Snj.x; nfy.v[0] = Snj.y; nfz.v[0] = Snj.z; }
+                nfx.v[0] = Snj.x; nfy.v[0] = Snj.y; nfz.v[0] = Snj.z;
             } else {
                 Snj = Sj;
             }
@@ -325,13 +296,18 @@ pair_kernel(const __grid_constant__ Params P, const __grid_constant__ PairGeom G
             const Vec3 tj = onsite_torque<ANISO>(Snj, P.Ku, ej, P.Kc, B);
             f[6] += ti.x + tj.x; f[7] += ti.y + tj.y; f[8] += ti.z + tj.z;
         }
-        if (VEC == 4) {
-#pragma unroll
-            for (int e = 0; e < 4; ++e) { nfx.v[e] = sF[e][threadIdx.x]; nfy.v[e] = sF[4 + e][threadIdx.x]; nfz.v[e] = sF[8 + e][threadIdx.x]; }
-        }
         st_rw<VEC>(Sc + aL, nlx); st_rw<VEC>(Sc + P.plane + aL, nly); st_rw<VEC>(Sc + 2 * P.plane + aL, nlz);
         st_rw<VEC>(Sc + aF, nfx); st_rw<VEC>(Sc + P.plane + aF, nfy); st_rw<VEC>(Sc + 2 * P.plane + aF, nfz);
         fx_flush_shared(sacc, f, P.fx_scale);        // every item (8 updates): this kernel has no registers to spare for running sums
+    }
+    };
+    if (VEC == 4) {
+        switch (rot) {
+            case 0: run(IntC<0>{}); break;  case 1: run(IntC<1>{}); break;
+            case 2: run(IntC<2>{}); break;  default: run(IntC<3>{}); break;
+        }
+    } else {
+        run(IntC<0>{});
     }
     long long acc[NQ];
 #pragma unroll

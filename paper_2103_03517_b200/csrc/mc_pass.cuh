@@ -12,14 +12,19 @@ namespace mc {
 // E_exch is accumulated by the BLACK pass only: every bond joins a red and a black site, so
 // E_exch = -sum_{i black} S_i.h_i with h already in registers (0 extra bytes).
 // --------------------------------------------------------------------------------------------------------------
+// 128 threads x 6 CTAs per SM (<= 80 registers; c5 film with 256-thread CTAs: one per SM 354, two 185, three 166 us per sweep;
+// 128 x 6: 160.6 against 162.3 for 256 x 3)
+#ifndef MC_PASS_BLOCK
+#define MC_PASS_BLOCK 128
+#endif
 #ifndef MC_PASS_MIN_BLOCKS
-#define MC_PASS_MIN_BLOCKS 3      // <= 80 registers: three CTAs per SM (c5 film: one 354, two 185, three 166 us per sweep)
+#define MC_PASS_MIN_BLOCKS 6
 #endif
 // LAT: 0 simple cubic; 1 bcc, 2 fcc (mc_common.cuh): VEC = 4 consecutive cells of one sublattice, site stride 1 instead of 2;
 // fcc: four colours, the exchange energy of a bond is summed in the pass of its higher colour (hl).
 // COL >= 0: the colour as a compile-time constant (fcc: which rows and shifts a sublattice reads is then resolved by the compiler).
 template <int VEC, int ANISO, bool MASKED, int MODE, int LAT = 0, int COL = -1>
-__global__ void __launch_bounds__(BLOCK, MC_PASS_MIN_BLOCKS)
+__global__ void __launch_bounds__(MC_PASS_BLOCK, MC_PASS_MIN_BLOCKS)
 pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, int colour_rt, float invT, int flags,
             float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
 {
@@ -33,14 +38,14 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
     float* Sc = P.S + (long long)colour * 3 * P.plane;
     const Vec3 B = { P.B[0], P.B[1], P.B[2] };
 
-    __shared__ long long sacc[NQ][BLOCK];   // exact fixed-point sums of every thread of the block (fx_flush_shared)
+    __shared__ long long sacc[NQ][MC_PASS_BLOCK];   // exact fixed-point sums of every thread of the block (fx_flush_shared)
     float fs[NQ];                    // fp32 running sums of at most FLUSH_ITEMS items
 #pragma unroll
     for (int q = 0; q < NQ; ++q) { sacc[q][threadIdx.x] = 0; fs[q] = 0.0f; }
     int cnt = 0, pending = 0;
 
-    const uint32_t stride = gridDim.x * BLOCK;
-    for (uint32_t item = blockIdx.x * BLOCK + threadIdx.x; item < G.n_items; item += stride) {
+    const uint32_t stride = gridDim.x * MC_PASS_BLOCK;
+    for (uint32_t item = blockIdx.x * MC_PASS_BLOCK + threadIdx.x; item < G.n_items; item += stride) {
         static_assert(!LAT || (VEC == 4 && !MASKED), "the bcc / fcc passes are VEC = 4, unmasked instantiations");
         constexpr uint32_t SS = LAT ? 1u : 2u;                    // site-id stride between the sites of an item
         ItemPos q;
