@@ -537,7 +537,7 @@ static int hook_common(mc_ctx* ctx, int colour, float* host_x, uint8_t* host_acc
     if (host_acc) { ha.resize(N); CU(cudaMemcpyAsync(ha.data(), da, (size_t)N, cudaMemcpyDeviceToHost, ctx->stream)); }
     CU(cudaStreamSynchronize(ctx->stream));
     const int nx = ctx->P.nx, ny = ctx->P.ny;
-    for (uint32_t s = 0; s < N; ++s) {
+    for (uint32_t s = 0; (host_x || host_acc) && s < N; ++s) {
         const int x = s % nx, y = (s / nx) % ny, z = s / ((uint32_t)nx * ny);
         if (((ctx->P.bcc || ctx->P.fcc) ? (int)(s / ctx->P.Nc) : ((x + y + z) & 1)) != colour) continue;      // bcc / fcc: colour = sublattice
         if (host_x) host_x[s] = hx[s];

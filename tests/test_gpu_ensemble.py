@@ -338,3 +338,75 @@ def test_full_size_march_pass_half_sweep_parity(mods):
     oracle, binding, inputs = mods
     g = binding.Lattice(256, 256, 256, Kc=0.01); assert g.debug_get_path() == binding.MC_PATH_MARCH; g.close()
     _full_size_half_sweep(mods, (256, 256, 256), 1.2, 1.2, 7, dict(Kc=0.01), colour=1)
+
+
+# ---------------------------------------------------------------------------------------------- maximum size
+def test_maximum_size_lattice_sampled_parity_and_path_equality(mods):
+    """The largest lattice the boundary accepts (N < 2^31, include/mc.h): 1280 x 1280 x 1310 = 2 146 304 000 spins, 25.8 GB of state
+    plus the staging area in one 51.5 GB workspace -- a quarter of a B200's HBM (the paper: "100 M spins in 6 GB").
+      * sampled parity: from the +z start, one red and one black pass (march pass); the oracle recomputes SAMPLED sites one by
+        one -- uniforms of the true site index (top of the 32-bit site-id range included), cone move, dE from the site's six
+        neighbours as the GPU left them -- and the GPU's spin must be the oracle's outcome (decisions inside the band skipped);
+      * any-size property: the same two passes through the gather (other index arithmetic, same counters) give the same
+        accepted count (exact), M and E of the trace row to 2e-7 per site, and bit-identical spins on the sampled sites."""
+    import torch
+    oracle, binding, inputs = mods
+    if torch.cuda.mem_get_info()[0] < 60e9:
+        pytest.skip("needs 52 GB of free device memory")
+    shape = (1280, 1280, 1310)
+    nx, ny, nz = shape
+    N = nx * ny * nz
+    assert 2 ** 31 - 2_000_000 < N < 2 ** 31
+    ham = dict(Ku=0.05, eu=(0.3, -0.5, 0.81), Kc=0.01, B=(0.02, 0.0, -0.01))
+    T, cone, sweep0 = 1.0, 0.6, (7 << 32) | 123
+    g = binding.Lattice(*shape, seed=42, cone0=cone, adaptive=False, **ham)
+    assert g.debug_get_path() == binding.MC_PATH_MARCH
+    ob = g.observables()
+    assert abs(ob.E_exch + 3.0) < 1e-6 and abs(ob.m - 1.0) < 1e-6
+    g.set_sweep(sweep0)
+    g.half_sweep(T, 0); g.half_sweep(T, 1); g.end_sweep()
+    S = g.get_spins()
+    row_march = g.trace(1)[0].copy()
+    assert 0.2 < row_march[0] < 0.8
+
+    # sampled sites: the corners of the index range, the planes at the periodic wrap, around site ids 2^30 and N - 1, random ones
+    rng = np.random.default_rng(5)
+    sites = [0, 1, nx - 1, nx, nx * ny - 1, N - 1, N - 2, N - nx, N - nx * ny, 2 ** 30 - 1, 2 ** 30, 2 ** 30 + 1, N // 2, N // 2 + 1]
+    sites += [int(v) for v in rng.integers(0, N, 300)] + [int(v) for v in rng.integers(N - 4 * nx * ny, N, 100)]
+    U = oracle.Oracle(nx, ny, 2, seed=42, cone0=cone, adaptive=False, **ham)          # the uniforms depend on nx, ny and the site index only
+    E = oracle.Oracle(4, 4, 4, seed=42, cone0=cone, adaptive=False, **ham)            # the energy of a site given its six neighbours
+    centre = 1 + 4 * (1 + 4 * 1)
+    nb_small = [2 + 4 * (1 + 4 * 1), 0 + 4 * (1 + 4 * 1), 1 + 4 * (2 + 4 * 1), 1 + 4 * (0 + 4 * 1), 1 + 4 * (1 + 4 * 2), 1 + 4 * (1 + 4 * 0)]
+    zhat = np.array([0.0, 0.0, 1.0])
+    checked = skipped = 0
+    expect = {}
+    for s in sites:
+        x, y, z = s % nx, (s // nx) % ny, s // (nx * ny)
+        colour = (x + y + z) & 1
+        u0, u1, u2 = U.site_uniforms(x, y, z, colour, sweep0)
+        Sn = oracle.cone_move(zhat, cone, u0, u1)
+        nb_big = [((x + 1) % nx) + nx * (y + ny * z), ((x - 1) % nx) + nx * (y + ny * z), x + nx * (((y + 1) % ny) + ny * z),
+                  x + nx * (((y - 1) % ny) + ny * z), x + nx * (y + ny * ((z + 1) % nz)), x + nx * (y + ny * ((z - 1) % nz))]
+        patch = np.tile(zhat, (64, 1))
+        if colour == 1:                                                                # the black pass sees the red sites as the red pass left them
+            for a, b in zip(nb_small, nb_big): patch[a] = S[b].astype(np.float64)
+        E.set_spins(patch)
+        xd = (E.site_energy(centre, Sn) - E.site_energy(centre, zhat)) / T + np.log(u2)
+        if abs(xd) < 1e-5:
+            skipped += 1; continue
+        want = Sn if xd < 0 else zhat
+        assert np.abs(S[s].astype(np.float64) - want).max() < 1e-4, (s, x, y, z, colour, xd)
+        expect[s] = S[s].copy(); checked += 1
+    assert checked > 400 and skipped < 5
+
+    # the same two passes through the gather
+    g.init_spins(0); g.set_sweep(sweep0); g.set_cone(cone); g.debug_set_path(binding.MC_PATH_GENERIC)
+    g.half_sweep(T, 0); g.half_sweep(T, 1); g.end_sweep()
+    row_gen = g.trace(1)[0].copy()
+    # accepted count and cone: exact; M and E: the per-thread fp32 partial sums group the sites differently (2e-7 per site)
+    assert (row_gen[:2] == row_march[:2]).all() and np.abs(row_gen[2:] - row_march[2:]).max() < 2e-7, (row_gen, row_march)
+    S2 = g.get_spins()
+    for s, v in expect.items():
+        assert (S2[s] == v).all()
+    del S, S2
+    g.close()
