@@ -63,6 +63,8 @@ def lib():
     L.orc_create_bcc.restype = vp
     L.orc_create_fcc.argtypes = [i32, i32, i32, vp, dbl, dbl, vp, dbl, vp, dbl, i32, u64]
     L.orc_create_fcc.restype = vp
+    L.orc_create_basis.argtypes = [i32, i32, i32, i32, dbl, dbl, dbl, vp, dbl, vp, dbl, i32, u64]
+    L.orc_create_basis.restype = vp
     L.orc_destroy.argtypes = [vp]; L.orc_destroy.restype = None
     for name in ("orc_set_spins", "orc_set_spins_f32", "orc_get_spins", "orc_init_uniform"):
         getattr(L, name).argtypes = [vp, vp]; getattr(L, name).restype = None
@@ -119,11 +121,11 @@ class Oracle:
     """One lattice + Hamiltonian + RNG seed, state in fp64 (lexicographic [N,3])."""
 
     def __init__(self, nx, ny, nz, periodic=(1, 1, 1), J=1.0, Ku=0.0, eu=(0, 0, 1), Kc=0.0, B=(0, 0, 0),
-                 bond_mask=None, region=None, region_axis=None, cone0=0.5, adaptive=True, seed=42, structure="sc"):
+                 bond_mask=None, region=None, region_axis=None, cone0=0.5, adaptive=True, seed=42, structure="sc", J2=0.0):
         self.L = lib()
         self.shape = (nx, ny, nz)
         self.structure = structure
-        self.N = nx * ny * nz * {"sc": 1, "bcc": 2, "fcc": 4}[structure]
+        self.N = nx * ny * nz * {"sc": 1, "bcc": 2, "fcc": 4, "hcp": 8, "sc_nnn": 8}[structure]
         per = np.asarray(periodic, dtype=np.int32)
         eu_ = np.asarray(eu, dtype=np.float64); B_ = np.asarray(B, dtype=np.float64)
         if structure in ("bcc", "fcc"):   # P:34: sc sublattices = colours; site = sublattice*nx*ny*nz + cell (readings C-30, C-31)
@@ -135,8 +137,17 @@ class Oracle:
             if not self.h:
                 raise ValueError("orc_create_bcc / orc_create_fcc rejected the lattice")
             return
+        if structure in ("hcp", "sc_nnn"):   # eight non-interacting subsets (reading C-32): nx x ny x nz periodic cells of eight sites
+            if bond_mask is not None or region is not None or tuple(int(v) for v in periodic) != (1, 1, 1):
+                raise ValueError("hcp / sc_nnn mode: periodic boxes without bond mask / regions")
+            self._mask = self._region = self._axis = None
+            self.h = self.L.orc_create_basis(3 if structure == "hcp" else 4, nx, ny, nz, J, J2, Ku, _p(eu_), Kc, _p(B_),
+                                             float(cone0), int(bool(adaptive)), int(seed))
+            if not self.h:
+                raise ValueError("orc_create_basis rejected the lattice")
+            return
         if structure != "sc":
-            raise ValueError("structure must be 'sc', 'bcc' or 'fcc'")
+            raise ValueError("structure must be 'sc', 'bcc', 'fcc', 'hcp' or 'sc_nnn'")
         self._mask = None if bond_mask is None else np.ascontiguousarray(bond_mask, dtype=np.uint8).ravel()
         self._region = None if region is None else np.ascontiguousarray(region, dtype=np.uint16).ravel()
         self._axis = None if region_axis is None else np.ascontiguousarray(region_axis, dtype=np.float64)

@@ -26,9 +26,13 @@ static const double PI = 3.14159265358979323846;
 
 struct orc_ctx {
     int nx, ny, nz, periodic[3];
-    int structure;          /* 0 = simple cubic (the paper's lattice); 1 = body-centred cubic, 2 = face-centred cubic, see "bcc / fcc mode" */
+    int structure;          /* 0 = simple cubic (the paper's lattice); 1 = body-centred cubic, 2 = face-centred cubic, see "bcc / fcc mode";
+                               3 = hexagonal close-packed, 4 = simple cubic with next-nearest neighbours: "basis mode" (eight subsets) */
     int n_colours;          /* non-interacting subsets swept one after the other: 2 (sc checkerboard, bcc sublattices), 4 (fcc sublattices)  */
     int64_t Ncell;          /* nx*ny*nz: sc N = Ncell; bcc N = 2 Ncell, fcc N = 4 Ncell (site = sublattice*Ncell + cell)                     */
+    /* basis mode: bonds of a site of sublattice a = the sites at the bonding distances, found from the coordinates at creation */
+    int n_bonds[8];
+    struct { int b, d[3]; double J; } bond[8][24];
     int64_t N;
     double J, Ku, eu[3], Kc, B[3];
     uint8_t* mask;          /* NULL = all bonds allowed by the boundary conditions */
@@ -192,6 +196,57 @@ static int64_t fcc_neighbour(const orc_ctx* c, int64_t site, int k12, int* b_out
     return (int64_t)b * c->Ncell + p[0] + (int64_t)c->nx * (p[1] + (int64_t)c->ny * p[2]);
 }
 
+/* ------------------------------------------------------------------ basis mode (reading C-32; "... 4 simple tetragonal
+ * sub-lattices for hcp ... up to 8 non-interacting subsets ... next-nearest neighbours").  A periodic box of nx x ny x nz
+ * cells, every cell holding the same basis of EIGHT sites; sublattice s = the s-th basis site of every cell = colour s (eight
+ * colour passes per Monte Carlo iteration); site index = s*Ncell + (i + nx*(j + ny*k)).  The bonds are not tabulated by hand:
+ * at creation, for every sublattice a, every (sublattice b, cell offset d in {-1,0,1}^3) whose separation
+ * r = pos_b + d*cell - pos_a has the bonding length is a bond.  Lengths are compared exactly, in integer units:
+ *   hcp (structure 3): orthohexagonal cell of the ideal hcp lattice doubled along x, cell = (2a, sqrt3 a, c), c^2 = 8/3 a^2;
+ *       units (a/2, sqrt3 a/6, c/2): cell = (4, 6, 2); basis (0,0,0) (1,3,0) (1,1,1) (0,4,1) and the same + (2,0,0);
+ *       |r|^2 = a^2/12 (3 dx^2 + dy^2 + 8 dz^2): nearest neighbours (12 per site, coupling J) have 3 dx^2 + dy^2 + 8 dz^2 = 12;
+ *   sc with next-nearest neighbours (structure 4): the 2 x 2 x 2 block of a simple cubic lattice as the cell, units a:
+ *       cell = (2,2,2), basis (x,y,z) in {0,1}^3 (s = x + 2y + 4z); |r|^2 = 1: 6 nearest neighbours, coupling J;
+ *       |r|^2 = 2: 12 next-nearest neighbours, coupling J2.  The box is a (2nx) x (2ny) x (2nz) simple cubic lattice.
+ * In both no bond joins two sites of one sublattice (checked at creation): the eight sublattices are non-interacting subsets.
+ * A 1- or 2-cell axis reaches the same site through several offsets and counts it as often (as L = 2 does in sc). */
+static const int HCP_POS[8][3] = { { 0, 0, 0 }, { 1, 3, 0 }, { 1, 1, 1 }, { 0, 4, 1 }, { 2, 0, 0 }, { 3, 3, 0 }, { 3, 1, 1 }, { 2, 4, 1 } };
+static int build_bonds(orc_ctx* c, double J2)
+{
+    const int hcp = c->structure == 3;
+    const int cell[3] = { hcp ? 4 : 2, hcp ? 6 : 2, 2 }, metric[3] = { hcp ? 3 : 1, 1, hcp ? 8 : 1 };
+    for (int a = 0; a < 8; ++a) {
+        c->n_bonds[a] = 0;
+        for (int b = 0; b < 8; ++b) for (int dz = -1; dz <= 1; ++dz) for (int dy = -1; dy <= 1; ++dy) for (int dx = -1; dx <= 1; ++dx) {
+            const int d[3] = { dx, dy, dz };
+            int q = 0;
+            for (int ax = 0; ax < 3; ++ax) {
+                int pa = hcp ? HCP_POS[a][ax] : (a >> ax) & 1, pb = hcp ? HCP_POS[b][ax] : (b >> ax) & 1;
+                int r = pb + d[ax] * cell[ax] - pa;
+                q += metric[ax] * r * r;
+            }
+            double J;
+            if (hcp) { if (q != 12) continue; J = c->J; }
+            else { if (q == 1) J = c->J; else if (q == 2) J = J2; else continue; }
+            if (b == a) return -1;                                    /* a bond inside a sublattice: not a non-interacting subset */
+            int k = c->n_bonds[a]++;
+            c->bond[a][k].b = b; c->bond[a][k].J = J;
+            for (int ax = 0; ax < 3; ++ax) c->bond[a][k].d[ax] = d[ax];
+        }
+        if (c->n_bonds[a] != (hcp ? 12 : 18)) return -1;
+    }
+    return 0;
+}
+static int64_t basis_neighbour(const orc_ctx* c, int64_t site, int k, double* J)
+{
+    int a = (int)(site / c->Ncell); int64_t cellidx = site % c->Ncell;
+    int p[3] = { (int)(cellidx % c->nx), (int)((cellidx / c->nx) % c->ny), (int)(cellidx / ((int64_t)c->nx * c->ny)) };
+    int dim[3] = { c->nx, c->ny, c->nz };
+    for (int ax = 0; ax < 3; ++ax) p[ax] = (p[ax] + c->bond[a][k].d[ax] + dim[ax]) % dim[ax];
+    *J = c->bond[a][k].J;
+    return (int64_t)c->bond[a][k].b * c->Ncell + p[0] + (int64_t)c->nx * (p[1] + (int64_t)c->ny * p[2]);
+}
+
 /* exchange field of ANY site, any structure (sc: decode the site and use the six-direction sum above) */
 static void field_at(const orc_ctx* c, int64_t site, double h[3])
 {
@@ -200,6 +255,13 @@ static void field_at(const orc_ctx* c, int64_t site, double h[3])
         return;
     }
     h[0] = h[1] = h[2] = 0.0;
+    if (c->structure >= 3) {
+        for (int k = 0; k < c->n_bonds[site / c->Ncell]; ++k) {
+            double J; int64_t j = basis_neighbour(c, site, k, &J);
+            for (int a = 0; a < 3; ++a) h[a] += J * c->S[3 * j + a];
+        }
+        return;
+    }
     if (c->structure == 2) {
         for (int k = 0; k < 12; ++k) {
             int64_t j = fcc_neighbour(c, site, k, NULL);
@@ -251,6 +313,23 @@ double orc_site_energy(const orc_ctx* c, int64_t site, const double S[3])
 double orc_total_energy(const orc_ctx* c)
 {
     double E = 0.0;
+    if (c->structure >= 3) {                 /* basis mode: a bond joins two different sublattices: visit it from the lower one */
+        for (int64_t i = 0; i < c->N; ++i) {
+            const double* S = &c->S[3 * i];
+            int a = (int)(i / c->Ncell);
+            for (int k = 0; k < c->n_bonds[a]; ++k) {
+                if (c->bond[a][k].b < a) continue;
+                double J; int64_t j = basis_neighbour(c, i, k, &J);
+                const double* Sj = &c->S[3 * j];
+                E -= J * (S[0] * Sj[0] + S[1] * Sj[1] + S[2] * Sj[2]);
+            }
+            double se = S[0] * c->eu[0] + S[1] * c->eu[1] + S[2] * c->eu[2];
+            double x2 = S[0] * S[0], y2 = S[1] * S[1], z2 = S[2] * S[2];
+            E += -c->Ku * se * se + c->Kc * (x2 * y2 + x2 * z2 + y2 * z2)
+                 - (S[0] * c->B[0] + S[1] * c->B[1] + S[2] * c->B[2]);
+        }
+        return E;
+    }
     if (c->structure == 2) {                 /* fcc: a bond joins two different sublattices: visit it from the lower one */
         for (int64_t i = 0; i < c->N; ++i) {
             const double* S = &c->S[3 * i];
@@ -368,6 +447,23 @@ orc_ctx* orc_create_fcc(int nx, int ny, int nz, const int periodic[3],
     orc_ctx* c = orc_create_bcc(nx, ny, nz, periodic, J, Ku, eu, Kc, B, cone0_rad, adaptive, seed);
     if (!c) return NULL;
     c->structure = 2; c->n_colours = 4; c->N = 4 * c->Ncell;
+    free(c->S);
+    c->S = (double*)malloc(sizeof(double) * 3 * c->N);
+    for (int64_t i = 0; i < c->N; ++i) { c->S[3 * i] = 0; c->S[3 * i + 1] = 0; c->S[3 * i + 2] = 1; }
+    return c;
+}
+
+/* basis mode above: kind 3 = hcp (J2 ignored), 4 = simple cubic with next-nearest neighbours (J, J2); nx x ny x nz cells of eight
+ * sites, 8 nx ny nz spins, every axis periodic, eight colours */
+orc_ctx* orc_create_basis(int kind, int nx, int ny, int nz, double J, double J2, double Ku, const double eu[3], double Kc, const double B[3],
+                          double cone0_rad, int adaptive, uint64_t seed)
+{
+    const int periodic[3] = { 1, 1, 1 };
+    if (kind != 3 && kind != 4) return NULL;
+    orc_ctx* c = orc_create_bcc(nx, ny, nz, periodic, J, Ku, eu, Kc, B, cone0_rad, adaptive, seed);
+    if (!c) return NULL;
+    c->structure = kind; c->n_colours = 8; c->N = 8 * c->Ncell;
+    if (build_bonds(c, J2)) { orc_destroy(c); return NULL; }
     free(c->S);
     c->S = (double*)malloc(sizeof(double) * 3 * c->N);
     for (int64_t i = 0; i < c->N; ++i) { c->S[3 * i] = 0; c->S[3 * i + 1] = 0; c->S[3 * i + 2] = 1; }
@@ -598,7 +694,7 @@ int64_t orc_site_of(const orc_ctx* c, int colour, int64_t a)
  * Replaces the paper's shuffled index array; requirements R1-R4 in DESIGN.md. */
 int orc_pairing(const orc_ctx* c, uint64_t sweep, int colour, int64_t* partner, uint8_t* is_leader)
 {
-    if (c->structure == 2) return -1;                        /* the constrained path sweeps two colours: sc and bcc (not the four of fcc) */
+    if (c->structure >= 2) return -1;                        /* the constrained path sweeps two colours: sc and bcc (not the four of fcc, the eight of basis mode) */
     if (!c->structure && (c->nx & 1)) return -1;
     int64_t Nc = c->N / 2;
     if (Nc & 1) return -1;                                   /* C-15 */

@@ -69,6 +69,13 @@ orc_ctx* orc_create_bcc(int nx, int ny, int nz, const int periodic[3],
 orc_ctx* orc_create_fcc(int nx, int ny, int nz, const int periodic[3],
                         double J, double Ku, const double eu[3], double Kc, const double B[3],
                         double cone0_rad, int adaptive, uint64_t seed);
+/* Basis mode ("4 simple tetragonal sub-lattices for hcp ... up to 8 non-interacting subsets ... next-nearest neighbours";
+ * reading C-32): nx x ny x nz periodic cells of EIGHT sites, 8 nx ny nz spins, eight colours (a sweep is eight colour passes),
+ * site = sublattice*nx*ny*nz + cell.  kind 3: ideal hcp, orthohexagonal cell doubled along x, 12 nearest neighbours (J; J2
+ * ignored).  kind 4: simple cubic lattice of (2nx) x (2ny) x (2nz) sites, cell = its 2 x 2 x 2 block (sublattice = x + 2y + 4z of
+ * the site in the block), 6 nearest (J) and 12 next-nearest (J2) neighbours.  Unconstrained sweeps only. */
+orc_ctx* orc_create_basis(int kind, int nx, int ny, int nz, double J, double J2, double Ku, const double eu[3], double Kc, const double B[3],
+                          double cone0_rad, int adaptive, uint64_t seed);
 void orc_destroy(orc_ctx*);
 /* periodic[a]: 0 open faces, 1 periodic, 2 anti-periodic (the spin across the wrap enters as -S_j). */
 /* Slice-averaged magnetisation along x: out[3*x + a], a = x,y,z component. */
