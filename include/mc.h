@@ -52,6 +52,8 @@ typedef struct {
 #define MC_SC   0
 #define MC_BCC  1
 #define MC_FCC  2
+#define MC_HCP  3
+#define MC_SC_NNN 4
 /* MC_BCC ("this approach can be extended to other crystal structures ... e.g. 2 simple cubic sub-lattices for bcc";
  * reading C-30): nx x ny x nz conventional cells, N = 2*nx*ny*nz spins.  Sublattice A (colour 0) sits at the cell corners,
  * B (colour 1) at the cell centres; site = sublattice*nx*ny*nz + (i + nx*(j + ny*k)); the 8 nearest neighbours of a site
@@ -62,7 +64,15 @@ typedef struct {
  * MC_FCC ("4 simple cubic sub-lattices for fcc"; reading C-31): N = 4*nx*ny*nz spins; sublattice 0 at the cell corners,
  * 1, 2, 3 at (0,1/2,1/2), (1/2,0,1/2), (1/2,1/2,0) from them; site = sublattice*nx*ny*nz + cell; 12 nearest neighbours, 4 in each
  * OTHER sublattice, so the four sublattices are FOUR colours: a Monte Carlo iteration is four colour passes (mc_half_sweep takes
- * colour 0..3).  Same restrictions as MC_BCC; unconstrained sweeps only (the constrained calls: MC_EINVAL). */
+ * colour 0..3).  Same restrictions as MC_BCC; unconstrained sweeps only (the constrained calls: MC_EINVAL).
+ * MC_HCP, MC_SC_NNN ("4 simple tetragonal sub-lattices for hcp ... up to 8 non-interacting subsets ... next-nearest
+ * neighbours"; reading C-32): nx x ny x nz periodic cells of EIGHT sites, N = 8*nx*ny*nz spins, site = sublattice*nx*ny*nz + cell,
+ * the eight sublattices are EIGHT colours: a Monte Carlo iteration is eight colour passes (mc_half_sweep takes colour 0..7).
+ * MC_HCP: ideal hcp (c/a = sqrt(8/3)), the four-site orthohexagonal cell (a, sqrt3 a, c) doubled along x; in units
+ * (a/2, sqrt3 a/6, c/2) the basis is (0,0,0) (1,3,0) (1,1,1) (0,4,1) and the same + (2,0,0); 12 nearest neighbours, coupling J.
+ * MC_SC_NNN: a simple cubic lattice of (2nx) x (2ny) x (2nz) sites, the cell is its 2 x 2 x 2 block, sublattice = x + 2y + 4z of
+ * the site in its block; 6 nearest neighbours (J) and 12 next-nearest neighbours (mc_hamiltonian.J2).  Same restrictions as
+ * MC_FCC. */
 
 /* Spin Hamiltonian, Eq. (2):  E_i = -sum_j J_ij S_i.S_j - Ku (S_i.e_i)^2 + Kc (Sx^2Sy^2 + Sx^2Sz^2 + Sy^2Sz^2) - S_i.B */
 typedef struct {
@@ -79,6 +89,7 @@ typedef struct {
     int32_t n_regions;
     double cone0_rad;            /* initial cone HALF-angle theta in radians (C-6), clamped to [1 deg, 180 deg]      */
     int32_t adaptive;            /* 1: +-1 degree per sweep toward acceptance 0.5 (C-2, C-9)        */
+    double J2;                   /* next-nearest-neighbour exchange, MC_SC_NNN only (ignored elsewhere)              */
 } mc_hamiltonian;
 
 /* Everything mc_observables() returns; all fp64; intensive quantities are per site. */

@@ -17,7 +17,8 @@ LIB_PATH = os.path.join(_HERE, "libmc_b200.so")
 MC_OK, MC_EINVAL, MC_ECUDA, MC_ESTATE = 0, -1, -2, -3
 MC_TRACE_CAPACITY = 16384
 MC_PATH_AUTO, MC_PATH_GENERIC, MC_PATH_STAGED, MC_PATH_MARCH = 0, 1, 2, 3
-MC_SC, MC_BCC, MC_FCC = 0, 1, 2
+MC_SC, MC_BCC, MC_FCC, MC_HCP, MC_SC_NNN = 0, 1, 2, 3, 4
+STRUCTURES = {"sc": (MC_SC, 1), "bcc": (MC_BCC, 2), "fcc": (MC_FCC, 4), "hcp": (MC_HCP, 8), "sc_nnn": (MC_SC_NNN, 8)}   # id, spins per cell
 
 # every symbol include/mc.h declares (tests/test_abi.py checks the header against this list and the .so)
 SYMBOLS = [
@@ -35,7 +36,7 @@ class McHamiltonian(C.Structure):
     _fields_ = [
         ("J", C.c_double), ("Ku", C.c_double), ("eu", C.c_double * 3), ("Kc", C.c_double), ("B", C.c_double * 3),
         ("bond_mask", C.c_void_p), ("region", C.c_void_p), ("region_axis", C.c_void_p), ("n_regions", C.c_int32),
-        ("cone0_rad", C.c_double), ("adaptive", C.c_int32),
+        ("cone0_rad", C.c_double), ("adaptive", C.c_int32), ("J2", C.c_double),
     ]
 
 
@@ -101,10 +102,10 @@ def _p(a):
 
 
 def make_structs(shape, periodic=(1, 1, 1), J=1.0, Ku=0.0, eu=(0, 0, 1), Kc=0.0, B=(0, 0, 0),
-                 bond_mask=None, region=None, region_axis=None, cone0=0.5, adaptive=True, structure="sc"):
+                 bond_mask=None, region=None, region_axis=None, cone0=0.5, adaptive=True, structure="sc", J2=0.0):
     """Fills mc_lattice / mc_hamiltonian; returns them plus the arrays that must stay alive during mc_create."""
     lat = McLattice(int(shape[0]), int(shape[1]), int(shape[2]), (C.c_int32 * 3)(*[int(p) for p in periodic]),   # 0 open, 1 periodic, 2 anti-periodic (x)
-                    {"sc": MC_SC, "bcc": MC_BCC, "fcc": MC_FCC}[structure])
+                    STRUCTURES[structure][0])
     keep = []
     def arr(a, dt):
         if a is None:
@@ -117,7 +118,7 @@ def make_structs(shape, periodic=(1, 1, 1), J=1.0, Ku=0.0, eu=(0, 0, 1), Kc=0.0,
     ham.region = arr(None if region is None else np.asarray(region).ravel(), np.uint16)
     ham.region_axis = arr(region_axis, np.float64)
     ham.n_regions = 0 if region_axis is None else int(np.asarray(region_axis).shape[0])
-    ham.cone0_rad = float(cone0); ham.adaptive = int(bool(adaptive))
+    ham.cone0_rad = float(cone0); ham.adaptive = int(bool(adaptive)); ham.J2 = float(J2)
     return lat, ham, keep
 
 
@@ -126,13 +127,13 @@ class Lattice:
 
     def __init__(self, nx, ny, nz, periodic=(1, 1, 1), J=1.0, Ku=0.0, eu=(0, 0, 1), Kc=0.0, B=(0, 0, 0),
                  bond_mask=None, region=None, region_axis=None, cone0=0.5, adaptive=True, seed=42,
-                 device="cuda:0", stream=None, structure="sc", guard_bytes=0):
+                 device="cuda:0", stream=None, structure="sc", guard_bytes=0, J2=0.0):
         import torch  # device memory and streams only
         self.L = load()
         self.shape = (int(nx), int(ny), int(nz))
-        self.N = int(nx) * int(ny) * int(nz) * {"sc": 1, "bcc": 2, "fcc": 4}[structure]      # spins per conventional cell
+        self.N = int(nx) * int(ny) * int(nz) * STRUCTURES[structure][1]                        # spins per cell
         self.h = None
-        lat, ham, keep = make_structs(self.shape, periodic, J, Ku, eu, Kc, B, bond_mask, region, region_axis, cone0, adaptive, structure)
+        lat, ham, keep = make_structs(self.shape, periodic, J, Ku, eu, Kc, B, bond_mask, region, region_axis, cone0, adaptive, structure, J2)
         nbytes = self.L.mc_workspace_bytes(C.byref(lat), C.byref(ham))
         if nbytes == 0:
             raise McError(MC_EINVAL, "mc_workspace_bytes rejected the lattice / Hamiltonian")

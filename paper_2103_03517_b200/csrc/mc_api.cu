@@ -17,7 +17,7 @@ constexpr size_t ALIGN = 256;
 inline size_t round_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {            // byte offsets into the caller's workspace
-    size_t spins, mask, region, axis, state, trace, staging, staging_bytes, total;
+    size_t spins, mask, region, axis, bonds, state, trace, staging, staging_bytes, total;
     long long plane, mask_plane, region_plane;
     int max_blocks;
 };
@@ -29,14 +29,50 @@ bool needs_mask(const mc_lattice* lat, const mc_hamiltonian* ham)
     return ham->bond_mask != nullptr || !lat->periodic[0] || !lat->periodic[1] || !lat->periodic[2];
 }
 
+int n_sublattices(int structure) { return structure == MC_BCC ? 2 : structure == MC_FCC ? 4 : (structure == MC_HCP || structure == MC_SC_NNN) ? 8 : 0; }
+
+// basis mode (C-32): the bonds of a site of every sublattice, found from the coordinates -- every (sublattice, cell offset in
+// {-1,0,1}^3) whose separation has the bonding length.  hcp: orthohexagonal cell doubled along x, units (a/2, sqrt3 a/6, c/2),
+// ideal c/a: |r|^2 = a^2/12 (3 dx^2 + dy^2 + 8 dz^2), nearest neighbours at |r| = a.  sc + next-nearest neighbours: the
+// 2 x 2 x 2 block as the cell, |r|^2 = 1 (J) and 2 (J2).  Returns false if a bond stays inside a sublattice.
+bool build_bond_table(int structure, float J, float J2, mc::BondEntry (*tab)[mc::MC_MAX_BONDS], unsigned char* n)
+{
+    static const int hcp_pos[8][3] = { { 0, 0, 0 }, { 1, 3, 0 }, { 1, 1, 1 }, { 0, 4, 1 }, { 2, 0, 0 }, { 3, 3, 0 }, { 3, 1, 1 }, { 2, 4, 1 } };
+    const bool hcp = structure == MC_HCP;
+    const int cell[3] = { hcp ? 4 : 2, hcp ? 6 : 2, 2 }, w[3] = { hcp ? 3 : 1, 1, hcp ? 8 : 1 };
+    for (int a = 0; a < 8; ++a) {
+        int cnt = 0;
+        for (int b = 0; b < 8; ++b)
+            for (int o = 0; o < 27; ++o) {
+                const int d[3] = { o % 3 - 1, (o / 3) % 3 - 1, o / 9 - 1 };
+                int q = 0;
+                for (int ax = 0; ax < 3; ++ax) {
+                    const int ra = hcp ? hcp_pos[a][ax] : (a >> ax) & 1, rb = hcp ? hcp_pos[b][ax] : (b >> ax) & 1;
+                    const int sep = rb + d[ax] * cell[ax] - ra;
+                    q += w[ax] * sep * sep;
+                }
+                float Jb;
+                if (hcp) { if (q != 12) continue; Jb = J; }
+                else if (q == 1) Jb = J; else if (q == 2) Jb = J2; else continue;
+                if (b == a || cnt == mc::MC_MAX_BONDS) return false;
+                tab[a][cnt].b = (signed char)b; tab[a][cnt].dx = (signed char)d[0]; tab[a][cnt].dy = (signed char)d[1]; tab[a][cnt].dz = (signed char)d[2];
+                tab[a][cnt].J = Jb; ++cnt;
+            }
+        if (cnt != (hcp ? 12 : 18)) return false;
+        n[a] = (unsigned char)cnt;
+    }
+    return true;
+}
+
 bool valid_lattice(const mc_lattice* lat)
 {
     if (!lat) return false;
     const int dim[3] = { lat->nx, lat->ny, lat->nz };
-    if (lat->structure == MC_BCC || lat->structure == MC_FCC) {          // P:34, C-30 / C-31: fully periodic, rows of float4 items
+    if (lat->structure == MC_BCC || lat->structure == MC_FCC || lat->structure == MC_HCP || lat->structure == MC_SC_NNN) {
+        // P:34, C-30 / C-31 / C-32: sublattices as colours; fully periodic, rows of float4 items
         for (int a = 0; a < 3; ++a) if (dim[a] < 1 || lat->periodic[a] != 1) return false;
         if (lat->nx % 4) return false;
-        return (lat->structure == MC_FCC ? 4.0 : 2.0) * (double)lat->nx * lat->ny * lat->nz < 2147483648.0;
+        return (double)n_sublattices(lat->structure) * (double)lat->nx * lat->ny * lat->nz < 2147483648.0;
     }
     if (lat->structure != MC_SC) return false;
     for (int a = 0; a < 3; ++a) {
@@ -52,8 +88,8 @@ bool valid_lattice(const mc_lattice* lat)
 Layout make_layout(const mc_lattice* lat, const mc_hamiltonian* ham)
 {
     Layout L{};
-    const bool sub = lat->structure == MC_BCC || lat->structure == MC_FCC;      // sublattices as colours, each a full grid of cells
-    const size_t ncol = lat->structure == MC_FCC ? 4 : 2;
+    const bool sub = n_sublattices(lat->structure) != 0;                        // sublattices as colours, each a full grid of cells
+    const size_t ncol = sub ? (size_t)n_sublattices(lat->structure) : 2;
     const size_t Nc = sub ? (size_t)lat->nx * lat->ny * lat->nz : (size_t)lat->nx / 2 * lat->ny * lat->nz;
     L.plane = (long long)round_up(Nc, 64);
     L.mask_plane = (long long)round_up(Nc, 256);
@@ -64,6 +100,7 @@ Layout make_layout(const mc_lattice* lat, const mc_hamiltonian* ham)
     L.mask = off;     if (needs_mask(lat, ham)) off += round_up((size_t)2 * L.mask_plane, ALIGN);
     L.region = off;   if (ham->region) off += round_up((size_t)2 * L.region_plane * sizeof(uint16_t), ALIGN);
     L.axis = off;     if (ham->region) off += round_up((size_t)ham->n_regions * sizeof(float4), ALIGN);
+    L.bonds = off;    if (lat->structure == MC_HCP || lat->structure == MC_SC_NNN) off += round_up(sizeof(mc::BondEntry) * 8 * mc::MC_MAX_BONDS, ALIGN);
     L.state = off;    off += round_up(sizeof(DevState), ALIGN);
     L.trace = off;    off += round_up((size_t)TRACE_CAP * 6 * sizeof(double), ALIGN);
     // staging: the [N][3] fp32 lexicographic image of the state during mc_set_spins / mc_get_spins, or the [N] fp32 + [N] u8
@@ -202,13 +239,15 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
 
     const int nx = lat->nx, ny = lat->ny, nz = lat->nz;
     const bool bcc = lat->structure == MC_BCC, fcc = lat->structure == MC_FCC;
-    const uint32_t ncol = fcc ? 4u : 2u;
-    const uint32_t Nc = (bcc || fcc) ? (uint32_t)nx * ny * nz : (uint32_t)nx / 2 * ny * nz, N = ncol * Nc, R = (bcc || fcc) ? nx : nx / 2;
+    const bool basis = lat->structure == MC_HCP || lat->structure == MC_SC_NNN, sub = bcc || fcc || basis;
+    const uint32_t ncol = sub ? (uint32_t)n_sublattices(lat->structure) : 2u;
+    const uint32_t Nc = sub ? (uint32_t)nx * ny * nz : (uint32_t)nx / 2 * ny * nz, N = ncol * Nc, R = sub ? nx : nx / 2;
     char* ws = (char*)dev_workspace;
     Params& P = ctx->P;
     P.nx = nx; P.ny = ny; P.nz = nz; P.R = (int)R; P.Nc = Nc; P.N = N; P.invN = 1.0 / (double)N;
     P.anti_x = lat->periodic[0] == 2 ? 1 : 0;
     P.bcc = bcc ? 1 : 0; P.fcc = fcc ? 1 : 0; P.ncol = (int)ncol;
+    P.basis = basis ? lat->structure : 0; P.sub = sub ? 1 : 0; P.bonds = nullptr;
     P.per_mask = (lat->periodic[0] ? 1 : 0) | (lat->periodic[1] ? 2 : 0) | (lat->periodic[2] ? 4 : 0);
     P.plane = L.plane; P.S = (float*)(ws + L.spins);
     P.mask = nullptr; P.mask_plane = L.mask_plane; P.region = nullptr; P.region_plane = L.region_plane; P.axis = nullptr;
@@ -219,7 +258,8 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     P.st = (DevState*)(ws + L.state); P.max_blocks = L.max_blocks;
     {   // fixed-point unit 2^-k of the fused sums: the largest k <= 40 with N * (largest per-site term) * 2^k < 2^61
         const double bmag = sqrt(ham->B[0] * ham->B[0] + ham->B[1] * ham->B[1] + ham->B[2] * ham->B[2]);
-        const double mag = 1.0 + 6.0 * fabs(ham->J) + 2.0 * fabs(ham->Ku) + 2.0 * fabs(ham->Kc) + bmag;
+        const double zJ = lat->structure == MC_SC_NNN ? 6.0 * fabs(ham->J) + 12.0 * fabs(ham->J2) : (bcc ? 8.0 : (fcc || basis) ? 12.0 : 6.0) * fabs(ham->J);
+        const double mag = 1.0 + zJ + 2.0 * fabs(ham->Ku) + 2.0 * fabs(ham->Kc) + bmag;
         int lg = 0; while (ldexp(1.0, lg) < (double)N * mag) ++lg;
         int k = 61 - lg; if (k > 40) k = 40;
         P.fx_scale = (float)ldexp(1.0, k); P.fx_inv = ldexp(1.0, -k);
@@ -230,13 +270,13 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     ctx->aniso = (ham->Ku != 0.0 ? 1 : 0) | (ham->Kc != 0.0 ? 2 : 0);
     ctx->field = ham->B[0] != 0.0 || ham->B[1] != 0.0 || ham->B[2] != 0.0;
     ctx->masked = needs_mask(lat, ham);
-    ctx->vec = (bcc || fcc || nx % 8 == 0) ? 4 : 1;
+    ctx->vec = (sub || nx % 8 == 0) ? 4 : 1;
     ctx->geom.RV = R / ctx->vec; ctx->geom.n_items = Nc / ctx->vec;
     ctx->geom.div_rv = make_div(ctx->geom.RV); ctx->geom.div_nz = make_div((uint32_t)nz);
     { uint32_t sh = 0; while (sh < 5 && ny % (2 << sh) == 0) ++sh; ctx->geom.yb_shift = sh; }      // up to 32 rows per block
 
     // pairing geometry (C-11); the constrained path needs an even colour population (C-15)
-    ctx->pair_ok = (Nc % 2 == 0) && Nc >= 2 && !fcc;           // two-colour lattices (sc, bcc); fcc has four passes per sweep
+    ctx->pair_ok = (Nc % 2 == 0) && Nc >= 2 && ncol == 2;      // two-colour lattices (sc, bcc); fcc has four passes per sweep, hcp / sc_nnn eight
     if (ctx->pair_ok) {
         PairGeom& G = ctx->pgeom;
         uint32_t Bc = 32; while (Nc % (2 * Bc)) Bc >>= 1;
@@ -249,6 +289,15 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
 
     // ---- side data: bond mask (boundary conditions AND the caller's mask) and grain ids, colour-split on the host
     cudaError_t ce = cudaSuccess;
+    if (basis) {                                                              // C-32: the bond table of the eight sublattices
+        mc::BondEntry tab[8][mc::MC_MAX_BONDS];
+        memset(tab, 0, sizeof tab);
+        if (!build_bond_table(lat->structure, (float)ham->J, (float)ham->J2, tab, P.nbonds)) return bail(MC_EINVAL, "basis mode: a bond inside a sublattice");
+        ce = cudaMemcpyAsync(ws + L.bonds, tab, sizeof tab, cudaMemcpyHostToDevice, ctx->stream);
+        if (ce == cudaSuccess) ce = cudaStreamSynchronize(ctx->stream);
+        if (ce != cudaSuccess) return bail(MC_ECUDA, cudaGetErrorString(ce));
+        P.bonds = (const mc::BondEntry*)(ws + L.bonds);
+    }
     if (ctx->masked) {
         std::vector<uint8_t> split((size_t)2 * L.mask_plane, 0);
         const int dim[3] = { nx, ny, nz };
@@ -539,7 +588,7 @@ static int hook_common(mc_ctx* ctx, int colour, float* host_x, uint8_t* host_acc
     const int nx = ctx->P.nx, ny = ctx->P.ny;
     for (uint32_t s = 0; (host_x || host_acc) && s < N; ++s) {
         const int x = s % nx, y = (s / nx) % ny, z = s / ((uint32_t)nx * ny);
-        if (((ctx->P.bcc || ctx->P.fcc) ? (int)(s / ctx->P.Nc) : ((x + y + z) & 1)) != colour) continue;      // bcc / fcc: colour = sublattice
+        if ((ctx->P.sub ? (int)(s / ctx->P.Nc) : ((x + y + z) & 1)) != colour) continue;      // bcc / fcc: colour = sublattice
         if (host_x) host_x[s] = hx[s];
         if (host_acc) host_acc[s] = ha[s];
     }
@@ -551,7 +600,7 @@ static int hook_common(mc_ctx* ctx, int colour, float* host_x, uint8_t* host_acc
 int mc_half_sweep(mc_ctx* ctx, double T, int colour, float* host_x, uint8_t* host_acc)
 {
     CHECK_CTX();
-    if (!(T > 0.0) || colour < 0 || colour >= ctx->P.ncol) return fail(ctx, MC_EINVAL, "mc_half_sweep: need T > 0 and a colour of the lattice (0, 1; fcc: 0..3)");
+    if (!(T > 0.0) || colour < 0 || colour >= ctx->P.ncol) return fail(ctx, MC_EINVAL, "mc_half_sweep: need T > 0 and a colour of the lattice (0, 1; fcc: 0..3; hcp, sc_nnn: 0..7)");
     return hook_common(ctx, colour, host_x, host_acc, false, (float)(1.0 / T));
 }
 
@@ -609,7 +658,7 @@ int mc_profile_x(mc_ctx* ctx, double* host_profile)
 {
     CHECK_CTX();
     if (!host_profile) return fail(ctx, MC_EINVAL, "mc_profile_x: null pointer");
-    if (ctx->P.bcc || ctx->P.fcc) return fail(ctx, MC_EINVAL, "mc_profile_x: simple cubic lattices only");
+    if (ctx->P.sub) return fail(ctx, MC_EINVAL, "mc_profile_x: simple cubic lattices only");
     const int nx = ctx->P.nx;
     const size_t bytes = (size_t)nx * 3 * sizeof(long long);
     long long* tmp = (long long*)((char*)ctx->staging + ctx->staging_bytes - round_up(bytes, ALIGN));   // tail of the staging area

@@ -42,6 +42,10 @@ struct DevState {
     long long isum[2][NQ];           // exact fixed-point sums in flight: [0] the sweep (both colour passes), [1] the measurement
 };
 
+// basis mode (C-32): one bond of a site of a sublattice = (other sublattice, cell offset in {-1,0,1}^3, coupling)
+constexpr int MC_MAX_BONDS = 18;
+struct BondEntry { signed char b, dx, dy, dz; float J; };
+
 struct Params {
     int nx, ny, nz, R;               // R = nx/2 sites of one colour per row
     int anti_x;                      // 1: anti-periodic boundary along x (domain-wall box); the wrap bond sees -S_j
@@ -49,6 +53,10 @@ struct Params {
     int fcc;                         // 1: face-centred cubic (C-31): FOUR colours = sublattices, R = nx, 12 neighbours
     int ncol;                        // colours swept per Monte Carlo iteration: 2 (sc, bcc), 4 (fcc)
     int bcc;                         // 1: body-centred cubic (C-30): colour = sublattice, R = nx cells per row, 8 neighbours
+    int basis;                       // MC_HCP / MC_SC_NNN (C-32): EIGHT colours = sublattices of an eight-site cell, bonds from the table
+    int sub;                         // 1: colours are sublattices stored as full grids of cells (bcc, fcc, basis): site = colour * Nc + cell
+    const BondEntry* bonds;          // basis: [8][MC_MAX_BONDS] bonds of a site of every sublattice (device memory in the workspace)
+    unsigned char nbonds[8];
     uint32_t Nc;                     // sites per colour
     uint32_t N;
     double invN;                     // 1 / N (host-computed: keeps an fp64 division off the finalising thread)
@@ -349,6 +357,51 @@ __device__ __forceinline__ void fcc_exchange_field(const Params& P, const FccPos
             }
 #pragma unroll
             for (int k = 0; k < 4; ++k) { hc[c][k] += s[k]; if (b < colour) hlc[c][k] += s[k]; }
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { h[k] = { hc[0][k], hc[1][k], hc[2][k] }; hl[k] = { hlc[0][k], hlc[1][k], hlc[2][k] }; }
+}
+
+// --------------------------------------------------------------------------------------------------------------
+// basis mode (C-32: hcp, simple cubic with next-nearest neighbours): eight sublattices = EIGHT colours, each a full
+// nx x ny x nz grid of cells (R = nx).  The bonds of a site of sublattice a come from a table the host derived from the
+// coordinates: (sublattice b, cell offset (dx,dy,dz), coupling J_b).  An item is 4 consecutive cells of a row; a bond with
+// dx = 0 costs one float4 per component, dx = +-1 a float4 plus the one cell outside the item.  h INCLUDES the couplings
+// (they differ per bond); hl collects the bonds into sublattices b < a (E_exch counts every bond once, as for fcc).
+// --------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void basis_exchange_field(const Params& P, const FccPos& q, int colour, Vec3 (&h)[4], Vec3 (&hl)[4])
+{
+    const uint32_t nx = (uint32_t)P.nx, ny = (uint32_t)P.ny, nz = (uint32_t)P.nz;
+    float hc[3][4], hlc[3][4];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { hc[c][k] = 0.0f; hlc[c][k] = 0.0f; }
+    const int2* tab = reinterpret_cast<const int2*>(P.bonds + colour * MC_MAX_BONDS);
+    const int n = P.nbonds[colour];
+    for (int e = 0; e < n; ++e) {
+        const int2 raw = __ldg(tab + e);
+        const int b = (int)(signed char)(raw.x & 0xFF), dx = (int)(signed char)((raw.x >> 8) & 0xFF);
+        const int dy = (int)(signed char)((raw.x >> 16) & 0xFF), dz = (int)(signed char)((raw.x >> 24) & 0xFF);
+        const float J = __int_as_float(raw.y);
+        const uint32_t y2 = dy > 0 ? (q.y + 1 == ny ? 0u : q.y + 1) : dy < 0 ? (q.y == 0 ? ny - 1 : q.y - 1) : q.y;
+        const uint32_t z2 = dz > 0 ? (q.z + 1 == nz ? 0u : q.z + 1) : dz < 0 ? (q.z == 0 ? nz - 1 : q.z - 1) : q.z;
+        const uint32_t xe = dx > 0 ? (q.i0 + 4 == nx ? 0u : q.i0 + 4) : (q.i0 == 0 ? nx - 1 : q.i0 - 1);
+        const float* O = P.S + (long long)b * 3 * P.plane + (z2 * ny + y2) * nx;
+        const float Jl = b < colour ? J : 0.0f;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const float* Oc = O + (long long)c * P.plane;
+            const Pack<4> o = ld_nc<4>(Oc + q.i0);
+            float s0 = o.v[0], s1 = o.v[1], s2 = o.v[2], s3 = o.v[3];
+            if (dx != 0) {
+                const float ex = __ldg(Oc + xe);
+                if (dx > 0) { s0 = o.v[1]; s1 = o.v[2]; s2 = o.v[3]; s3 = ex; }
+                else        { s3 = o.v[2]; s2 = o.v[1]; s1 = o.v[0]; s0 = ex; }
+            }
+            hc[c][0] = fmaf(J, s0, hc[c][0]); hc[c][1] = fmaf(J, s1, hc[c][1]); hc[c][2] = fmaf(J, s2, hc[c][2]); hc[c][3] = fmaf(J, s3, hc[c][3]);
+            hlc[c][0] = fmaf(Jl, s0, hlc[c][0]); hlc[c][1] = fmaf(Jl, s1, hlc[c][1]); hlc[c][2] = fmaf(Jl, s2, hlc[c][2]); hlc[c][3] = fmaf(Jl, s3, hlc[c][3]);
         }
     }
 #pragma unroll

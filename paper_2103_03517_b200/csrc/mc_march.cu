@@ -45,7 +45,7 @@ bool plan_march(mc_ctx* c)
 {
     c->march_ok = c->march_possible = false;
     const mc_lattice& lat = c->lat;
-    if (c->P.anti_x || c->P.fcc) return false;
+    if (c->P.anti_x || c->P.fcc || c->P.basis) return false;
     if (!c->masked && !(lat.periodic[0] == 1 && lat.periodic[1] == 1 && lat.periodic[2] == 1)) return false;
     if (c->P.bcc ? (lat.nx % 4 != 0 || lat.nz < 8) : (lat.nx % 8 != 0)) return false;     // bcc: 4 cells per item, z-march only
     MarchGeom& G = c->mgeom;

@@ -20,7 +20,8 @@ namespace mc {
 #ifndef MC_PASS_MIN_BLOCKS
 #define MC_PASS_MIN_BLOCKS 6
 #endif
-// LAT: 0 simple cubic; 1 bcc, 2 fcc (mc_common.cuh): VEC = 4 consecutive cells of one sublattice, site stride 1 instead of 2;
+// LAT: 0 simple cubic; 1 bcc, 2 fcc, 3 basis mode (hcp, sc + next-nearest neighbours: eight colours, bond table) (mc_common.cuh):
+// VEC = 4 consecutive cells of one sublattice, site stride 1 instead of 2;
 // fcc: four colours, the exchange energy of a bond is summed in the pass of its higher colour (hl).
 // COL >= 0: the colour as a compile-time constant (fcc: which rows and shifts a sublattice reads is then resolved by the compiler).
 template <int VEC, int ANISO, bool MASKED, int MODE, int LAT = 0, int COL = -1>
@@ -49,7 +50,8 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
         static_assert(!LAT || (VEC == 4 && !MASKED), "the bcc / fcc passes are VEC = 4, unmasked instantiations");
         constexpr uint32_t SS = LAT ? 1u : 2u;                    // site-id stride between the sites of an item
         ItemPos q;
-        Vec3 h[VEC], e[VEC], hl[LAT == 2 ? VEC : 1];
+        Vec3 h[VEC], e[VEC], hl[LAT >= 2 ? VEC : 1];
+        const float Jm = LAT == 3 ? 1.0f : P.J;                   // basis mode: the couplings are already in h, hl
         if (LAT == 1) {
             const BccPos b = bcc_locate(P, G, item, colour);
             q.a0 = b.a0; q.site0 = b.site0; q.xh0 = b.i0; q.par = 0u;
@@ -58,6 +60,10 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
             const FccPos b = fcc_locate(P, G, item, colour);
             q.a0 = b.a0; q.site0 = b.site0; q.xh0 = b.i0; q.par = 0u;
             if (VEC == 4) fcc_exchange_field(P, b, colour, reinterpret_cast<Vec3(&)[4]>(h), reinterpret_cast<Vec3(&)[4]>(hl));
+        } else if (LAT == 3) {
+            const FccPos b = fcc_locate(P, G, item, colour);
+            q.a0 = b.a0; q.site0 = b.site0; q.xh0 = b.i0; q.par = 0u;
+            if (VEC == 4) basis_exchange_field(P, b, colour, reinterpret_cast<Vec3(&)[4]>(h), reinterpret_cast<Vec3(&)[4]>(hl));
         } else {
             q = locate<VEC>(P, G, item, colour);
             exchange_field<VEC, MASKED>(P, q, colour, h);
@@ -91,7 +97,7 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
             for (int kp = 0; kp < 4; kp += 2) {
                 V3p S = { make_float2(sx.v[kp], sx.v[kp + 1]), make_float2(sy.v[kp], sy.v[kp + 1]), make_float2(sz.v[kp], sz.v[kp + 1]) };
                 const V3p hp = pack3(h[kp], h[kp + 1]);
-                const f2 J2 = splat(P.J);
+                const f2 J2 = splat(Jm);
                 const V3p hJ = { mul2(J2, hp.x), mul2(J2, hp.y), mul2(J2, hp.z) };
                 const V3p ep = (ANISO & 1) ? pack3(e[kp], e[kp + 1]) : B2;
                 V3p d, Sn;
@@ -110,8 +116,8 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
                 if (dbg_x)   { dbg_x[q.site0 + SS * kp] = xx.x; dbg_x[q.site0 + SS * kp + SS] = xx.y; }
                 if (dbg_acc) { dbg_acc[q.site0 + SS * kp] = (uint8_t)ok0; dbg_acc[q.site0 + SS * kp + SS] = (uint8_t)ok1; }
                 f2s[0] = add2(f2s[0], S.x); f2s[1] = add2(f2s[1], S.y); f2s[2] = add2(f2s[2], S.z);
-                if (LAT == 2) {
-                    const V3p hlp = pack3(hl[LAT == 2 ? kp : 0], hl[LAT == 2 ? kp + 1 : 0]);
+                if (LAT >= 2) {
+                    const V3p hlp = pack3(hl[LAT >= 2 ? kp : 0], hl[LAT >= 2 ? kp + 1 : 0]);
                     f2s[3] = sub2(f2s[3], dot3p(S, V3p{ mul2(J2, hlp.x), mul2(J2, hlp.y), mul2(J2, hlp.z) }));
                 } else if (colour == 1) f2s[3] = sub2(f2s[3], dot3p(S, hJ));
                 if (ANISO) f2s[4] = add2(f2s[4], onsite_from<ANISO>(ok0, ok1, s4S, s4v, euS, euv, P.Ku, P.Kc));
@@ -123,7 +129,7 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
 #pragma unroll
         for (int k = 0; k < ((VEC == 4 && MODE == MODE_SWEEP) ? 0 : VEC); ++k) {
             Vec3 S = { sx.v[k], sy.v[k], sz.v[k] };
-            const Vec3 hJ = { P.J * h[k].x, P.J * h[k].y, P.J * h[k].z };
+            const Vec3 hJ = { Jm * h[k].x, Jm * h[k].y, Jm * h[k].z };
             if (MODE == MODE_SWEEP) {
                 Vec3 d, Sn;
                 cone_move(S, omc, uniform01(w0[k]), uniform_azimuth(w0[k], w1[k]), d, Sn);
@@ -137,7 +143,7 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
                 if (dbg_acc) dbg_acc[q.site0 + SS * k] = (uint8_t)ok;
             }
             f[0] += S.x; f[1] += S.y; f[2] += S.z;
-            if (LAT == 2) { const Vec3& g = hl[LAT == 2 ? k : 0]; f[3] -= dot3(S, Vec3{ P.J * g.x, P.J * g.y, P.J * g.z }); }
+            if (LAT >= 2) { const Vec3& g = hl[LAT >= 2 ? k : 0]; f[3] -= dot3(S, Vec3{ Jm * g.x, Jm * g.y, Jm * g.z }); }
             else if (colour == 1) f[3] -= dot3(S, hJ);
             if (ANISO) f[4] += aniso_energy<ANISO>(S, P.Ku, e[(ANISO & 1) ? k : 0], P.Kc);
             f[5] -= dot3(S, B);

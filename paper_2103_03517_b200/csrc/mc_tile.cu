@@ -37,7 +37,7 @@ bool plan_tile(mc_ctx* c)
 {
     c->tile_ok = c->tile_possible = false;
     const mc_lattice& lat = c->lat;
-    if (c->masked || c->P.region || c->P.bcc || c->P.fcc) return false;
+    if (c->masked || c->P.region || c->P.sub) return false;
     if (!(lat.periodic[0] >= 1 && lat.periodic[1] == 1 && lat.periodic[2] == 1)) return false;   // x may be anti-periodic (ANTI instantiation)
     const int R = lat.nx / 2;
     if (R % 4) return false;                                    // TMA bulk copies move whole rows: 16-byte multiples

@@ -54,7 +54,7 @@ __global__ void lex_to_split_kernel(const __grid_constant__ Params P, const floa
     if (s >= P.N) return;
     const uint32_t x = s % (uint32_t)P.nx, row = s / (uint32_t)P.nx, y = row % (uint32_t)P.ny, z = row / (uint32_t)P.ny;
     uint32_t c = (x + y + z) & 1u, a = row * (uint32_t)P.R + (x >> 1);
-    if (P.bcc || P.fcc) { c = s / P.Nc; a = s - c * P.Nc; }        // bcc / fcc: site = sublattice * Ncell + cell
+    if (P.sub) { c = s / P.Nc; a = s - c * P.Nc; }        // bcc / fcc / basis: site = sublattice * Ncell + cell
     float vx = lex[3ull * s], vy = lex[3ull * s + 1], vz = lex[3ull * s + 2];
     // a spin that is already unit to fp32 rounding (what mc_get_spins returns) is stored as it is: upload(download(state)) is
     // the identity, so a checkpoint restores bit for bit; anything else is normalised
@@ -71,7 +71,7 @@ __global__ void split_to_lex_kernel(const __grid_constant__ Params P, float* __r
     if (s >= P.N) return;
     const uint32_t x = s % (uint32_t)P.nx, row = s / (uint32_t)P.nx, y = row % (uint32_t)P.ny, z = row / (uint32_t)P.ny;
     uint32_t c = (x + y + z) & 1u, a = row * (uint32_t)P.R + (x >> 1);
-    if (P.bcc || P.fcc) { c = s / P.Nc; a = s - c * P.Nc; }
+    if (P.sub) { c = s / P.Nc; a = s - c * P.Nc; }
     const float* Sc = P.S + (long long)c * 3 * P.plane;
     lex[3ull * s] = Sc[a]; lex[3ull * s + 1] = Sc[P.plane + a]; lex[3ull * s + 2] = Sc[2 * P.plane + a];
 }
@@ -94,7 +94,7 @@ __global__ void init_random_kernel(const __grid_constant__ Params P)
     if (a >= P.Nc) return;
     const uint32_t R = (uint32_t)P.R, row = a / R, xh = a - row * R, y = row % (uint32_t)P.ny, z = row / (uint32_t)P.ny;
     for (uint32_t c = 0; c < (uint32_t)P.ncol; ++c) {
-        const uint32_t site = (P.bcc || P.fcc) ? c * P.Nc + a : row * (uint32_t)P.nx + 2u * xh + ((y + z + c) & 1u);
+        const uint32_t site = P.sub ? c * P.Nc + a : row * (uint32_t)P.nx + 2u * xh + ((y + z + c) & 1u);
         uint32_t r0, r1, r2, r3;
         philox4x32_10(P.key, site, TAG_INIT, 0u, 0u, r0, r1, r2, r3);
         const float zz = fmaf(2.0f, uniform01(r0), -1.0f);

@@ -35,7 +35,7 @@ def test_library_exports_every_declared_symbol(lib):
 
 def test_struct_sizes_match_the_header_layout():
     assert C.sizeof(binding.McLattice) == 28
-    assert C.sizeof(binding.McHamiltonian) == 8 + 8 + 24 + 8 + 24 + 8 + 8 + 8 + 8 + 8 + 8
+    assert C.sizeof(binding.McHamiltonian) == 8 + 8 + 24 + 8 + 24 + 8 + 8 + 8 + 8 + 8 + 8 + 8
     assert C.sizeof(binding.McObs) == 8 * (2 + 2 + 3 + 1 + 4 + 3 + 1 + 4 + 4 + 2 + 3)
 
 
