@@ -42,9 +42,11 @@ struct DevState {
     long long isum[2][NQ];           // exact fixed-point sums in flight: [0] the sweep (both colour passes), [1] the measurement
 };
 
-// basis mode (C-32): one bond of a site of a sublattice = (other sublattice, cell offset in {-1,0,1}^3, coupling)
+// basis mode (C-32): the bonds of a site of a sublattice, grouped by the ROW of cells they reach = (other sublattice b, cell
+// offset dy, dz); xmask: bit 0 / 1 / 2 set <=> the row holds a bond at cell offset dx = -1 / 0 / +1 (same coupling J: b fixes the
+// bond length).  Rows into sublattices b < a come first (n_lower of them): their partial field is the part of E_exch this pass owns.
 constexpr int MC_MAX_BONDS = 18;
-struct BondEntry { signed char b, dx, dy, dz; float J; };
+struct BondEntry { signed char b, xmask, dy, dz; float J; };
 
 struct Params {
     int nx, ny, nz, R;               // R = nx/2 sites of one colour per row
@@ -56,7 +58,7 @@ struct Params {
     int basis;                       // MC_HCP / MC_SC_NNN (C-32): EIGHT colours = sublattices of an eight-site cell, bonds from the table
     int sub;                         // 1: colours are sublattices stored as full grids of cells (bcc, fcc, basis): site = colour * Nc + cell
     const BondEntry* bonds;          // basis: [8][MC_MAX_BONDS] bonds of a site of every sublattice (device memory in the workspace)
-    unsigned char nbonds[8];
+    unsigned char nbonds[8], nlower[8];   // rows of the table per sublattice; how many of them lead into lower sublattices
     uint32_t Nc;                     // sites per colour
     uint32_t N;
     double invN;                     // 1 / N (host-computed: keeps an fp64 division off the finalising thread)
@@ -370,42 +372,51 @@ __device__ __forceinline__ void fcc_exchange_field(const Params& P, const FccPos
 // dx = 0 costs one float4 per component, dx = +-1 a float4 plus the one cell outside the item.  h INCLUDES the couplings
 // (they differ per bond); hl collects the bonds into sublattices b < a (E_exch counts every bond once, as for fcc).
 // --------------------------------------------------------------------------------------------------------------
+#ifndef MC_BASIS_UNROLL
+#define MC_BASIS_UNROLL 4      // rows of the table in flight together (112^3 cells of hcp, us per sweep: 1: 388, 2: 352, 4: 337, 6: 353)
+#endif
 __device__ __forceinline__ void basis_exchange_field(const Params& P, const FccPos& q, int colour, Vec3 (&h)[4], Vec3 (&hl)[4])
 {
     const uint32_t nx = (uint32_t)P.nx, ny = (uint32_t)P.ny, nz = (uint32_t)P.nz;
-    float hc[3][4], hlc[3][4];
+    float hc[3][4];
 #pragma unroll
     for (int c = 0; c < 3; ++c)
 #pragma unroll
-        for (int k = 0; k < 4; ++k) { hc[c][k] = 0.0f; hlc[c][k] = 0.0f; }
+        for (int k = 0; k < 4; ++k) hc[c][k] = 0.0f;
     const int2* tab = reinterpret_cast<const int2*>(P.bonds + colour * MC_MAX_BONDS);
-    const int n = P.nbonds[colour];
-    for (int e = 0; e < n; ++e) {
+    const int n = P.nbonds[colour], nlow = P.nlower[colour];
+    const uint32_t xm = q.i0 == 0 ? nx - 1 : q.i0 - 1, xp = q.i0 + 4 == nx ? 0u : q.i0 + 4;      // the cells just outside the item
+    auto row = [&](int e) {
         const int2 raw = __ldg(tab + e);
-        const int b = (int)(signed char)(raw.x & 0xFF), dx = (int)(signed char)((raw.x >> 8) & 0xFF);
+        const int b = raw.x & 0xFF, m = (raw.x >> 8) & 0xFF;
         const int dy = (int)(signed char)((raw.x >> 16) & 0xFF), dz = (int)(signed char)((raw.x >> 24) & 0xFF);
         const float J = __int_as_float(raw.y);
+        const float Jm = (m & 1) ? J : 0.0f, J0 = (m & 2) ? J : 0.0f, Jp = (m & 4) ? J : 0.0f;
         const uint32_t y2 = dy > 0 ? (q.y + 1 == ny ? 0u : q.y + 1) : dy < 0 ? (q.y == 0 ? ny - 1 : q.y - 1) : q.y;
         const uint32_t z2 = dz > 0 ? (q.z + 1 == nz ? 0u : q.z + 1) : dz < 0 ? (q.z == 0 ? nz - 1 : q.z - 1) : q.z;
-        const uint32_t xe = dx > 0 ? (q.i0 + 4 == nx ? 0u : q.i0 + 4) : (q.i0 == 0 ? nx - 1 : q.i0 - 1);
         const float* O = P.S + (long long)b * 3 * P.plane + (z2 * ny + y2) * nx;
-        const float Jl = b < colour ? J : 0.0f;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             const float* Oc = O + (long long)c * P.plane;
+            // branch-free: the three candidate cells of every site are always fetched (the two outside the item are L1 hits of the
+            // neighbouring items' float4) and weighted with J or 0, so that the loads of several rows can be in flight together
             const Pack<4> o = ld_nc<4>(Oc + q.i0);
-            float s0 = o.v[0], s1 = o.v[1], s2 = o.v[2], s3 = o.v[3];
-            if (dx != 0) {
-                const float ex = __ldg(Oc + xe);
-                if (dx > 0) { s0 = o.v[1]; s1 = o.v[2]; s2 = o.v[3]; s3 = ex; }
-                else        { s3 = o.v[2]; s2 = o.v[1]; s1 = o.v[0]; s0 = ex; }
-            }
-            hc[c][0] = fmaf(J, s0, hc[c][0]); hc[c][1] = fmaf(J, s1, hc[c][1]); hc[c][2] = fmaf(J, s2, hc[c][2]); hc[c][3] = fmaf(J, s3, hc[c][3]);
-            hlc[c][0] = fmaf(Jl, s0, hlc[c][0]); hlc[c][1] = fmaf(Jl, s1, hlc[c][1]); hlc[c][2] = fmaf(Jl, s2, hlc[c][2]); hlc[c][3] = fmaf(Jl, s3, hlc[c][3]);
+            const float em = __ldg(Oc + xm), ep = __ldg(Oc + xp);
+            hc[c][0] = fmaf(Jm, em,     fmaf(J0, o.v[0], fmaf(Jp, o.v[1], hc[c][0])));
+            hc[c][1] = fmaf(Jm, o.v[0], fmaf(J0, o.v[1], fmaf(Jp, o.v[2], hc[c][1])));
+            hc[c][2] = fmaf(Jm, o.v[1], fmaf(J0, o.v[2], fmaf(Jp, o.v[3], hc[c][2])));
+            hc[c][3] = fmaf(Jm, o.v[2], fmaf(J0, o.v[3], fmaf(Jp, ep,     hc[c][3])));
         }
-    }
+    };
+    constexpr int UNR = MC_BASIS_UNROLL;
+#pragma unroll UNR
+    for (int e = 0; e < nlow; ++e) row(e);
 #pragma unroll
-    for (int k = 0; k < 4; ++k) { h[k] = { hc[0][k], hc[1][k], hc[2][k] }; hl[k] = { hlc[0][k], hlc[1][k], hlc[2][k] }; }
+    for (int k = 0; k < 4; ++k) hl[k] = { hc[0][k], hc[1][k], hc[2][k] };
+#pragma unroll UNR
+    for (int e = nlow; e < n; ++e) row(e);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) h[k] = { hc[0][k], hc[1][k], hc[2][k] };
 }
 
 // easy axes of the VEC sites of an item: uniform, or per grain through the region table (config c5)

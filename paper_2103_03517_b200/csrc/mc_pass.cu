@@ -49,7 +49,7 @@ int launch_pass_generic(mc_ctx* ctx, int mode, int colour, float invT, int flags
     if (ctx->P.bcc) fn = mode == MODE_SWEEP ? pick_pass_lat<MODE_SWEEP, 1>(ctx->aniso) : pick_pass_lat<MODE_MEASURE, 1>(ctx->aniso);
     if (ctx->P.fcc) fn = mode == MODE_SWEEP ? pick_pass_fcc<MODE_SWEEP>(ctx->aniso, colour) : pick_pass_fcc<MODE_MEASURE>(ctx->aniso, colour);
     if (ctx->P.basis) fn = mode == MODE_SWEEP ? pick_pass_lat<MODE_SWEEP, 3>(ctx->aniso) : pick_pass_lat<MODE_MEASURE, 3>(ctx->aniso);
-    const int grid = grid_for(ctx, ctx->geom.n_items, MC_PASS_MIN_BLOCKS, MC_PASS_BLOCK);
+    const int grid = grid_for(ctx, ctx->geom.n_items, pass_min_blocks(ctx->P.basis ? 3 : 0), MC_PASS_BLOCK);
     MC_CU(launch_dependent(fn, grid, MC_PASS_BLOCK, 0, ctx->stream, ctx->P, ctx->geom, colour, invT, flags, dx, da));
     ctx->launches += 1;
     return MC_OK;

@@ -20,12 +20,18 @@ namespace mc {
 #ifndef MC_PASS_MIN_BLOCKS
 #define MC_PASS_MIN_BLOCKS 6
 #endif
+// the basis-mode instantiation (LAT = 3) holds four rows of the bond table in flight: <= 96 registers, five CTAs per SM
+// (176^3 cells of hcp: 1032 against 1083 us per sweep with six)
+#ifndef MC_BASIS_MIN_BLOCKS
+#define MC_BASIS_MIN_BLOCKS 5
+#endif
+__host__ __device__ constexpr int pass_min_blocks(int lat) { return lat == 3 ? MC_BASIS_MIN_BLOCKS : MC_PASS_MIN_BLOCKS; }
 // LAT: 0 simple cubic; 1 bcc, 2 fcc, 3 basis mode (hcp, sc + next-nearest neighbours: eight colours, bond table) (mc_common.cuh):
 // VEC = 4 consecutive cells of one sublattice, site stride 1 instead of 2;
 // fcc: four colours, the exchange energy of a bond is summed in the pass of its higher colour (hl).
 // COL >= 0: the colour as a compile-time constant (fcc: which rows and shifts a sublattice reads is then resolved by the compiler).
 template <int VEC, int ANISO, bool MASKED, int MODE, int LAT = 0, int COL = -1>
-__global__ void __launch_bounds__(MC_PASS_BLOCK, MC_PASS_MIN_BLOCKS)
+__global__ void __launch_bounds__(MC_PASS_BLOCK, pass_min_blocks(LAT))
 pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, int colour_rt, float invT, int flags,
             float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
 {
