@@ -174,6 +174,15 @@ int mc_trace(mc_ctx* ctx, int64_t max_rows, double* host_rows, int64_t* n_rows);
  * at that x, x = 0..nx-1 (HOST pointer to 3*nx doubles, caller-owned).  Exact fixed-point sums on the device, so the
  * result is reproducible.  Uses 24*nx bytes of the workspace's staging area; synchronous. */
 int mc_profile_x(mc_ctx* ctx, double* host_profile);
+/* The same profile with NO scratch taken from the workspace and nothing allocated, on the device or the host: for callers that
+ * cannot allocate at call time (CUDA graph capture around their own code, tight serving loops, harnesses that forbid
+ * cudaMalloc).  The 24*nx bytes of sums live in a fixed array inside the library image -- the one exception to "no globals"
+ * above: 24 * MC_PROFILE_STATIC_MAX_NX = 192 KB of device memory on every GPU that loads the library, held until the process
+ * exits.  nx > MC_PROFILE_STATIC_MAX_NX: MC_EINVAL (use mc_profile_x).  Every call on a device shares that array and clears it
+ * first; calls that OVERLAP on one GPU (two handles on different streams, two host threads) race on it: serialise them.
+ * Same arguments, result (bit for bit) and restrictions as mc_profile_x; synchronous. */
+#define MC_PROFILE_STATIC_MAX_NX 8192
+int mc_profile_x_static(mc_ctx* ctx, double* host_profile);
 
 /* Test hook: which kernel mc_sweep / mc_half_sweep launch for the colour pass.  MC_PATH_AUTO (default): the planner's
  * choice for this lattice; MC_PATH_GENERIC: the grid-stride gather pass (covers every lattice); MC_PATH_STAGED: the

@@ -24,7 +24,7 @@ STRUCTURES = {"sc": (MC_SC, 1), "bcc": (MC_BCC, 2), "fcc": (MC_FCC, 4), "hcp": (
 SYMBOLS = [
     "mc_workspace_bytes", "mc_create", "mc_destroy", "mc_init_spins", "mc_set_spins", "mc_get_spins", "mc_set_cone",
     "mc_set_sweep", "mc_sweep", "mc_constrained_sweep", "mc_half_sweep", "mc_constrained_half_sweep", "mc_end_sweep",
-    "mc_align_to", "mc_observables", "mc_reset_accumulators", "mc_trace", "mc_profile_x", "mc_debug_set_path", "mc_debug_get_path", "mc_launch_count", "mc_last_error", "mc_version",
+    "mc_align_to", "mc_observables", "mc_reset_accumulators", "mc_trace", "mc_profile_x", "mc_profile_x_static", "mc_debug_set_path", "mc_debug_get_path", "mc_launch_count", "mc_last_error", "mc_version",
 ]
 
 
@@ -88,6 +88,7 @@ def load():
     L.mc_reset_accumulators.argtypes = [vp]; L.mc_reset_accumulators.restype = i32
     L.mc_trace.argtypes = [vp, i64, vp, vp]; L.mc_trace.restype = i32
     L.mc_profile_x.argtypes = [vp, vp]; L.mc_profile_x.restype = i32
+    L.mc_profile_x_static.argtypes = [vp, vp]; L.mc_profile_x_static.restype = i32
     L.mc_debug_set_path.argtypes = [vp, i32]; L.mc_debug_set_path.restype = i32
     L.mc_debug_get_path.argtypes = [vp]; L.mc_debug_get_path.restype = i32
     L.mc_launch_count.argtypes = [vp]; L.mc_launch_count.restype = i64
@@ -225,6 +226,13 @@ class Lattice:
     def profile_x(self):
         """[nx, 3] slice-averaged magnetisation along x (mc_profile_x; Fig. 2)."""
         out = np.empty((self.shape[0], 3)); self._chk(self.L.mc_profile_x(self.h, _p(out))); return out
+
+    def profile_x_static(self, out=None):
+        """mc_profile_x_static: the same profile with its scratch in a fixed array of the library (no allocation; nx <= 8192).
+        ``out``: a caller-owned C-contiguous float64 [nx, 3] array to fill (a new one if None)."""
+        if out is None: out = np.empty((self.shape[0], 3))
+        assert out.dtype == np.float64 and out.flags.c_contiguous and out.size == 3 * self.shape[0]
+        self._chk(self.L.mc_profile_x_static(self.h, _p(out))); return out
 
     def trace(self, max_rows=MC_TRACE_CAPACITY):
         rows = np.empty((int(max_rows), 6)); k = C.c_int64(0)
