@@ -49,7 +49,7 @@ bool plan_tile(mc_ctx* c)
     int RP = 1;
     for (int d = 1; d <= lat.ny; ++d) if (lat.ny % d == 0 && PR * d <= max_threads) RP = d;
     int NP = 1;
-    const size_t smem_cap = (size_t)(220 * 1024) / TILE_MIN_BLOCKS - 3 * 1024;   // TILE_MIN_BLOCKS CTAs per SM
+    const size_t smem_cap = (size_t)(220 * 1024) / TILE_MIN_BLOCKS - 3 * 1024;   // TILE_MIN_BLOCKS CTAs per SM (run-time-R shape)
     auto slot_bytes = [&](int ty) { return (size_t)3 * (ty + 2) * R * sizeof(float); };
     if (lat.ny % (2 * RP) == 0 && TILE_NSLOT * slot_bytes(2 * RP) <= smem_cap) NP = 2;
     // row lengths with a compile-time specialisation take its slab shape when it tiles ny

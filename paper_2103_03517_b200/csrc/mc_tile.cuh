@@ -34,9 +34,19 @@ constexpr int TILE_NSLOT = 4;
 constexpr int TILE_MAX_THREADS = MC_TILE_MAX_THREADS;   // launch bounds of the tiled pass: threads per CTA ...
 constexpr int TILE_MIN_BLOCKS = MC_TILE_MIN_BLOCKS;     // ... and CTAs per SM the register allocation must allow
 constexpr int TILE_NPASS_RT = 2;                        // passes (row groups) a thread of a compile-time-R specialisation covers per plane (unrolled)
-// Slab shape of the specialisation for R colour-sites per row: RP rows per pass = as many as TILE_MAX_THREADS threads cover
-// (one thread = one x-adjacent pair), at most MC_TILE_TY_RT / 2; slab height Ty = 2 RP.  R <= 112: 8 x 2 = 16 rows.
-__host__ __device__ constexpr int tile_rp_rt(int R) { return R <= 0 ? 0 : ((TILE_MAX_THREADS / (R / 2)) < (MC_TILE_TY_RT / 2) ? (TILE_MAX_THREADS / (R / 2)) : (MC_TILE_TY_RT / 2)); }
+// CTA shape of a specialisation: threads per CTA, CTAs per SM and the largest slab height.  Default 448 x 2, slabs of 16 rows.
+// R = 112 (224^3, the headline lattice): 224 x 4 with slabs of 8 rows -- the same 28 warps per SM in twice as many, smaller CTAs:
+// a CTA's per-plane barrier holds up 7 warps instead of 14 (87.7 against 89.9 us per sweep; R = 96 and 32 lose with it: 61.1
+// against 57.7 and 12.6 against 11.8 us).
+#ifndef MC_TILE_SMALL_CTA_R
+#define MC_TILE_SMALL_CTA_R 112
+#endif
+__host__ __device__ constexpr int tile_threads_rt(int R) { return R == MC_TILE_SMALL_CTA_R ? TILE_MAX_THREADS / 2 : TILE_MAX_THREADS; }
+__host__ __device__ constexpr int tile_blocks_rt(int R)  { return R == MC_TILE_SMALL_CTA_R ? 2 * TILE_MIN_BLOCKS : TILE_MIN_BLOCKS; }
+__host__ __device__ constexpr int tile_tymax_rt(int R)   { return R == MC_TILE_SMALL_CTA_R ? MC_TILE_TY_RT / 2 : MC_TILE_TY_RT; }
+// Slab shape of the specialisation for R colour-sites per row: RP rows per pass = as many as its threads cover
+// (one thread = one x-adjacent pair), at most tile_tymax_rt / 2; slab height Ty = 2 RP.  R = 32, 96: 8 x 2 = 16 rows; R = 112: 4 x 2 = 8.
+__host__ __device__ constexpr int tile_rp_rt(int R) { return R <= 0 ? 0 : ((tile_threads_rt(R) / (R / 2)) < (tile_tymax_rt(R) / 2) ? (tile_threads_rt(R) / (R / 2)) : (tile_tymax_rt(R) / 2)); }
 __host__ __device__ constexpr int tile_ty_rt(int R) { return TILE_NPASS_RT * tile_rp_rt(R); }
 // Row lengths R = nx / 2 with a specialised instantiation (every shared-memory offset an immediate, both passes unrolled).
 #ifndef MC_TILE_RT_LIST
@@ -128,7 +138,7 @@ __device__ __forceinline__ float mantissa_1p(uint32_t w) { return __uint_as_floa
 // ANTI: anti-periodic boundary along x (domain-wall box; C-27): the one x-neighbour a pair reads across the row
 // end enters with the opposite sign.  Instantiated for the run-time row length only.
 template <int ANISO, bool FIELD, int RT, bool DEBUG, bool ANTI = false>
-__global__ void __launch_bounds__(TILE_MAX_THREADS, TILE_MIN_BLOCKS)
+__global__ void __launch_bounds__(tile_threads_rt(RT), tile_blocks_rt(RT))
 tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileGeom G, int colour, float invT, int flags,
                   float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
 {
