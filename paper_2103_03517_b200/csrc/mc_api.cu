@@ -373,7 +373,7 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     DevState st; memset(&st, 0, sizeof st);
     const double deg = M_PI / 180.0;
     double cone = ham->cone0_rad; if (!(cone >= deg)) cone = deg; if (cone > M_PI) cone = M_PI;
-    st.cone = cone; st.one_minus_cos = (float)(1.0 - cos(cone)); st.adaptive = ctx->adaptive;
+    st.cone = cone; st.one_minus_cos = mc::one_minus_cos_of(cone); st.adaptive = ctx->adaptive;
     st.eC[2] = 1.0;
     ce = cudaMemcpyAsync(P.st, &st, sizeof st, cudaMemcpyHostToDevice, ctx->stream);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(ctx->stream);

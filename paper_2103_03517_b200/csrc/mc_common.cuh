@@ -486,6 +486,25 @@ __device__ __forceinline__ void block_reduce(const long long (&acc)[NQ], int cnt
     if (threadIdx.x == 0 && scnt) atomicAdd(&P.st->count, (unsigned long long)scnt);
 }
 
+// 1 - cos(cone) for the cone move (C-6), cone in [0, pi]: 2 sin^2(cone / 2) with sin from its Taylor series to h^17 (h <= pi/2:
+// truncation < 5e-14, far below the fp32 it is rounded to).  Straight-line fma code, the same bits on the host (mc_create) and on
+// the device (mc_set_cone, end-of-sweep controller): the library routine cos() in fp64 is a call into cold code with table
+// look-ups on the one thread the whole grid waits for -- 0.8-2 us per sweep at the tail of the last colour pass.
+__host__ __device__ inline float one_minus_cos_of(double cone)
+{
+    const double h = 0.5 * cone, z = h * h;
+    double p = -1.0 / 355687428096000.0;                       // -1/17!
+    p = fma(p, z, 1.0 / 1307674368000.0);                       // +1/15!
+    p = fma(p, z, -1.0 / 6227020800.0);                         // -1/13!
+    p = fma(p, z, 1.0 / 39916800.0);                            // +1/11!
+    p = fma(p, z, -1.0 / 362880.0);                             // -1/9!
+    p = fma(p, z, 1.0 / 5040.0);                                // +1/7!
+    p = fma(p, z, -1.0 / 120.0);                                // -1/5!
+    p = fma(p, z, 1.0 / 6.0);                                   // +1/3!  (sign folded below)
+    const double s = h * fma(-p, z, 1.0);                       // sin h = h (1 - z/3! + z^2/5! - ...)
+    return (float)(2.0 * s * s);
+}
+
 // Pass 2 of the reduction (one block, fixed order) + what follows a sweep: cone controller (P:168-171 read with
 // P:205-209; C-2, C-3, C-9), sweep counter, Eq. (6) accumulators, trace row.  mode 0: end of a sweep; 1: measurement.
 // Pass 1 left exact fixed-point totals in DevState.isum; here they become fp64.  This block runs alone at the tail of
@@ -510,7 +529,7 @@ static __device__ __noinline__ void final_reduce(const Params& P, int mode, int 
         double up = sst.cone + deg; if (up > pi) up = pi;
         double dn = sst.cone - deg; if (dn < deg) dn = deg;
         cone_next[0] = up; cone_next[1] = dn;
-        omc_next[0] = (float)(1.0 - cos(up)); omc_next[1] = (float)(1.0 - cos(dn));
+        omc_next[0] = one_minus_cos_of(up); omc_next[1] = one_minus_cos_of(dn);
     }
     double s[NQ];
     if (threadIdx.x == 0) {

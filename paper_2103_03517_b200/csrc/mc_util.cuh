@@ -128,7 +128,7 @@ __global__ void rotate_kernel(const __grid_constant__ Params P, const __grid_con
 enum : int { ST_CONE = 0, ST_SWEEP = 1, ST_RESET_ACC = 2, ST_EC = 3, ST_ML = 4, ST_RESET_SWEEP = 5 };
 __global__ void state_kernel(DevState* st, int what, double a, double b, double c, unsigned long long u)
 {
-    if (what == ST_CONE) { st->cone = a; st->one_minus_cos = (float)(1.0 - cos(a)); }
+    if (what == ST_CONE) { st->cone = a; st->one_minus_cos = one_minus_cos_of(a); }
     else if (what == ST_SWEEP) { st->sweep = u; }
     else if (what == ST_RESET_ACC) {
         st->n_samples = 0ull;
