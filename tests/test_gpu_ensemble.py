@@ -340,6 +340,74 @@ def test_full_size_march_pass_half_sweep_parity(mods):
     _full_size_half_sweep(mods, (256, 256, 256), 1.2, 1.2, 7, dict(Kc=0.01), colour=1)
 
 
+# ---------------------------------------------------------------------------------------------- f-2 lattices at bench size
+@pytest.mark.parametrize("structure,L,T,colour,ham", [
+    ("bcc", 176, 1.8, 1, dict()),                    # 10.9 M spins, 8 neighbours
+    ("fcc", 140, 2.8, 3, dict()),                    # 11.0 M spins, 12 neighbours, four colours
+    ("hcp", 176, 2.8, 5, dict()),                    # 43.6 M spins, 12 neighbours through the bond table, eight colours
+    ("sc_nnn", 176, 2.0, 2, dict(J2=0.3)),           # 43.6 M spins, 6 + 12 neighbours
+])
+def test_full_size_sublattice_lattices_at_the_sizes_bench_times(mods, structure, L, T, colour, ham):
+    """The lattices of bench.py's `other_paths` at the sizes and in the launch configuration it times: the library
+    runs 12 sweeps at T from the seeded random-sphere start with the adaptive cone (as the bench does), then ONE colour pass from
+    that state, with that cone and sweep counter, is compared with the oracle site by site (C-14 bar)."""
+    oracle, binding, inputs = mods
+    g = binding.Lattice(L, L, L, Ku=0.01, cone0=0.5, adaptive=True, seed=42, structure=structure, **ham)
+    g.init_spins(2); g.sweep(T, 12)
+    ob = g.observables()
+    o = oracle.Oracle(L, L, L, Ku=0.01, cone0=ob.cone_rad, adaptive=False, seed=42, structure=structure, **ham)
+    o.set_sweep(ob.sweep)
+    before = g.get_spins(); o.set_spins(before)
+    _, x_o, acc_o = o.half_sweep(T, colour, want_detail=True)
+    x_g, acc_g = g.half_sweep(T, colour, want_detail=True)
+    after_g = g.get_spins(); after_o = o.get_spins()
+    nc = L ** 3
+    mine = np.zeros(g.N, bool); mine[colour * nc:(colour + 1) * nc] = True
+    differ = mine & (acc_g != acc_o)
+    assert (np.abs(x_o[differ]) < 1e-5).all()
+    agree = mine & ~differ
+    assert np.abs(after_g[agree].astype(np.float64) - after_o[agree]).max() < 1e-4
+    assert (after_g[~mine] == before[~mine]).all()
+    near = mine & (np.abs(x_o) < 2.0)
+    dx = np.abs(x_g[near] - x_o[near]).max()
+    print(f"\n{structure} {L}^3 cells T={T} cone={ob.cone_rad:.3f} colour {colour}: {nc} updates, accepted {acc_g[mine].mean():.3f}, "
+          f"marginal flips {differ.sum()}, max |dx| near the boundary {dx:.2e}")
+    assert dx < 1e-5 and differ.sum() < 50
+    g.close()
+
+
+def test_full_size_bcc_constrained_half_sweep_parity(mods):
+    """The constrained pair pass on the 176^3-cell bcc lattice bench.py times (Table A2 with the 8-bond field): after 12
+    constrained sweeps of the library, one pair pass of sublattice B against the oracle: same pairs decided the same way outside
+    the band, both members of every agreeing pair to 1e-4."""
+    oracle, binding, inputs = mods
+    L, T, theta, phi = 176, 0.8, 0.6, 0.0
+    e = np.array([np.sin(theta) * np.cos(phi), np.sin(theta) * np.sin(phi), np.cos(theta)])
+    g = binding.Lattice(L, L, L, Ku=0.01, cone0=0.5, adaptive=True, seed=42, structure="bcc")
+    g.constrained_sweep(T, theta, phi, 12)
+    ob = g.observables()
+    o = oracle.Oracle(L, L, L, Ku=0.01, cone0=ob.cone_rad, adaptive=False, seed=42, structure="bcc")
+    o.set_sweep(ob.sweep)
+    before = g.get_spins(); o.set_spins(before)
+    ML = float((before.astype(np.float64) @ e).sum())
+    colour, nc = 1, L ** 3
+    _, _, x_o, acc_o = o.constrained_half_sweep(T, e, colour, ML, want_detail=True)
+    x_g, acc_g = g.constrained_half_sweep(T, theta, phi, colour, ML, want_detail=True)
+    after_g = g.get_spins().astype(np.float64); after_o = o.get_spins()
+    partner, lead = o.pairing(int(ob.sweep), colour)
+    la = np.nonzero(lead)[0]
+    lead_sites, foll_sites = colour * nc + la, colour * nc + partner[la]
+    assert not np.isnan(x_g[lead_sites]).any() and np.isnan(x_g[foll_sites]).all()
+    assert (acc_g[lead_sites] == acc_g[foll_sites]).all()
+    differ = acc_g[lead_sites] != acc_o[lead_sites]
+    assert (np.abs(x_o[lead_sites][differ]) < 1e-5).all() and differ.sum() < 50
+    for sites in (lead_sites[~differ], foll_sites[~differ]):
+        assert np.abs(after_g[sites] - after_o[sites]).max() < 1e-4
+    assert (after_g[:nc] == before[:nc].astype(np.float64)).all()
+    print(f"\nbcc constrained 176^3 cells: {len(la)} pairs, accepted {acc_g[lead_sites].mean():.3f}, marginal flips {differ.sum()}")
+    g.close()
+
+
 # ---------------------------------------------------------------------------------------------- maximum size
 def test_maximum_size_lattice_sampled_parity_and_path_equality(mods):
     """The largest lattice the boundary accepts (N < 2^31, include/mc.h): 1280 x 1280 x 1310 = 2 146 304 000 spins, 25.8 GB of state
