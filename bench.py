@@ -228,7 +228,7 @@ def time_other_paths(binding, torch, local_rank, sweeps=100):
         ms = e0.elapsed_time(e1)
         ups = g.N * sweeps / (ms * 1e-3)
         out[f"{name}_176^3_cells_Ku0.01_T{T}"] = {"value": ups, "unit": UNIT, "us_per_sweep": 1e3 * ms / sweeps, "algorithmic_GBs": 96 * ups / 1e9,
-                                              "kernel": "pass_kernel<4, uniaxial, basis> (gather through the bond table, rows of cells merged: 12 / 18 bonds, 8 passes per sweep; 96 B per update)"}
+                                              "kernel": "pass_kernel<4, uniaxial, structure, colour> (gather through the bond table of the sublattice as a compile-time constant: 12 / 18 bonds, 8 passes per sweep; 96 B per update)"}
         g.close()
     return out
 

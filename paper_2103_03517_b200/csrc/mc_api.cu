@@ -31,45 +31,19 @@ bool needs_mask(const mc_lattice* lat, const mc_hamiltonian* ham)
 
 int n_sublattices(int structure) { return structure == MC_BCC ? 2 : structure == MC_FCC ? 4 : (structure == MC_HCP || structure == MC_SC_NNN) ? 8 : 0; }
 
-// basis mode (C-32): the bonds of a site of every sublattice, found from the coordinates -- every (sublattice, cell offset in
-// {-1,0,1}^3) whose separation has the bonding length, grouped by the row of cells (sublattice, dy, dz) they reach.  hcp: orthohexagonal cell doubled along x, units (a/2, sqrt3 a/6, c/2),
-// ideal c/a: |r|^2 = a^2/12 (3 dx^2 + dy^2 + 8 dz^2), nearest neighbours at |r| = a.  sc + next-nearest neighbours: the
-// 2 x 2 x 2 block as the cell, |r|^2 = 1 (J) and 2 (J2).  Returns false if a bond stays inside a sublattice.
+// basis mode (C-32): the run-time copy of the bond table (make_bond_table, mc_common.cuh: derived from the coordinates) with the
+// couplings filled in.  Returns false if a bond stays inside a sublattice.
 bool build_bond_table(int structure, float J, float J2, mc::BondEntry (*tab)[mc::MC_MAX_BONDS], unsigned char* n, unsigned char* n_lower)
 {
-    static const int hcp_pos[8][3] = { { 0, 0, 0 }, { 1, 3, 0 }, { 1, 1, 1 }, { 0, 4, 1 }, { 2, 0, 0 }, { 3, 3, 0 }, { 3, 1, 1 }, { 2, 4, 1 } };
-    const bool hcp = structure == MC_HCP;
-    const int cell[3] = { hcp ? 4 : 2, hcp ? 6 : 2, 2 }, w[3] = { hcp ? 3 : 1, 1, hcp ? 8 : 1 };
     for (int a = 0; a < 8; ++a) {
-        int rows = 0, bonds = 0, lower = 0;
-        for (int pass = 0; pass < 2; ++pass)                                 // rows into lower sublattices first
-            for (int b = 0; b < 8; ++b) {
-                if ((b < a) != (pass == 0)) continue;
-                for (int o = 0; o < 9; ++o) {
-                    const int dy = o % 3 - 1, dz = o / 3 - 1;
-                    int mask = 0; float Jb = 0.0f;
-                    for (int dx = -1; dx <= 1; ++dx) {
-                        const int d[3] = { dx, dy, dz };
-                        int q = 0;
-                        for (int ax = 0; ax < 3; ++ax) {
-                            const int ra = hcp ? hcp_pos[a][ax] : (a >> ax) & 1, rb = hcp ? hcp_pos[b][ax] : (b >> ax) & 1;
-                            const int sep = rb + d[ax] * cell[ax] - ra;
-                            q += w[ax] * sep * sep;
-                        }
-                        if (hcp) { if (q != 12) continue; Jb = J; }
-                        else if (q == 1) Jb = J; else if (q == 2) Jb = J2; else continue;
-                        if (b == a) return false;
-                        mask |= 1 << (dx + 1); ++bonds;
-                    }
-                    if (!mask) continue;
-                    if (rows == mc::MC_MAX_BONDS) return false;
-                    tab[a][rows].b = (signed char)b; tab[a][rows].xmask = (signed char)mask; tab[a][rows].dy = (signed char)dy; tab[a][rows].dz = (signed char)dz;
-                    tab[a][rows].J = Jb; ++rows;
-                    if (b < a) ++lower;
-                }
-            }
-        if (bonds != (hcp ? 12 : 18)) return false;
-        n[a] = (unsigned char)rows; n_lower[a] = (unsigned char)lower;
+        const mc::BondTableCT T = mc::make_bond_table(structure, a);
+        if (!T.ok) return false;
+        for (int r = 0; r < T.n; ++r) {
+            tab[a][r].b = (signed char)T.row[r].b; tab[a][r].xmask = (signed char)T.row[r].xmask;
+            tab[a][r].dy = (signed char)T.row[r].dy; tab[a][r].dz = (signed char)T.row[r].dz;
+            tab[a][r].J = T.row[r].kind == 1 ? J : J2;
+        }
+        n[a] = (unsigned char)T.n; n_lower[a] = (unsigned char)T.nlower;
     }
     return true;
 }
@@ -261,7 +235,7 @@ int mc_create(const mc_lattice* lat, const mc_hamiltonian* ham, uint64_t seed,
     P.per_mask = (lat->periodic[0] ? 1 : 0) | (lat->periodic[1] ? 2 : 0) | (lat->periodic[2] ? 4 : 0);
     P.plane = L.plane; P.S = (float*)(ws + L.spins);
     P.mask = nullptr; P.mask_plane = L.mask_plane; P.region = nullptr; P.region_plane = L.region_plane; P.axis = nullptr;
-    P.J = (float)ham->J; P.Ku = (float)ham->Ku; P.Kc = (float)ham->Kc;
+    P.J = (float)ham->J; P.Ku = (float)ham->Ku; P.Kc = (float)ham->Kc; P.J2 = (float)ham->J2;
     for (int a = 0; a < 3; ++a) { P.eu[a] = (float)ctx->eu[a]; P.B[a] = (float)ham->B[a]; }
     P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32);
     P.key = philox_key(P.seed_lo, P.seed_hi);

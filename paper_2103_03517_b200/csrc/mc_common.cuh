@@ -47,6 +47,58 @@ struct DevState {
 // bond length).  Rows into sublattices b < a come first (n_lower of them): their partial field is the part of E_exch this pass owns.
 constexpr int MC_MAX_BONDS = 18;
 struct BondEntry { signed char b, xmask, dy, dz; float J; };
+// The same table before the couplings are filled in, derived from the coordinates -- every (sublattice b, cell offset in {-1,0,1}^3)
+// whose separation from a site of sublattice a has a bonding length.  hcp (structure 3): orthohexagonal cell doubled along x,
+// units (a/2, sqrt3 a/6, c/2), ideal c/a: |r|^2 = a^2/12 (3 dx^2 + dy^2 + 8 dz^2), nearest neighbours at |r| = a (kind 1).
+// sc + next-nearest neighbours (structure 4): the 2 x 2 x 2 block as the cell, |r|^2 = 1 (kind 1: J) and 2 (kind 2: J2).
+// constexpr: mc_api.cu evaluates it at run time for the table it uploads, the compile-time instantiations of the pass evaluate it
+// in the compiler.  ok = false if a bond stays inside the sublattice or the bond count is not 12 / 18.
+struct BondRowCT { int b, xmask, dy, dz, kind; };
+struct BondTableCT { BondRowCT row[MC_MAX_BONDS]; int n, nlower; bool ok; };
+__host__ __device__ constexpr int hcp_basis_pos(int s, int ax)
+{
+    // (0,0,0) (1,3,0) (1,1,1) (0,4,1) and the same + (2,0,0)
+    const int x = ((s & 3) == 1 || (s & 3) == 2 ? 1 : 0) + (s >= 4 ? 2 : 0);
+    const int y = (s & 3) == 0 ? 0 : (s & 3) == 1 ? 3 : (s & 3) == 2 ? 1 : 4;
+    const int z = (s & 3) >= 2 ? 1 : 0;
+    return ax == 0 ? x : ax == 1 ? y : z;
+}
+__host__ __device__ constexpr BondTableCT make_bond_table(int structure, int a)
+{
+    BondTableCT T{};
+    const bool hcp = structure == 3;
+    const int cell[3] = { hcp ? 4 : 2, hcp ? 6 : 2, 2 }, w[3] = { hcp ? 3 : 1, 1, hcp ? 8 : 1 };
+    int rows = 0, bonds = 0, lower = 0;
+    bool ok = true;
+    for (int pass = 0; pass < 2; ++pass)                                 // rows into lower sublattices first
+        for (int b = 0; b < 8; ++b) {
+            if ((b < a) != (pass == 0)) continue;
+            for (int o = 0; o < 9; ++o) {
+                const int dy = o % 3 - 1, dz = o / 3 - 1;
+                int mask = 0, kind = 0;
+                for (int dx = -1; dx <= 1; ++dx) {
+                    const int d[3] = { dx, dy, dz };
+                    int q = 0;
+                    for (int ax = 0; ax < 3; ++ax) {
+                        const int ra = hcp ? hcp_basis_pos(a, ax) : (a >> ax) & 1, rb = hcp ? hcp_basis_pos(b, ax) : (b >> ax) & 1;
+                        const int sep = rb + d[ax] * cell[ax] - ra;
+                        q += w[ax] * sep * sep;
+                    }
+                    if (hcp) { if (q != 12) continue; kind = 1; }
+                    else if (q == 1) kind = 1; else if (q == 2) kind = 2; else continue;
+                    if (b == a) ok = false;
+                    mask |= 1 << (dx + 1); ++bonds;
+                }
+                if (!mask) continue;
+                if (rows == MC_MAX_BONDS) { ok = false; continue; }
+                T.row[rows].b = b; T.row[rows].xmask = mask; T.row[rows].dy = dy; T.row[rows].dz = dz; T.row[rows].kind = kind;
+                ++rows;
+                if (b < a) ++lower;
+            }
+        }
+    T.n = rows; T.nlower = lower; T.ok = ok && bonds == (hcp ? 12 : 18);
+    return T;
+}
 
 struct Params {
     int nx, ny, nz, R;               // R = nx/2 sites of one colour per row
@@ -68,6 +120,7 @@ struct Params {
     const uint16_t* region; long long region_plane;  // [2][region_plane] colour-split grain ids (or null)
     const float4* axis;              // [n_regions] easy axes
     float J, Ku, Kc;
+    float J2;                        // next-nearest-neighbour coupling (MC_SC_NNN)
     float eu[3], B[3];
     uint32_t seed_lo, seed_hi;
     PhiloxKey key;                   // the 10 round keys of (seed_lo, seed_hi), filled by the host: constant-bank operands
@@ -415,6 +468,54 @@ __device__ __forceinline__ void basis_exchange_field(const Params& P, const FccP
     for (int k = 0; k < 4; ++k) hl[k] = { hc[0][k], hc[1][k], hc[2][k] };
 #pragma unroll UNR
     for (int e = nlow; e < n; ++e) row(e);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) h[k] = { hc[0][k], hc[1][k], hc[2][k] };
+}
+
+// The same field with the table as a compile-time constant (STRUCT 3 hcp / 4 sc + next-nearest neighbours, COL the sublattice):
+// the rows are unrolled, the wrapped y / z indices are computed once, a row loads the cells outside the item only where it has a
+// bond to them, and the neighbours of a row are summed before ONE multiplication by its coupling.
+template <int STRUCT, int COL, int ROW>
+__device__ __forceinline__ void basis_rows_ct(const Params& P, const FccPos& q, const uint32_t (&yy)[3], const uint32_t (&zz)[3],
+                                              uint32_t xm, uint32_t xp, float (&hc)[3][4], Vec3 (&hl)[4])
+{
+    constexpr BondTableCT T = make_bond_table(STRUCT, COL);
+    static_assert(T.ok, "basis mode: a bond inside a sublattice");
+    if constexpr (ROW == T.nlower) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) hl[k] = { hc[0][k], hc[1][k], hc[2][k] };
+    }
+    if constexpr (ROW < T.n) {
+        constexpr BondRowCT r = T.row[ROW];
+        const float J = r.kind == 1 ? P.J : P.J2;
+        const float* O = P.S + (long long)r.b * 3 * P.plane + (zz[r.dz + 1] * (uint32_t)P.ny + yy[r.dy + 1]) * (uint32_t)P.nx;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const float* Oc = O + (long long)c * P.plane;
+            const Pack<4> o = ld_nc<4>(Oc + q.i0);
+            float s[4] = { 0.f, 0.f, 0.f, 0.f };
+            if constexpr ((r.xmask & 2) != 0) { s[0] = o.v[0]; s[1] = o.v[1]; s[2] = o.v[2]; s[3] = o.v[3]; }
+            if constexpr ((r.xmask & 1) != 0) { const float em = __ldg(Oc + xm); s[0] += em; s[1] += o.v[0]; s[2] += o.v[1]; s[3] += o.v[2]; }
+            if constexpr ((r.xmask & 4) != 0) { const float ep = __ldg(Oc + xp); s[0] += o.v[1]; s[1] += o.v[2]; s[2] += o.v[3]; s[3] += ep; }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) hc[c][k] = fmaf(J, s[k], hc[c][k]);
+        }
+        basis_rows_ct<STRUCT, COL, ROW + 1>(P, q, yy, zz, xm, xp, hc, hl);
+    }
+}
+template <int STRUCT, int COL>
+__device__ __forceinline__ void basis_exchange_field_ct(const Params& P, const FccPos& q, Vec3 (&h)[4], Vec3 (&hl)[4])
+{
+    const uint32_t nx = (uint32_t)P.nx, ny = (uint32_t)P.ny, nz = (uint32_t)P.nz;
+    const uint32_t yy[3] = { q.y == 0 ? ny - 1 : q.y - 1, q.y, q.y + 1 == ny ? 0u : q.y + 1 };
+    const uint32_t zz[3] = { q.z == 0 ? nz - 1 : q.z - 1, q.z, q.z + 1 == nz ? 0u : q.z + 1 };
+    const uint32_t xm = q.i0 == 0 ? nx - 1 : q.i0 - 1, xp = q.i0 + 4 == nx ? 0u : q.i0 + 4;
+    float hc[3][4];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int k = 0; k < 4; ++k) hc[c][k] = 0.0f;
+    basis_rows_ct<STRUCT, COL, 0>(P, q, yy, zz, xm, xp, hc, hl);
 #pragma unroll
     for (int k = 0; k < 4; ++k) h[k] = { hc[0][k], hc[1][k], hc[2][k] };
 }

@@ -75,6 +75,10 @@ inline int grid_for(const mc_ctx* c, uint32_t n_threads_needed, int resident_per
 
 // ---- mc_pass.cu: generic colour pass / standalone measurement (any lattice)
 int launch_pass_generic(mc_ctx* ctx, int mode, int colour, float invT, int flags, float* dx, uint8_t* da);
+// ---- mc_basis_hcp.cu / mc_basis_nnn.cu: the sweep passes of the eight-colour lattices with compile-time bond tables
+typedef void (*PassFn)(const Params, const Geom, int, float, int, float*, uint8_t*);
+PassFn pick_pass_basis_hcp(int aniso, int colour);
+PassFn pick_pass_basis_nnn(int aniso, int colour);
 // ---- mc_pair.cu: constrained pair pass
 int launch_pair_generic(mc_ctx* ctx, int colour, float invT, int flags, float* dx, uint8_t* da);
 // ---- mc_march.cu: register-carried z-march colour pass; plan_march fills ctx->march_* at creation

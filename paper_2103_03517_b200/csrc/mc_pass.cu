@@ -5,7 +5,7 @@
 namespace mc {
 namespace {
 
-typedef void (*PassFn)(const Params, const Geom, int, float, int, float*, uint8_t*);
+
 
 template <int VEC, int MODE> PassFn pick_pass(int aniso, bool masked)
 {
@@ -48,7 +48,11 @@ int launch_pass_generic(mc_ctx* ctx, int mode, int colour, float invT, int flags
                                 : (mode == MODE_SWEEP ? pick_pass<1, MODE_SWEEP>(ctx->aniso, ctx->masked) : pick_pass<1, MODE_MEASURE>(ctx->aniso, ctx->masked));
     if (ctx->P.bcc) fn = mode == MODE_SWEEP ? pick_pass_lat<MODE_SWEEP, 1>(ctx->aniso) : pick_pass_lat<MODE_MEASURE, 1>(ctx->aniso);
     if (ctx->P.fcc) fn = mode == MODE_SWEEP ? pick_pass_fcc<MODE_SWEEP>(ctx->aniso, colour) : pick_pass_fcc<MODE_MEASURE>(ctx->aniso, colour);
-    if (ctx->P.basis) fn = mode == MODE_SWEEP ? pick_pass_lat<MODE_SWEEP, 3>(ctx->aniso) : pick_pass_lat<MODE_MEASURE, 3>(ctx->aniso);
+    // eight-colour lattices: sweeps through the compile-time tables, unless the test hook forces the run-time table (MC_PATH_GENERIC);
+    // the stand-alone measurement reads the run-time table
+    if (ctx->P.basis) fn = mode != MODE_SWEEP ? pick_pass_lat<MODE_MEASURE, 3>(ctx->aniso)
+                         : ctx->path == MC_PATH_GENERIC ? pick_pass_lat<MODE_SWEEP, 3>(ctx->aniso)
+                         : ctx->P.basis == MC_HCP ? pick_pass_basis_hcp(ctx->aniso, colour) : pick_pass_basis_nnn(ctx->aniso, colour);
     const int grid = grid_for(ctx, ctx->geom.n_items, pass_min_blocks(ctx->P.basis ? 3 : 0), MC_PASS_BLOCK);
     MC_CU(launch_dependent(fn, grid, MC_PASS_BLOCK, 0, ctx->stream, ctx->P, ctx->geom, colour, invT, flags, dx, da));
     ctx->launches += 1;

@@ -25,8 +25,9 @@ namespace mc {
 #ifndef MC_BASIS_MIN_BLOCKS
 #define MC_BASIS_MIN_BLOCKS 5
 #endif
-__host__ __device__ constexpr int pass_min_blocks(int lat) { return lat == 3 ? MC_BASIS_MIN_BLOCKS : MC_PASS_MIN_BLOCKS; }
-// LAT: 0 simple cubic; 1 bcc, 2 fcc, 3 basis mode (hcp, sc + next-nearest neighbours: eight colours, bond table) (mc_common.cuh):
+__host__ __device__ constexpr int pass_min_blocks(int lat) { return lat >= 3 ? MC_BASIS_MIN_BLOCKS : MC_PASS_MIN_BLOCKS; }
+// LAT: 0 simple cubic; 1 bcc, 2 fcc, 3 / 4 basis mode (hcp / sc + next-nearest neighbours: eight colours, bond table; with
+// COL < 0 the run-time table of either structure under LAT = 3, with COL >= 0 the compile-time table of structure LAT) (mc_common.cuh):
 // VEC = 4 consecutive cells of one sublattice, site stride 1 instead of 2;
 // fcc: four colours, the exchange energy of a bond is summed in the pass of its higher colour (hl).
 // COL >= 0: the colour as a compile-time constant (fcc: which rows and shifts a sublattice reads is then resolved by the compiler).
@@ -57,7 +58,7 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
         constexpr uint32_t SS = LAT ? 1u : 2u;                    // site-id stride between the sites of an item
         ItemPos q;
         Vec3 h[VEC], e[VEC], hl[LAT >= 2 ? VEC : 1];
-        const float Jm = LAT == 3 ? 1.0f : P.J;                   // basis mode: the couplings are already in h, hl
+        const float Jm = LAT >= 3 ? 1.0f : P.J;                   // basis mode: the couplings are already in h, hl
         if (LAT == 1) {
             const BccPos b = bcc_locate(P, G, item, colour);
             q.a0 = b.a0; q.site0 = b.site0; q.xh0 = b.i0; q.par = 0u;
@@ -66,10 +67,12 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
             const FccPos b = fcc_locate(P, G, item, colour);
             q.a0 = b.a0; q.site0 = b.site0; q.xh0 = b.i0; q.par = 0u;
             if (VEC == 4) fcc_exchange_field(P, b, colour, reinterpret_cast<Vec3(&)[4]>(h), reinterpret_cast<Vec3(&)[4]>(hl));
-        } else if (LAT == 3) {
+        } else if (LAT >= 3) {
             const FccPos b = fcc_locate(P, G, item, colour);
             q.a0 = b.a0; q.site0 = b.site0; q.xh0 = b.i0; q.par = 0u;
-            if (VEC == 4) basis_exchange_field(P, b, colour, reinterpret_cast<Vec3(&)[4]>(h), reinterpret_cast<Vec3(&)[4]>(hl));
+            if constexpr (VEC == 4 && LAT >= 3 && COL >= 0)        // structure LAT and sublattice COL fixed at compile time: unrolled table
+                basis_exchange_field_ct<LAT, COL>(P, b, reinterpret_cast<Vec3(&)[4]>(h), reinterpret_cast<Vec3(&)[4]>(hl));
+            else if (VEC == 4) basis_exchange_field(P, b, colour, reinterpret_cast<Vec3(&)[4]>(h), reinterpret_cast<Vec3(&)[4]>(hl));
         } else {
             q = locate<VEC>(P, G, item, colour);
             exchange_field<VEC, MASKED>(P, q, colour, h);

@@ -62,10 +62,18 @@ CASES = [
 ]
 
 
+@pytest.mark.parametrize("structure,shape,T,cone,ham", [CASES[0], CASES[3], CASES[5], CASES[8]])
+def test_basis_half_sweep_parity_with_the_run_time_bond_table(mods, structure, shape, T, cone, ham):
+    """The sweep passes default to the instantiations with compile-time bond tables; MC_PATH_GENERIC forces the one that reads
+    the table mc_create uploaded (the stand-alone measurement always does)."""
+    test_basis_half_sweep_parity(mods, structure, shape, T, cone, ham, path=1)
+
+
 @pytest.mark.parametrize("structure,shape,T,cone,ham", CASES)
-def test_basis_half_sweep_parity(mods, structure, shape, T, cone, ham):
+def test_basis_half_sweep_parity(mods, structure, shape, T, cone, ham, path=None):
     oracle, binding, inputs = mods
     o, g = _pair(mods, structure, shape, cone=cone, sweep=(5 << 32) | 777, **ham)
+    if path is not None: g.debug_set_path(path)
     g.set_spins(inputs.random_unit_spins(g.N, seed=8))
     worst = 0.0
     for colour in (0, 1, 2, 3, 4, 5, 6, 7, 2, 5):
