@@ -230,6 +230,28 @@ def time_other_paths(binding, torch, local_rank, sweeps=100):
         out[f"{name}_176^3_cells_Ku0.01_T{T}"] = {"value": ups, "unit": UNIT, "us_per_sweep": 1e3 * ms / sweeps, "algorithmic_GBs": 96 * ups / 1e9,
                                               "kernel": "pass_kernel<4, uniaxial, structure, colour> (gather through the bond table of the sublattice as a compile-time constant: 12 / 18 bonds, 8 passes per sweep; 96 B per update)"}
         g.close()
+    # c2 (BASELINE.json configs[1]): 16 temperature points of 64^3.  A 64^3 colour pass fills a fraction of the GPU and a sweep is two
+    # ~5 us launches whatever the size: one after another the points run launch-bound; replicas.run_points_concurrent runs them all
+    # at once, one stream each, their sweeps replayed as CUDA graphs (same results bit for bit: tests/test_gpu_replicas.py).
+    # Wall-clock around a synchronised region (16 streams), 1000 sweeps per point.
+    from paper_2103_03517_b200 import replicas
+    pts = [(0.1 * k, 64, 500, 500) for k in range(1, 17)]
+    mk = lambda p, seed, device, stream: binding.Lattice(p[1], p[1], p[1], Ku=0.01, cone0=0.5, adaptive=True, seed=seed, device=device, stream=stream)
+    ph = lambda p: [("sweep", p[0], p[2]), ("reset",), ("sweep", p[0], p[3])]
+    def fin(g, p):
+        m = g.observables().m; g.close(); return m
+    dev = f"cuda:{local_rank}"
+    replicas.run_points_concurrent(pts[:2], mk, ph, fin, device=dev)                     # warm-up (module load, graph machinery)
+    torch.cuda.synchronize(); t0 = time.perf_counter()
+    replicas.run_points_concurrent(pts, mk, ph, fin, device=dev)
+    torch.cuda.synchronize(); t_conc = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    for k, p in enumerate(pts):
+        g = mk(p, 43 + k, dev, None); g.sweep(p[0], p[2]); g.reset_accumulators(); g.sweep(p[0], p[3]); fin(g, p)
+    torch.cuda.synchronize(); t_ser = time.perf_counter() - t0
+    work = 16 * 64 ** 3 * 1000
+    out["c2_16_points_64^3_concurrent"] = {"value": work / t_conc, "unit": UNIT, "seconds": t_conc, "one_after_another": work / t_ser,
+                                           "kernel": "tile_pass_kernel<1, 0, 32> on 16 streams, 50-sweep CUDA graphs replayed round robin; wall clock incl. handle creation, capture and read-back"}
     return out
 
 

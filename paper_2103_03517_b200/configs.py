@@ -45,10 +45,33 @@ def _c2_point(point, seed, device):
     return {"m": ob.sum_m[0] / ob.n_samples, "chi_l": float(chi[0]), "chi_t": float(0.5 * (chi[1] + chi[2]))}
 
 
-def c2(device=None, L=64, equil=5000, sample=5000, dist=None):
-    """16 independent temperature points: dealt over the ranks by replicas.run_points (one rank: the plain loop)."""
+def _c2_create(point, seed, device, stream):
+    T, L, equil, sample = point
+    return binding.Lattice(L, L, L, Ku=0.01, cone0=0.5, adaptive=True, seed=seed, device=device, stream=stream)
+
+
+def _c2_phases(point):
+    T, L, equil, sample = point
+    return [("sweep", T, equil), ("reset",), ("sweep", T, sample)]
+
+
+def _c2_collect(g, point):
+    ob = g.observables()
+    chi = analysis.susceptibilities(ob, point[0])
+    g.close()
+    return {"m": ob.sum_m[0] / ob.n_samples, "chi_l": float(chi[0]), "chi_t": float(0.5 * (chi[1] + chi[2]))}
+
+
+def c2(device=None, L=64, equil=5000, sample=5000, dist=None, concurrent=True):
+    """16 independent temperature points: dealt over the ranks by replicas.run_points (several ranks), or -- one process, the default
+    -- all at once on one device, one stream each, their sweeps replayed as CUDA graphs (replicas.run_points_concurrent; the same
+    numbers bit for bit)."""
     Ts = [0.1 * k for k in range(1, 17)]
-    res = replicas.run_points([(T, L, equil, sample) for T in Ts], _c2_point, base_seed=42, dist=dist, device=device)
+    pts = [(T, L, equil, sample) for T in Ts]
+    if dist is None and concurrent:
+        res = replicas.run_points_concurrent(pts, _c2_create, _c2_phases, _c2_collect, device=device or "cuda:0", base_seed=42)
+    else:
+        res = replicas.run_points(pts, _c2_point, base_seed=42, dist=dist, device=device)
     if res is None:
         return None                                           # not rank 0
     m, chi_l, chi_t = [r["m"] for r in res], [r["chi_l"] for r in res], [r["chi_t"] for r in res]
@@ -87,11 +110,31 @@ def _c4_point(point, seed, device):
     return {"tau_y": ob.sum_torque[1] / ob.n_samples, "m": ob.sum_m[0] / ob.n_samples}
 
 
-def c4(device=None, L=128, sweeps=5000, discard=1000, dist=None):
-    """33 independent (T, theta) points through replicas.run_points."""
+def _c4_create(point, seed, device, stream):
+    return binding.Lattice(point[2], point[2], point[2], Ku=0.05, cone0=0.5, adaptive=True, seed=42, device=device, stream=stream)
+
+
+def _c4_phases(point):
+    T, th, L, sweeps, discard = point
+    return [("constrained", T, th, 0.0, discard), ("reset",), ("constrained", T, th, 0.0, sweeps - discard)]
+
+
+def _c4_collect(g, point):
+    ob = g.observables()
+    g.close()
+    return {"tau_y": ob.sum_torque[1] / ob.n_samples, "m": ob.sum_m[0] / ob.n_samples}
+
+
+def c4(device=None, L=128, sweeps=5000, discard=1000, dist=None, concurrent=True):
+    """33 independent (T, theta) points through replicas.run_points (several ranks) or, one process, concurrently on one device
+    (replicas.run_points_concurrent, 11 at a time)."""
     thetas = np.deg2rad(np.arange(0, 91, 9))                  # 0..90 deg in 10 steps (C-20)
     temps = (0.3, 0.8, 1.2)
-    res = replicas.run_points([(T, float(th), L, sweeps, discard) for T in temps for th in thetas], _c4_point, base_seed=42, dist=dist, device=device)
+    pts = [(T, float(th), L, sweeps, discard) for T in temps for th in thetas]
+    if dist is None and concurrent:
+        res = replicas.run_points_concurrent(pts, _c4_create, _c4_phases, _c4_collect, device=device or "cuda:0", base_seed=42, max_concurrent=11)
+    else:
+        res = replicas.run_points(pts, _c4_point, base_seed=42, dist=dist, device=device)
     if res is None:
         return None
     out = {"config": f"c4 {L}^3, Ku=0.05, constrained, theta=0..90 deg (11 points), T in (0.3, 0.8, 1.2), {sweeps} sweeps per point", "points": []}

@@ -72,3 +72,9 @@ def test_gloo_world_sizes_give_the_same_answer(tmp_path):
         if not use_costs:
             assert ranks == [k % ws for k in range(11)]                          # round robin
         assert got["slowest"] == 10.0 + ws - 1                                   # max over ranks
+
+
+def test_split_chunks():
+    assert replicas.split_chunks(170, 50) == (3, 20) and replicas.split_chunks(0, 50) == (0, 0) and replicas.split_chunks(50, 50) == (1, 0)
+    with pytest.raises(ValueError):
+        replicas.split_chunks(10, 0)
