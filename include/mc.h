@@ -133,7 +133,12 @@ int mc_set_sweep(mc_ctx* ctx, uint64_t sweep);
 
 /* n Monte Carlo iterations of Table A1 at temperature T > 0: red pass, black pass, cone controller,
  * per-sweep reductions (acceptance, M, E) and Eq. (6) accumulators.  Asynchronous: enqueues 2n kernels on the
- * handle's stream and returns; no host synchronisation, the controller state lives on the device. */
+ * handle's stream and returns; no host synchronisation, the controller state lives on the device.
+ * CUDA graphs: the call only launches kernels on the handle's stream (no allocation, no synchronisation, no host read of device
+ * state), so it may be issued while that stream is being captured and the graph replayed any number of times (the sweep counter
+ * and the cone live on the device and advance with every replay).  The same holds for mc_reset_accumulators, mc_set_cone,
+ * mc_set_sweep, and for mc_constrained_sweep once a constrained sweep with the same (theta, phi) has run outside the capture
+ * (the first one aligns M and synchronises).  paper_2103_03517_b200/replicas.py uses this to run many small lattices at once. */
 int mc_sweep(mc_ctx* ctx, double T, int64_t n);
 
 /* n iterations of the constrained algorithm, Table A2, holding M/|M| along
