@@ -340,6 +340,23 @@ def test_full_size_march_pass_half_sweep_parity(mods):
     _full_size_half_sweep(mods, (256, 256, 256), 1.2, 1.2, 7, dict(Kc=0.01), colour=1)
 
 
+# ---------------------------------------------------------------------------------------------- f-1 domain-wall workload
+def test_domain_wall_workload_gives_the_exchange_stiffness(mods):
+    """SURVEY 8f-1 end to end: anti-periodic box, slice profiles, tanh fits, K(T) from the constrained torque,
+    A(T) = K Delta^2 / pi^2.  Checks against what the model fixes: A(T -> 0) = J/2 per lattice spacing (sc, nearest neighbours),
+    Delta(T -> 0) = pi sqrt(J / 2 K_u), and an exponent of A ~ m^k between the paper's low-temperature values and mean field
+    (Table I: 1.48 ... 1.79; MFA: 2)."""
+    from paper_2103_03517_b200 import configs
+    out = configs.dw(shape=(96, 32, 32), Ku=0.05, temps=(0.2, 0.5, 0.8, 1.0), equil=1500, snapshots=120, every=10)
+    pts = out["points"]
+    assert all(p["fits"] > 100 for p in pts)
+    assert abs(pts[0]["Delta"] / out["expected_T0"]["Delta"] - 1) < 0.06            # T = 0.2: a few per cent wider than at T = 0
+    assert all(a["Delta"] < b["Delta"] for a, b in zip(pts, pts[1:]))               # the wall widens with T (Fig. 2)
+    assert abs(out["A0_extrapolated"] / 0.5 - 1) < 0.08
+    # four points and short runs: the slope is good to about +-0.25 (the full schedule of configs.dw gives 1.76)
+    assert 1.1 < out["A_over_m_exponent_m_gt_0.6"] < 2.1, out["A_over_m_exponent_m_gt_0.6"]
+
+
 # ---------------------------------------------------------------------------------------------- f-2 lattices at bench size
 @pytest.mark.parametrize("structure,L,T,colour,ham", [
     ("bcc", 176, 1.8, 1, dict()),                    # 10.9 M spins, 8 neighbours
