@@ -219,11 +219,41 @@ def dw(device="cuda:0", shape=(160, 48, 48), Ku=0.05, temps=(0.2, 0.4, 0.6, 0.8,
     return out
 
 
+def f4(device="cuda:0", L=48, Ku=0.05, temps=(0.2, 0.4, 0.6, 0.8, 1.0, 1.2), equil=3000, samples=300, every=20):
+    """SURVEY 8f-4, the paper's second anisotropy route and its susceptibility check on observables the library already returns:
+    Eq. (4) -- K(T)/K(0) from the easy-axis anisotropy energy of a STANDARD run -- against the constrained torque route
+    ("identical results"), and Eq. (7) -- chi_perp = m^2 / (2 K(T)) -- against the transverse susceptibility of
+    Eq. (6) accumulated by the same standard run."""
+    out = {"config": f"f-4 {L}^3, Ku={Ku} along z, {equil} + {samples}x{every} sweeps per T (standard), 32^3 constrained at 45 deg", "points": []}
+    for i, T in enumerate(temps):
+        g = binding.Lattice(L, L, L, Ku=Ku, cone0=0.5, adaptive=True, seed=42 + i, device=device)
+        g.sweep(T, equil); g.reset_accumulators()
+        Ea = []
+        for _ in range(samples):
+            g.sweep(T, every); Ea.append(g.observables().E_aniso)
+        ob = g.observables(); g.close()
+        chi = analysis.susceptibilities(ob, T)
+        m = ob.sum_m[0] / ob.n_samples
+        k4 = analysis.anisotropy_scaling_easy_axis(float(np.mean(Ea)), Ku=Ku)
+        c = binding.Lattice(32, 32, 32, Ku=Ku, cone0=0.5, adaptive=True, seed=142 + i, device=device)
+        c.constrained_sweep(T, np.pi / 4, 0.0, 1500); c.reset_accumulators(); c.constrained_sweep(T, np.pi / 4, 0.0, 4000)
+        oc = c.observables(); c.close()
+        kt = -oc.sum_torque[1] / oc.n_samples / Ku
+        out["points"].append({"T": T, "m": float(m), "k_eq4": float(k4), "k_torque": float(kt), "m^2.95": float(m ** 2.95),
+                              "chi_perp_eq6": float(0.5 * (chi[1] + chi[2])), "chi_perp_eq7": float(analysis.chi_perp_uniaxial(m, Ku * k4)),
+                              "chi_l": float(chi[0])})
+    ms = np.array([p["m"] for p in out["points"]])
+    out["exponent_eq4"] = analysis.power_law_exponent(ms, np.array([p["k_eq4"] for p in out["points"]]))[0]
+    out["exponent_torque"] = analysis.power_law_exponent(ms, np.array([p["k_torque"] for p in out["points"]]))[0]
+    out["paper"] = {"uniaxial_exponent": 2.95, "where": "P:52-59, P:105"}
+    return out
+
+
 def main(argv=None):
     """python -m paper_2103_03517_b200.configs [c1 ...]; under torchrun the point loops of c2 / c4 are dealt over the ranks
     (replicas), the single-lattice configs run on rank 0 only."""
     names = (argv or sys.argv[1:]) or ["c1", "c2", "c3", "c4", "c5"]
-    table = {"c1": c1, "c2": c2, "c3": c3, "c4": c4, "c5": c5, "dw": dw}
+    table = {"c1": c1, "c2": c2, "c3": c3, "c4": c4, "c5": c5, "dw": dw, "f4": f4}
     dist = replicas.init_distributed()
     rank, local_rank, _ = replicas.world()
     dev = f"cuda:{local_rank}"

@@ -357,6 +357,18 @@ def test_domain_wall_workload_gives_the_exchange_stiffness(mods):
     assert 1.1 < out["A_over_m_exponent_m_gt_0.6"] < 2.1, out["A_over_m_exponent_m_gt_0.6"]
 
 
+# ---------------------------------------------------------------------------------------------- f-4 second anisotropy route
+def test_easy_axis_route_of_eq4_follows_the_callen_callen_law(mods):
+    """SURVEY 8f-4 end to end: K(T)/K(0) from the easy-axis anisotropy energy of a standard run (Eq. (4)) against the
+    l = 2 Callen-Callen law the paper measures (m^2.95) and against the constrained torque route ("identical results")."""
+    from paper_2103_03517_b200 import configs
+    out = configs.f4(L=32, Ku=0.05, temps=(0.3, 0.6, 0.9), equil=1500, samples=150, every=10)
+    for p in out["points"]:
+        assert abs(p["k_eq4"] - p["m^2.95"]) < 0.02, p
+        assert abs(p["k_torque"] - p["k_eq4"]) < 0.06, p
+        assert 0.3 < p["chi_perp_eq6"] / p["chi_perp_eq7"] < 3.0, p             # Eq. (7): same order (the macrospin mode is slow to sample)
+
+
 # ---------------------------------------------------------------------------------------------- f-2 lattices at bench size
 @pytest.mark.parametrize("structure,L,T,colour,ham", [
     ("bcc", 176, 1.8, 1, dict()),                    # 10.9 M spins, 8 neighbours
