@@ -175,6 +175,14 @@ template <> __device__ __forceinline__ void st_rw<4>(float* p, const Pack<4>& r)
     *reinterpret_cast<float4*>(p) = make_float4(r.v[0], r.v[1], r.v[2], r.v[3]);
 }
 
+// the same store with the evict-first ("streaming") policy: the written spins are not read again before the next pass has swept
+// the whole other colour.  Pays on the bcc pass only (176^3 cells: 98.6 -> 95.1 us per sweep, 224^3: 187.6 -> 179.5); the film
+// (159 -> 178), the march pass (89.4 -> 92.2) and the eight-colour passes (no change) keep the default policy.
+__device__ __forceinline__ void st_rw_streaming(float* p, const Pack<4>& r)
+{
+    __stcs(reinterpret_cast<float4*>(p), make_float4(r.v[0], r.v[1], r.v[2], r.v[3]));
+}
+
 // One item = VEC consecutive same-colour sites of one row.  Coordinates + neighbour offsets.
 struct ItemPos {
     uint32_t a0;        // colour-linear index of the first site

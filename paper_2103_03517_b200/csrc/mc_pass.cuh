@@ -162,7 +162,11 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
             }
         }
         if (MODE == MODE_SWEEP) {
-            st_rw<VEC>(Sc + q.a0, nxv); st_rw<VEC>(Sc + P.plane + q.a0, nyv); st_rw<VEC>(Sc + 2 * P.plane + q.a0, nzv);
+            if constexpr (LAT == 1 && VEC == 4) {
+                st_rw_streaming(Sc + q.a0, nxv); st_rw_streaming(Sc + P.plane + q.a0, nyv); st_rw_streaming(Sc + 2 * P.plane + q.a0, nzv);
+            } else {
+                st_rw<VEC>(Sc + q.a0, nxv); st_rw<VEC>(Sc + P.plane + q.a0, nyv); st_rw<VEC>(Sc + 2 * P.plane + q.a0, nzv);
+            }
         }
 #pragma unroll
         for (int k = 0; k < NQ; ++k) fs[k] += f[k];
