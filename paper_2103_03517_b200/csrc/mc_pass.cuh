@@ -162,7 +162,7 @@ pass_kernel(const __grid_constant__ Params P, const __grid_constant__ Geom G, in
             }
         }
         if (MODE == MODE_SWEEP) {
-            if constexpr (LAT == 1 && VEC == 4) {
+            if constexpr ((LAT == 1 || (LAT == 0 && !MASKED)) && VEC == 4) {          // evict-first stores: bcc +4 %, sc 128^3 +2.6 %; masked films lose 11 %
                 st_rw_streaming(Sc + q.a0, nxv); st_rw_streaming(Sc + P.plane + q.a0, nyv); st_rw_streaming(Sc + 2 * P.plane + q.a0, nzv);
             } else {
                 st_rw<VEC>(Sc + q.a0, nxv); st_rw<VEC>(Sc + P.plane + q.a0, nyv); st_rw<VEC>(Sc + 2 * P.plane + q.a0, nzv);
