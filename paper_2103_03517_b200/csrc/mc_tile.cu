@@ -5,24 +5,24 @@ namespace mc {
 namespace {
 
 typedef void (*TileFn)(const Params, const TileGeom, int, float, int, float*, uint8_t*);
-template <int RT, bool DEBUG, bool ANTI = false> TileFn pick_tile_rt(int aniso, bool field)
+template <int RT, bool DEBUG, bool ANTI = false, bool L2S = false> TileFn pick_tile_rt(int aniso, bool field)
 {
     switch (aniso * 2 + (field ? 1 : 0)) {
-        case 0: return tile_pass_kernel<0, false, RT, DEBUG, ANTI>;  case 1: return tile_pass_kernel<0, true, RT, DEBUG, ANTI>;
-        case 2: return tile_pass_kernel<1, false, RT, DEBUG, ANTI>;  case 3: return tile_pass_kernel<1, true, RT, DEBUG, ANTI>;
-        case 4: return tile_pass_kernel<2, false, RT, DEBUG, ANTI>;  case 5: return tile_pass_kernel<2, true, RT, DEBUG, ANTI>;
-        case 6: return tile_pass_kernel<3, false, RT, DEBUG, ANTI>;  default: return tile_pass_kernel<3, true, RT, DEBUG, ANTI>;
+        case 0: return tile_pass_kernel<0, false, RT, DEBUG, ANTI, L2S>;  case 1: return tile_pass_kernel<0, true, RT, DEBUG, ANTI, L2S>;
+        case 2: return tile_pass_kernel<1, false, RT, DEBUG, ANTI, L2S>;  case 3: return tile_pass_kernel<1, true, RT, DEBUG, ANTI, L2S>;
+        case 4: return tile_pass_kernel<2, false, RT, DEBUG, ANTI, L2S>;  case 5: return tile_pass_kernel<2, true, RT, DEBUG, ANTI, L2S>;
+        case 6: return tile_pass_kernel<3, false, RT, DEBUG, ANTI, L2S>;  default: return tile_pass_kernel<3, true, RT, DEBUG, ANTI, L2S>;
     }
 }
 // Row lengths with a specialised instantiation: MC_TILE_RT_LIST (mc_tile.cuh).  Any other R, the anti-periodic wrap and the
 // decision-variable debug outputs of the test hooks run the run-time-R instantiation (same arithmetic, same slab shape).
-TileFn pick_tile(int R, int Ty, int npass, bool debug, int aniso, bool field, bool anti)
+TileFn pick_tile(int R, int Ty, int npass, bool debug, int aniso, bool field, bool anti, bool stream_l2)
 {
     if (anti) return debug ? pick_tile_rt<0, true, true>(aniso, field) : pick_tile_rt<0, false, true>(aniso, field);
     if (debug) return pick_tile_rt<0, true>(aniso, field);
     if (!tile_has_rt(R) || Ty != tile_ty_rt(R) || npass != TILE_NPASS_RT) return pick_tile_rt<0, false>(aniso, field);
     switch (R) {
-#define MC_TILE_X(r) case r: return pick_tile_rt<r, false>(aniso, field);
+#define MC_TILE_X(r) case r: return stream_l2 ? pick_tile_rt<r, false, false, true>(aniso, field) : pick_tile_rt<r, false>(aniso, field);
         MC_TILE_RT_LIST(MC_TILE_X)
 #undef MC_TILE_X
         default: return pick_tile_rt<0, false>(aniso, field);
@@ -59,11 +59,16 @@ bool plan_tile(mc_ctx* c)
     G.n_slabs = lat.ny / G.Ty;
     G.slot_floats = 3 * (G.Ty + 2) * R;
     G.n_active = PR * RP;
+    {   // does the spin state (12 B per site) fit the L2?
+        int l2 = 0;
+        if (cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, c->device) != cudaSuccess) { cudaGetLastError(); l2 = 0; }
+        G.stream_l2 = (12ull * (unsigned long long)c->P.N > (unsigned long long)l2) ? 1 : 0;
+    }
     c->tile_threads = (G.n_active + 31) / 32 * 32;
     c->tile_smem = TILE_NSLOT * slot_bytes(G.Ty);
     if (c->tile_smem > 200 * 1024) return false;
     // every instantiation this handle can launch must be allowed its dynamic shared memory
-    TileFn fns[2] = { pick_tile(R, G.Ty, G.NPASS, false, c->aniso, c->field, c->P.anti_x != 0), pick_tile(R, G.Ty, G.NPASS, true, c->aniso, c->field, c->P.anti_x != 0) };
+    TileFn fns[2] = { pick_tile(R, G.Ty, G.NPASS, false, c->aniso, c->field, c->P.anti_x != 0, G.stream_l2 != 0), pick_tile(R, G.Ty, G.NPASS, true, c->aniso, c->field, c->P.anti_x != 0, G.stream_l2 != 0) };
     int per_sm = 1;
     for (TileFn f : fns) {
         if (cudaFuncSetAttribute((const void*)f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->tile_smem) != cudaSuccess) { cudaGetLastError(); return false; }
@@ -84,7 +89,7 @@ bool plan_tile(mc_ctx* c)
 
 int launch_pass_tile(mc_ctx* ctx, int colour, float invT, int flags, float* dx, uint8_t* da)
 {
-    TileFn fn = pick_tile(ctx->tgeom.R, ctx->tgeom.Ty, ctx->tgeom.NPASS, dx || da, ctx->aniso, ctx->field, ctx->P.anti_x != 0);
+    TileFn fn = pick_tile(ctx->tgeom.R, ctx->tgeom.Ty, ctx->tgeom.NPASS, dx || da, ctx->aniso, ctx->field, ctx->P.anti_x != 0, ctx->tgeom.stream_l2 != 0);
     const int grid = ctx->tgeom.n_slabs * ctx->tgeom.n_segs;
     MC_CU(launch_dependent(fn, grid, ctx->tile_threads, ctx->tile_smem, ctx->stream, ctx->P, ctx->tgeom, colour, invT, flags, dx, da));
     ctx->launches += 1;

@@ -68,6 +68,7 @@ struct TileGeom {
     int Lz, Lz_rem;            // segment s covers Lz + (s < Lz_rem ? 1 : 0) planes
     int slot_floats;           // 3 * (Ty + 2) * R
     int n_active;              // PR * RP working threads (block size is this rounded up to a warp multiple)
+    int stream_l2;             // 1: the spin state does not fit the L2 (the specialised instantiations then copy with the evict-first policy)
 };
 
 // ---- packed two-wide fp32 helpers (FFMA2 / FADD2 / FMUL2 on sm_100a)
@@ -95,15 +96,28 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
         "MC_DONE:\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
 }
+// L2S: the plane copies carry the evict-first L2 policy.  For lattices whose spin state does not fit the L2: the other colour
+// streams through it (each row is wanted again only by the neighbouring slabs and segments, at about the same time), 224^3:
+// 86.5 -> 84.9 us per sweep.  A lattice that fits loses with it (192^3: 54.0 -> 57.2: the next pass would have found the rows
+// cached), so the choice is a template parameter resolved by the planner, not a run-time branch in the copy.
+template <bool L2S>
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
 {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+    if constexpr (L2S) {
+        unsigned long long pol;
+        asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                     ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+    } else {
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+    }
 }
 
 // One plane (Ty + 2 rows x 3 components, periodic wrap in y) of the other colour -> one ring slot, issued by ONE thread.
 // Rows that are consecutive in y are consecutive in HBM and in the slot, so a slab in the interior of the lattice
 // needs one bulk copy per component; a slab touching y = 0 or y = ny-1 needs one more per wrapped row.
+template <bool L2S>
 __device__ __forceinline__ void tile_issue_plane(const TileGeom& G, int R, const float* __restrict__ Oth, long long plane, int z, int y0,
                                                  uint32_t slot_addr, uint32_t bar)
 {
@@ -118,7 +132,7 @@ __device__ __forceinline__ void tile_issue_plane(const TileGeom& G, int R, const
         int run = nrows - ry; if (run > G.ny - y) run = G.ny - y;
 #pragma unroll
         for (int comp = 0; comp < 3; ++comp)
-            bulk_g2s(slot_addr + (uint32_t)(comp * nrows + ry) * row_bytes, zbase + (long long)comp * plane + (long long)y * R,
+            bulk_g2s<L2S>(slot_addr + (uint32_t)(comp * nrows + ry) * row_bytes, zbase + (long long)comp * plane + (long long)y * R,
                      (uint32_t)run * row_bytes, bar);
         ry += run;
     }
@@ -137,7 +151,7 @@ __device__ __forceinline__ float mantissa_1p(uint32_t w) { return __uint_as_floa
 // (S.e)^2 and its difference form.
 // ANTI: anti-periodic boundary along x (domain-wall box; C-27): the one x-neighbour a pair reads across the row
 // end enters with the opposite sign.  Instantiated for the run-time row length only.
-template <int ANISO, bool FIELD, int RT, bool DEBUG, bool ANTI = false>
+template <int ANISO, bool FIELD, int RT, bool DEBUG, bool ANTI = false, bool L2S = false>
 __global__ void __launch_bounds__(tile_threads_rt(RT), tile_blocks_rt(RT))
 tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileGeom G, int colour, float invT, int flags,
                   float* __restrict__ dbg_x, uint8_t* __restrict__ dbg_acc)
@@ -176,7 +190,7 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
         const int nseq = Lz + 2 < TILE_NSLOT ? Lz + 2 : TILE_NSLOT;
         for (int k = 0; k < nseq; ++k) {
             int z = z0 - 1 + k; if (z < 0) z += G.nz; else if (z >= G.nz) z -= G.nz;
-            tile_issue_plane(G, R, Oth, P.plane, z, y0, smem_base + (uint32_t)k * slot_bytes, bar_base + 8u * k);
+            tile_issue_plane<L2S>(G, R, Oth, P.plane, z, y0, smem_base + (uint32_t)k * slot_bytes, bar_base + 8u * k);
         }
     }
     __syncthreads();
@@ -323,7 +337,7 @@ tile_pass_kernel(const __grid_constant__ Params P, const __grid_constant__ TileG
             const int k = j + TILE_NSLOT;
             int zn = z0 - 1 + k; if (zn >= G.nz) zn -= G.nz;
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-            tile_issue_plane(G, R, Oth, P.plane, zn, y0, smem_base + (uint32_t)(k & 3) * slot_bytes, bar_base + 8u * (k & 3));
+            tile_issue_plane<L2S>(G, R, Oth, P.plane, zn, y0, smem_base + (uint32_t)(k & 3) * slot_bytes, bar_base + 8u * (k & 3));
         }
     }
 
