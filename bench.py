@@ -159,18 +159,24 @@ def run_reference(args, rank, world):
 
 
 def time_other_paths(binding, torch, local_rank, sweeps=100):
-    """Constrained pair sweeps (Table A2) on the 224^3 lattice: CUDA events on the handle's stream, state resident."""
+    """The other rows of the hot-path table: CUDA events on the handle's stream, state resident; per row 200 warm-up sweeps (the legs are separated by host-side set-up during which the GPU
+    idles and drops its clocks), then the best of three timed runs of `sweeps` sweeps (context numbers next to the headline, whose own protocol is the contract's)."""
     out = {}
+
+    def best_ms(run, warm):
+        warm(); torch.cuda.synchronize()
+        best = None
+        for _ in range(3):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); run(); b.record(); torch.cuda.synchronize()
+            t = a.elapsed_time(b); best = t if best is None else min(best, t)
+        return best
     g = binding.Lattice(*SHAPE, Ku=0.05, cone0=0.5, adaptive=True, seed=42, device=f"cuda:{local_rank}")
-    g.constrained_sweep(0.8, 0.6, 0.0, 20)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(); g.constrained_sweep(0.8, 0.6, 0.0, sweeps); e1.record(); torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1)
+    ms = best_ms(lambda: g.constrained_sweep(0.8, 0.6, 0.0, sweeps), lambda: g.constrained_sweep(0.8, 0.6, 0.0, 200))
     N = SHAPE[0] * SHAPE[1] * SHAPE[2]
     ups = N * sweeps / (ms * 1e-3)
     out["constrained_224^3_Ku0.05_T0.8_theta0.6"] = {"value": ups, "unit": UNIT, "us_per_sweep": 1e3 * ms / sweeps,
-                                                     "algorithmic_GBs": BYTES_PER_UPDATE * ups / 1e9, "kernel": "pair_kernel (generic, not tiled yet)"}
+                                                     "algorithmic_GBs": BYTES_PER_UPDATE * ups / 1e9, "kernel": "pair_kernel<4, uniaxial> (gather; compile-time in-group rotation, 4 x 128 threads per SM)"}
     g.close()
     # granular film c5 (BASELINE.json configs[4]): 2048 x 2048 x 4, Voronoi grains, J = 0 across grains, per-grain axes
     from paper_2103_03517_b200 import inputs
@@ -178,10 +184,7 @@ def time_other_paths(binding, torch, local_rank, sweeps=100):
     mask, region, axes = inputs.voronoi_film(nx, ny, nz, 40, seed=42)
     g = binding.Lattice(nx, ny, nz, periodic=(1, 1, 0), Ku=0.02, bond_mask=mask, region=region, region_axis=axes,
                         cone0=0.5, adaptive=True, seed=42, device=f"cuda:{local_rank}")
-    g.sweep(0.5, 10)
-    torch.cuda.synchronize()
-    e0.record(); g.sweep(0.5, sweeps); e1.record(); torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1)
+    ms = best_ms(lambda: g.sweep(0.5, sweeps), lambda: g.sweep(0.5, 200))
     N5 = nx * ny * nz
     ups = N5 * sweeps / (ms * 1e-3)
     out["c5_film_2048x2048x4_T0.5"] = {"value": ups, "unit": UNIT, "us_per_sweep": 1e3 * ms / sweeps, "algorithmic_GBs": 39 * ups / 1e9,
@@ -190,18 +193,14 @@ def time_other_paths(binding, torch, local_rank, sweeps=100):
     # bcc lattice: 176^3 conventional cells = 10.9 M spins, 8 neighbours, the two sublattices as colours
     Lb = 176
     g = binding.Lattice(Lb, Lb, Lb, Ku=0.01, cone0=0.5, adaptive=True, seed=42, structure="bcc", device=f"cuda:{local_rank}")
-    g.init_spins(2); g.sweep(1.8, 10)
-    torch.cuda.synchronize()
-    e0.record(); g.sweep(1.8, sweeps); e1.record(); torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1)
+    g.init_spins(2)
+    ms = best_ms(lambda: g.sweep(1.8, sweeps), lambda: g.sweep(1.8, 200))
     ups = g.N * sweeps / (ms * 1e-3)
     out["bcc_176^3_cells_Ku0.01_T1.8"] = {"value": ups, "unit": UNIT, "us_per_sweep": 1e3 * ms / sweeps, "algorithmic_GBs": BYTES_PER_UPDATE * ups / 1e9,
                                         "kernel": "pass_kernel<4, uniaxial, bcc> (generic gather, 8 neighbours)"}
     # the constrained pair pass on the same bcc lattice (Table A2 with the 8-bond field)
-    g.init_spins(0); g.constrained_sweep(0.8, 0.6, 0.0, 10)
-    torch.cuda.synchronize()
-    e0.record(); g.constrained_sweep(0.8, 0.6, 0.0, sweeps); e1.record(); torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1)
+    g.init_spins(0)
+    ms = best_ms(lambda: g.constrained_sweep(0.8, 0.6, 0.0, sweeps), lambda: g.constrained_sweep(0.8, 0.6, 0.0, 200))
     ups = g.N * sweeps / (ms * 1e-3)
     out["bcc_constrained_176^3_cells_T0.8_theta0.6"] = {"value": ups, "unit": UNIT, "us_per_sweep": 1e3 * ms / sweeps, "algorithmic_GBs": BYTES_PER_UPDATE * ups / 1e9,
                                                       "kernel": "pair_kernel<4, uniaxial, bcc>"}
@@ -209,10 +208,8 @@ def time_other_paths(binding, torch, local_rank, sweeps=100):
     # fcc lattice: 140^3 conventional cells = 11.0 M spins, 12 neighbours, FOUR colour passes per sweep
     Lf = 140
     g = binding.Lattice(Lf, Lf, Lf, Ku=0.01, cone0=0.5, adaptive=True, seed=42, structure="fcc", device=f"cuda:{local_rank}")
-    g.init_spins(2); g.sweep(2.8, 10)
-    torch.cuda.synchronize()
-    e0.record(); g.sweep(2.8, sweeps); e1.record(); torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1)
+    g.init_spins(2)
+    ms = best_ms(lambda: g.sweep(2.8, sweeps), lambda: g.sweep(2.8, 200))
     ups = g.N * sweeps / (ms * 1e-3)
     out["fcc_140^3_cells_Ku0.01_T2.8"] = {"value": ups, "unit": UNIT, "us_per_sweep": 1e3 * ms / sweeps, "algorithmic_GBs": 60 * ups / 1e9,
                                         "kernel": "pass_kernel<4, uniaxial, fcc, colour> (generic gather, colour as a compile-time constant, 12 neighbours, 4 passes per sweep; 60 B per update: each pass reads the three other sublattices)"}
@@ -222,10 +219,8 @@ def time_other_paths(binding, torch, local_rank, sweeps=100):
     for name, kw, T in (("hcp", dict(), 2.8), ("sc_nnn", dict(J2=0.3), 2.0)):
         Lc = 176
         g = binding.Lattice(Lc, Lc, Lc, Ku=0.01, cone0=0.5, adaptive=True, seed=42, structure=name, device=f"cuda:{local_rank}", **kw)
-        g.init_spins(2); g.sweep(T, 10)
-        torch.cuda.synchronize()
-        e0.record(); g.sweep(T, sweeps); e1.record(); torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1)
+        g.init_spins(2)
+        ms = best_ms(lambda: g.sweep(T, sweeps), lambda: g.sweep(T, 200))
         ups = g.N * sweeps / (ms * 1e-3)
         out[f"{name}_176^3_cells_Ku0.01_T{T}"] = {"value": ups, "unit": UNIT, "us_per_sweep": 1e3 * ms / sweeps, "algorithmic_GBs": 96 * ups / 1e9,
                                               "kernel": "pass_kernel<4, uniaxial, structure, colour> (gather through the bond table of the sublattice as a compile-time constant: 12 / 18 bonds, 8 passes per sweep; 96 B per update)"}
@@ -269,6 +264,9 @@ def time_other_paths(binding, torch, local_rank, sweeps=100):
     work = 16 * 64 ** 3 * 1000
     out["c2_16_points_64^3_concurrent"] = {"value": work / t_conc, "unit": UNIT, "seconds": t_conc, "one_after_another": work / t_ser,
                                            "kernel": "tile_pass_kernel<1, 0, 32> on 16 streams, 50-sweep CUDA graphs replayed round robin; wall clock incl. handle creation, capture and read-back"}
+    out["note"] = ("these legs run back to back after the headline: by then the GPU sits at its software power cap (SM clock ~1780 instead of "
+                   "1965 MHz after about a second of continuous load), so they are SUSTAINED figures; each kernel timed alone for ~0.2 s "
+                   "(BASELINE.md section 4, profiles/) runs 5-10 % faster")
     return out
 
 
